@@ -1,0 +1,157 @@
+/* qsl.h -- C ABI of libqsl: B200-native (sm_100a) field-line tracing, squashing factor Q, field-line length L,
+ * FLEDGE edge maps and adaptive seed refinement, after Tassev & Savcheva, "QSL Squasher" (arXiv:1609.00724).
+ * Citations are "PAPER.md:<line>" of the paper text plus the section / equation they fall in; readings of silent
+ * or ambiguous passages (A1..A14) are listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Every function returns int: 0 = QSL_OK, < 0 = error (see qsl_strerror).  Nothing throws or aborts across the ABI.
+ *  - Unless marked "host", every array argument is a DEVICE pointer owned by the caller (e.g. torch.Tensor.data_ptr());
+ *    the library neither frees nor retains it.  The one exception is qsl_field_create, which copies its input into a
+ *    library-owned packed buffer released by qsl_field_destroy.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are asynchronous on that
+ *    stream except where a count is returned to the host (qsl_refine's n_children), which synchronises the stream.
+ *    Scratch memory is taken from the stream-ordered CUDA memory pool of the current device.
+ *  - Per-line problems are not errors: they are bits of the per-seed `status` output.
+ *  - There is no CPU fallback: without a CUDA device every compute entry point returns QSL_ECUDA.
+ */
+#ifndef QSL_H
+#define QSL_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes ------------------------------------------------------------------------------------------ */
+#define QSL_OK       0
+#define QSL_EINVAL  (-1)   /* bad argument (NULL pointer, size < minimum, unknown enum, inconsistent sizes)       */
+#define QSL_ENOMEM  (-2)   /* device or host allocation failed                                                    */
+#define QSL_ECUDA   (-3)   /* a CUDA runtime call failed (qsl_last_cuda_error() gives the cudaError_t)             */
+#define QSL_ERANGE  (-4)   /* a size exceeds what the implementation indexes (e.g. > 2^31 - 1 nodes per axis)      */
+const char *qsl_strerror(int code);
+int qsl_last_cuda_error(void);
+/* Library version and the SM architecture the kernels were compiled for (e.g. 100 for sm_100a). */
+int qsl_version(void);
+int qsl_compiled_arch(void);
+
+/* ---- enums ------------------------------------------------------------------------------------------------ */
+enum { QSL_F32 = 0, QSL_F64 = 1 };                       /* storage type of the packed field samples             */
+enum { QSL_NORMALIZE_FIRST = 0, QSL_INTERP_FIRST = 1 };  /* PAPER.md:178 (fn. 9) = NORMALIZE_FIRST, the default   */
+enum { QSL_RK4 = 0, QSL_EULER = 1 };                     /* PAPER.md:141; RK4: BASELINE.json configs (reading A5) */
+enum { QSL_TRACE_L = 0, QSL_TRACE_LQ = 1 };              /* L only (FLEDGE pass) | L and Q                        */
+enum { QSL_ARITH_F64 = 0, QSL_ARITH_F32 = 1 };           /* arithmetic of the integrator (F32 only with F32 samples) */
+
+/* status bits of qsl_trace_out.status */
+#define QSL_ST_SEED_OUTSIDE 1u    /* seed not inside the closed trace box: all outputs NaN / 255 / 0             */
+#define QSL_ST_NULL_AT_SEED 2u    /* |b(seed)| < null_eps: all outputs NaN / 255 / 0                             */
+#define QSL_ST_STALL_F      4u    /* |b| < null_eps met while integrating forwards (line stops there, face 255)   */
+#define QSL_ST_STALL_B      8u
+#define QSL_ST_CAP_F        16u   /* max_steps or max_length reached forwards                      */
+#define QSL_ST_CAP_B        32u
+#define QSL_ST_OPEN         64u   /* an end lies on a face other than -z of the trace box     */
+
+/* tuning flags of qsl_trace_params.flags (results never depend on them) */
+#define QSL_FLAG_NO_SORT    1u    /* do not Morton-order the seeds before tracing                                  */
+#define QSL_FLAG_NO_REFILL  2u    /* one work item per thread instead of the persistent work queue                 */
+#define QSL_FLAG_KERNEL_V1  4u    /* baseline kernel: 8 AoS gathers per RK stage, no per-thread cell cache         */
+
+/* ---- field (PAPER.md:54 input cubes; :93-107 eq. 3-4 interpolation; :178 normalise-then-interpolate) --------- */
+typedef struct qsl_field qsl_field;          /* opaque, library-owned */
+
+typedef struct {
+    int nx, ny, nz;              /* nodes per axis, each >= 2; sample index = (k*ny + j)*nx + i (x fastest)      */
+    int stretched;               /* 0: uniform nodes lo + i (hi - lo)/(n - 1); 1: node coordinates xs, ys, zs     */
+    double lo[3], hi[3];         /* grid box (ignored when stretched: taken from the coordinate arrays)           */
+    const double *xs, *ys, *zs;  /* HOST arrays of nx, ny, nz strictly increasing coordinates; only if stretched  */
+    int sample_type;             /* QSL_F32 | QSL_F64: storage type of the packed samples                         */
+    int interp_mode;             /* QSL_NORMALIZE_FIRST (paper) | QSL_INTERP_FIRST (reading A2)                   */
+} qsl_grid_desc;
+
+/* Packs the three component cubes (DEVICE, fp64, nx*ny*nz each) into one AoS array of (b^x, b^y, b^z, |B|) samples
+ * [NORMALIZE_FIRST] or (Bx, By, Bz, |B|) [INTERP_FIRST], rounded to sample_type: inputs are first rounded to
+ * sample_type, |B| and B/|B| are formed in fp64 with IEEE sqrt / division, then rounded; |B| < 1e-300 gives zeros.
+ * Errors: QSL_EINVAL (NULL, n < 2, non-increasing coordinates, unknown enum), QSL_ERANGE, QSL_ENOMEM, QSL_ECUDA.  */
+int qsl_field_create(qsl_field **out, const qsl_grid_desc *desc, const double *bx, const double *by,
+                     const double *bz, void *stream);
+int qsl_field_destroy(qsl_field *f);
+/* Test hook: copies the packed samples (nx*ny*nz*4 values of sample_type) to `packed_out` (DEVICE). */
+int qsl_field_export(const qsl_field *f, void *packed_out, void *stream);
+/* Bytes of device memory held by the field. */
+long long qsl_field_bytes(const qsl_field *f);
+
+/* ---- trace (PAPER.md:79 eq. 1; :119 eq. 5; :141 integrators; :156-176 eq. 9-11 Q; :163 boundaries; :165 cap) --- */
+typedef struct {
+    double box_lo[3], box_hi[3]; /* trace box, inside the grid box; may be smaller (raised lower boundary) */
+    int method;                  /* QSL_RK4 | QSL_EULER                                                            */
+    double step_frac;            /* h = step_frac * min_d h_c,d of the cell containing x; > 0   */
+    int mode;                    /* QSL_TRACE_L | QSL_TRACE_LQ                                                      */
+    int arith;                   /* QSL_ARITH_F64 | QSL_ARITH_F32                                                   */
+    double max_length;           /* cap on the affine parameter lambda per direction; +inf = off     */
+    long long max_steps;         /* cap on accepted steps per direction; >= 1                                       */
+    double null_eps;             /* stall threshold on |b|                                                          */
+    unsigned int flags;          /* QSL_FLAG_*                                                                      */
+} qsl_trace_params;
+
+typedef struct {                 /* every member may be NULL (output not wanted); n = number of seeds               */
+    double *end_f, *end_b;       /* n*3: end points forwards (along +B) / backwards                                 */
+    double *L;                   /* n: field-line length L_F + L_B                              */
+    double *q_perp;              /* n: eq. (11) verbatim, field-perpendicular projections            */
+    double *q_bnd;               /* n: the same bracket with projections along the field onto the end faces and the
+                                    normal field components (Titov's Q for face-to-face mapping; reading A1)        */
+    unsigned char *face_f, *face_b;       /* n: 0..5 = -x,+x,-y,+y,-z,+z of the trace box; 255 = none (stall / cap) */
+    unsigned int *status;        /* n: QSL_ST_* bits                                                                */
+    unsigned int *nsteps_f, *nsteps_b;    /* n: accepted steps per direction (the landing step counts once)         */
+    double *dev_f, *dev_b;       /* n*6: raw deviation vectors (delta1, delta2) at each end (QSL_TRACE_LQ only)      */
+} qsl_trace_out;
+
+/* Traces n seeds (DEVICE, n*3 fp64) forwards and backwards and writes the requested outputs in seed order.
+ * total_steps (DEVICE, optional) receives the number of accepted RK steps summed over all lines and directions.
+ * n = 0 is valid.  Errors: QSL_EINVAL, QSL_ENOMEM, QSL_ECUDA.                                                       */
+int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long long n, const double *seeds,
+              const qsl_trace_out *out, unsigned long long *total_steps, void *stream);
+
+/* ---- FLEDGE (Sobel gradient magnitude of the field-line-length map; reading A10) ----------------- */
+typedef struct {
+    int ndim;                    /* 2 or 3                                                                          */
+    long long n[3];              /* level-0 seed lattice dims (n[2] = 1 for 2-D)                                    */
+    double origin[3], e0[3], e1[3], e2[3];  /* seed(c) at level l = origin + sum_d (c_d + 0.5)/(n_d 2^l) e_d         */
+} qsl_lattice;
+
+typedef struct {
+    const qsl_lattice *lat;      /* host                                                                            */
+    int nlevels;                 /* number of levels described, >= level + 1                                        */
+    const double *L0;            /* DEVICE, dense level-0 map, index (c2*n1 + c1)*n0 + c0                           */
+    const long long *count;      /* host [nlevels]; count[0] ignored (level 0 is dense)                             */
+    const unsigned int *const *coords;  /* host array [nlevels] of DEVICE pointers: count[l]*ndim integer coords at
+                                           level l, in the order qsl_refine emitted them; [0] ignored                */
+    const double *const *L;      /* host array [nlevels] of DEVICE pointers: count[l] lengths; [0] ignored          */
+    const long long *const *child_base; /* host array [nlevels] of DEVICE pointers: child_base[l][i] = index at level
+                                           l+1 of the first of the 2^ndim children of cell i of level l, or -1 if the
+                                           cell was not refined (as written by qsl_refine); entries for l >= level
+                                           are not read                                                              */
+} qsl_levels;
+
+/* Dense map: dims d0 x d1 (x d2), index (c2*d1 + c1)*d0 + c0.  S = sqrt(sum_d G_d^2), G_d = difference [-1,0,1] along
+ * d, smoothing [1,2,1] along the other axes, un-normalised, edges replicated.  Non-finite L propagates to S.       */
+int qsl_fledge_dense(int ndim, const long long dims[3], const double *L, double *S, void *stream);
+/* Sparse level >= 1: the same stencil on the virtual lattice n_d 2^level, a missing neighbour takes the L of its
+ * nearest existing ancestor (level 0 is dense).  S (DEVICE) has count[level] entries.                              */
+int qsl_fledge_sparse(const qsl_levels *lv, int level, double *S, void *stream);
+
+/* ---- threshold and refinement (BASELINE.json configs[2],[4]; reading A11) --------------------- */
+/* tau (DEVICE, 1 double) = the ceil(p N)-th smallest of the N finite values of S (nearest rank); NaN if N = 0.       */
+int qsl_select(long long n, const double *S, double p, double *tau, void *stream);
+/* For each cell i with S[i] > *tau (NaN never flags), in input order, emits 2^ndim children: coord' = 2 coord + bit
+ * (child-index bit d -> axis d) and position = origin + sum_d w_d e_d, w_d = (coord'_d + 0.5)/(n_d 2^(level+1)),
+ * accumulated with fma, axis 0 first (bit-reproducible).  coords = NULL means "the dense level-0 lattice in index
+ * order" (then level must be 0 and n = n0*n1*n2).  tau is a DEVICE pointer (as written by qsl_select).
+ * child_coords (n_out*ndim), child_seeds (n_out*3) hold up to capacity children; child_base (n, optional) receives the
+ * index of each cell's first child or -1.  n_children (host) is written after synchronising the stream; if it exceeds
+ * `capacity` nothing beyond capacity was written and QSL_ERANGE is returned (call again with larger buffers).       */
+int qsl_refine(int ndim, int level, long long n, const unsigned int *coords, const double *S, const double *tau,
+               const qsl_lattice *lat, long long capacity, unsigned int *child_coords, double *child_seeds,
+               long long *child_base, long long *n_children, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QSL_H */

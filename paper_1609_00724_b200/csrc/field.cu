@@ -1,0 +1,193 @@
+// Field packing and library plumbing.
+// PAPER.md:178 (fn. 9): "To speed up the code, we first normalize the magnetic field data cubes, and only then
+// interpolate them"; B_F, B_B, B_0 are unnormalised magnitudes, so |B| rides along as the 4th sample.
+#include <math.h>
+#include <new>
+
+#include "qsl_internal.cuh"
+
+namespace qsl {
+
+int g_last_cuda_error = 0;
+int record_cuda(cudaError_t e)
+{
+    g_last_cuda_error = (int)e;
+    cudaGetLastError();  // clear the sticky-free error state
+    return e == cudaErrorMemoryAllocation ? QSL_ENOMEM : QSL_ECUDA;
+}
+
+int scratch_alloc(void **p, size_t bytes, cudaStream_t s)
+{
+    static bool pool_set = false;
+    if (!pool_set) {
+        int dev = 0;
+        cudaMemPool_t pool;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            uint64_t keep = UINT64_MAX;  // keep freed scratch in the pool: repeated calls never go back to the OS
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        pool_set = true;
+    }
+    if (bytes == 0) bytes = 16;
+    QSL_CUDA(cudaMallocAsync(p, bytes, s));
+    return QSL_OK;
+}
+void scratch_free(void *p, cudaStream_t s)
+{
+    if (p) cudaFreeAsync(p, s);
+}
+
+int sm_count()
+{
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            n = 148;
+    }
+    return n;
+}
+
+// One thread per node.  All arithmetic is explicit-rounding fp64 (no FMA contraction) so that the packed samples are
+// bit-identical to the definition in qsl.h: round inputs to the storage type, m = sqrt((bx*bx + by*by) + bz*bz),
+// v = B/m (IEEE), round.
+template <typename S4, typename S>
+__global__ void __launch_bounds__(256) pack_kernel(long long n, const double *__restrict__ bx, const double *__restrict__ by,
+                                                   const double *__restrict__ bz, int interp_mode, S4 *__restrict__ out)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (; p < n; p += stride) {
+        const double x = (double)(S)bx[p], y = (double)(S)by[p], z = (double)(S)bz[p];
+        double m = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z)));
+        double vx = x, vy = y, vz = z;
+        if (interp_mode == QSL_NORMALIZE_FIRST) {
+            if (m < 1e-300) { vx = vy = vz = 0.0; m = 0.0; }
+            else { vx = __ddiv_rn(x, m); vy = __ddiv_rn(y, m); vz = __ddiv_rn(z, m); }
+        }
+        S4 o;
+        o.x = (S)vx; o.y = (S)vy; o.z = (S)vz; o.w = (S)m;
+        out[p] = o;
+    }
+}
+
+}  // namespace qsl
+
+using namespace qsl;
+
+extern "C" {
+
+const char *qsl_strerror(int code)
+{
+    switch (code) {
+        case QSL_OK: return "ok";
+        case QSL_EINVAL: return "invalid argument";
+        case QSL_ENOMEM: return "out of memory";
+        case QSL_ECUDA: return "CUDA runtime error (see qsl_last_cuda_error)";
+        case QSL_ERANGE: return "size out of range";
+        default: return "unknown error";
+    }
+}
+int qsl_last_cuda_error(void) { return g_last_cuda_error; }
+int qsl_version(void) { return 100; }
+int qsl_compiled_arch(void)
+{
+#ifdef QSL_TARGET_ARCH
+    return QSL_TARGET_ARCH;
+#else
+    return 0;
+#endif
+}
+
+int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, const double *by, const double *bz,
+                     void *stream)
+{
+    if (!out || !d || !bx || !by || !bz) return QSL_EINVAL;
+    *out = nullptr;
+    if (d->nx < 2 || d->ny < 2 || d->nz < 2) return QSL_EINVAL;
+    if (d->sample_type != QSL_F32 && d->sample_type != QSL_F64) return QSL_EINVAL;
+    if (d->interp_mode != QSL_NORMALIZE_FIRST && d->interp_mode != QSL_INTERP_FIRST) return QSL_EINVAL;
+    const long long n = (long long)d->nx * d->ny * d->nz;
+    if (n >= (1ll << 31)) return QSL_ERANGE;   // node index is 32-bit inside the gather
+    const int dims[3] = { d->nx, d->ny, d->nz };
+    const double *host_axes[3] = { d->xs, d->ys, d->zs };
+    if (d->stretched) {
+        for (int a = 0; a < 3; ++a) {
+            if (!host_axes[a]) return QSL_EINVAL;
+            for (int i = 1; i < dims[a]; ++i)
+                if (!(host_axes[a][i] > host_axes[a][i - 1])) return QSL_EINVAL;
+        }
+    } else {
+        for (int a = 0; a < 3; ++a)
+            if (!(d->hi[a] > d->lo[a])) return QSL_EINVAL;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    qsl_field *f = new (std::nothrow) qsl_field();
+    if (!f) return QSL_ENOMEM;
+    f->d_samples = nullptr;
+    for (int a = 0; a < 3; ++a) f->d_axis[a] = nullptr;
+    f->sample_type = d->sample_type;
+    f->n_nodes = n;
+    const size_t sbytes = (size_t)n * 4 * (d->sample_type == QSL_F32 ? 4 : 8);
+    f->bytes = sbytes;
+    cudaError_t e = cudaMalloc(&f->d_samples, sbytes);
+    if (e != cudaSuccess) { delete f; return record_cuda(e); }
+    FieldView &v = f->view;
+    v.samples = f->d_samples;
+    v.nx = d->nx; v.ny = d->ny; v.nz = d->nz;
+    v.stretched = d->stretched ? 1 : 0;
+    v.interp_mode = d->interp_mode;
+    for (int a = 0; a < 3; ++a) {
+        // node coordinates: given (stretched) or lo + i*h (uniform), always resident for the locate of the stretched path
+        double *tmp = new (std::nothrow) double[dims[a]];
+        if (!tmp) { qsl_field_destroy(f); return QSL_ENOMEM; }
+        if (d->stretched) {
+            for (int i = 0; i < dims[a]; ++i) tmp[i] = host_axes[a][i];
+            v.lo[a] = tmp[0]; v.hi[a] = tmp[dims[a] - 1];
+        } else {
+            v.lo[a] = d->lo[a]; v.hi[a] = d->hi[a];
+            const double h = (d->hi[a] - d->lo[a]) / (double)(dims[a] - 1);
+            for (int i = 0; i < dims[a]; ++i) tmp[i] = d->lo[a] + (double)i * h;
+        }
+        v.h[a] = (v.hi[a] - v.lo[a]) / (double)(dims[a] - 1);
+        e = cudaMalloc(&f->d_axis[a], sizeof(double) * dims[a]);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(f->d_axis[a], tmp, sizeof(double) * dims[a], cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);   // tmp is pageable host memory
+        delete[] tmp;
+        if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+        v.axis[a] = f->d_axis[a];
+        f->bytes += sizeof(double) * dims[a];
+    }
+    const int threads = 256;
+    const int blocks = (int)((n + threads - 1) / threads < (long long)sm_count() * 16 ? (n + threads - 1) / threads : (long long)sm_count() * 16);
+    if (d->sample_type == QSL_F32)
+        pack_kernel<float4, float><<<blocks, threads, 0, s>>>(n, bx, by, bz, d->interp_mode, (float4 *)f->d_samples);
+    else
+        pack_kernel<double4, double><<<blocks, threads, 0, s>>>(n, bx, by, bz, d->interp_mode, (double4 *)f->d_samples);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+    *out = f;
+    return QSL_OK;
+}
+
+int qsl_field_destroy(qsl_field *f)
+{
+    if (!f) return QSL_OK;
+    if (f->d_samples) cudaFree(f->d_samples);
+    for (int a = 0; a < 3; ++a)
+        if (f->d_axis[a]) cudaFree(f->d_axis[a]);
+    delete f;
+    return QSL_OK;
+}
+
+int qsl_field_export(const qsl_field *f, void *packed_out, void *stream)
+{
+    if (!f || !packed_out) return QSL_EINVAL;
+    const size_t sbytes = (size_t)f->n_nodes * 4 * (f->sample_type == QSL_F32 ? 4 : 8);
+    QSL_CUDA(cudaMemcpyAsync(packed_out, f->d_samples, sbytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return QSL_OK;
+}
+
+long long qsl_field_bytes(const qsl_field *f) { return f ? (long long)f->bytes : 0; }
+
+}  // extern "C"

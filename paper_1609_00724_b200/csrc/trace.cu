@@ -1,0 +1,67 @@
+// qsl_trace: host entry point.  Orders the seeds, runs the trace kernel over 2n work items
+// (one per direction), then the Q/L epilogue, all asynchronously on the caller's stream.
+#include <math.h>
+
+#include "trace_kernels.cuh"
+
+namespace qsl {
+cudaError_t launch_trace_f32(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
+cudaError_t launch_trace_f64(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
+cudaError_t launch_epilogue_f32(const EpilogueArgs &E, cudaStream_t s);
+cudaError_t launch_epilogue_f64(const EpilogueArgs &E, cudaStream_t s);
+}  // namespace qsl
+
+using namespace qsl;
+
+extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long long n, const double *seeds,
+                         const qsl_trace_out *out, unsigned long long *total_steps, void *stream)
+{
+    if (!f || !p || !out || n < 0 || (n > 0 && !seeds)) return QSL_EINVAL;
+    if (p->method != QSL_RK4 && p->method != QSL_EULER) return QSL_EINVAL;
+    if (p->mode != QSL_TRACE_L && p->mode != QSL_TRACE_LQ) return QSL_EINVAL;
+    if (p->arith != QSL_ARITH_F64 && p->arith != QSL_ARITH_F32) return QSL_EINVAL;
+    if (p->arith == QSL_ARITH_F32) return QSL_EINVAL;   // throughput mode not built yet
+    if (!(p->step_frac > 0.0) || p->max_steps < 1 || !(p->max_length > 0.0) || !(p->null_eps >= 0.0)) return QSL_EINVAL;
+    for (int d = 0; d < 3; ++d)
+        if (!(p->box_hi[d] >= p->box_lo[d])) return QSL_EINVAL;
+    if (n >= (1ll << 31)) return QSL_ERANGE;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (total_steps) QSL_CUDA(cudaMemsetAsync(total_steps, 0, sizeof(unsigned long long), s));
+    if (n == 0) return QSL_OK;
+
+    TraceArgs A;
+    A.fv = f->view;
+    for (int d = 0; d < 3; ++d) {
+        A.inv_h[d] = 1.0 / f->view.h[d];
+        A.box_lo[d] = p->box_lo[d]; A.box_hi[d] = p->box_hi[d];
+    }
+    A.h_uniform = p->step_frac * fmin(f->view.h[0], fmin(f->view.h[1], f->view.h[2]));
+    A.step_frac = p->step_frac; A.max_length = p->max_length; A.null_eps = p->null_eps;
+    A.max_steps = p->max_steps > 0xffffffffll ? 0xffffffffll : p->max_steps;
+    A.method = p->method;
+    const bool refill = !(p->flags & QSL_FLAG_NO_REFILL);
+    A.interleave = refill ? 1 : 0;
+    A.n = n; A.seeds = seeds; A.total_steps = total_steps;
+
+    void *perm = nullptr, *rec = nullptr, *queue = nullptr;
+    int rc = scratch_alloc(&perm, sizeof(uint32_t) * (size_t)n, s);
+    if (rc == QSL_OK) rc = scratch_alloc(&rec, sizeof(double) * REC_DOUBLES * 2 * (size_t)n, s);
+    if (rc == QSL_OK) rc = scratch_alloc(&queue, sizeof(unsigned long long), s);
+    if (rc == QSL_OK) rc = morton_order(f->view, n, seeds, (uint32_t *)perm, !(p->flags & QSL_FLAG_NO_SORT), s);
+    cudaError_t e = cudaSuccess;
+    if (rc == QSL_OK) {
+        A.perm = (const uint32_t *)perm; A.rec = (double *)rec; A.queue = (unsigned long long *)queue;
+        e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
+        const bool dev = p->mode == QSL_TRACE_LQ;
+        if (e == cudaSuccess)
+            e = f->sample_type == QSL_F32 ? launch_trace_f32(A, dev, refill, s) : launch_trace_f64(A, dev, refill, s);
+        if (e == cudaSuccess) {
+            EpilogueArgs E;
+            E.T = A; E.with_dev = dev ? 1 : 0; E.out = *out;
+            e = f->sample_type == QSL_F32 ? launch_epilogue_f32(E, s) : launch_epilogue_f64(E, s);
+        }
+        if (e != cudaSuccess) rc = record_cuda(e);
+    }
+    scratch_free(perm, s); scratch_free(rec, s); scratch_free(queue, s);
+    return rc;
+}

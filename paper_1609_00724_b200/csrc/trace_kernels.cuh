@@ -1,0 +1,516 @@
+// Device code of the field-line tracer: field evaluation, fused RK step of the 10-component
+// state (x, delta1, delta2, L), termination + landing, per-direction records, and the Q/L epilogue.
+//
+//  PAPER.md:79  (eq. 1)   d x/d lambda = B^(x)
+//  PAPER.md:95  (eq. 3)   B^(x) = sum_v B^{v+c} f_v(x - x_c; h_c), trilinear kernels eq. (4)
+//  PAPER.md:119 (eq. 5)   d delta/d lambda = (delta . grad) B^, gradient taken analytically on the kernels (:123, :137)
+//  PAPER.md:141           fixed-step integrators (Euler in the paper; RK4 by BASELINE.json, reading A5)
+//  PAPER.md:163, 165      integrate forwards and backwards to any boundary of the box / to a maximum length
+//  PAPER.md:156, 174, 176 (eq. 11) perpendicular projection and Q at the end points
+#pragma once
+#include <math.h>
+
+#include "qsl_internal.cuh"
+
+namespace qsl {
+
+// ---------------------------------------------------------------------------------------------------------------
+// Kernel arguments
+struct TraceArgs {
+    FieldView fv;
+    double inv_h[3];             // 1 / uniform spacing
+    double box_lo[3], box_hi[3];
+    double h_uniform;            // step_frac * min_d h_d on a uniform grid
+    double step_frac, max_length, null_eps;
+    long long max_steps;
+    int method;
+    int interleave;              // work item q -> (pos, dir): interleave ? (q >> 1, q & 1) : (q % n, q / n)
+    long long n;                 // number of seeds
+    const double *seeds;         // n*3, caller order
+    const uint32_t *perm;        // sorted position -> seed index
+    double *rec;                 // 2n per-direction records of REC_DOUBLES doubles, index = dir*n + pos
+    unsigned long long *total_steps;
+    unsigned long long *queue;   // work counter of the persistent kernel
+};
+
+// Per-direction record written once when a line ends: x[3], d1[3], d2[3], L, then (nsteps, face|flags) as two uint32.
+constexpr int REC_DOUBLES = 12;
+constexpr uint32_t REC_STALL = 1u << 8, REC_CAP = 1u << 9, REC_SEED_OUTSIDE = 1u << 10, REC_NULL_AT_SEED = 1u << 11;
+
+template <typename S> struct Sample4;
+template <> struct Sample4<float> { using type = float4; };
+template <> struct Sample4<double> { using type = double4; };
+
+// One gather per cell corner: LDG.128 for a float4 sample, one 256-bit LDG (sm_100) for a double4 sample.
+__device__ __forceinline__ float4 load_sample(const float4 *p) { return __ldg(p); }
+__device__ __forceinline__ double4 load_sample(const double4 *p)
+{
+    double4 r;
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Cell location (PAPER.md:93: "identify the cell within the input array within which x lies"; :97 h_c).
+// Reading A8: index clamped to [0, n-2], fraction not clamped.
+template <bool STRETCHED>
+__device__ __forceinline__ void locate(const TraceArgs &A, int d, int n, double x, int &i, double &t, double &inv_h, double &hc)
+{
+    if (!STRETCHED) {
+        const double u = (x - A.fv.lo[d]) * A.inv_h[d];
+        int ii = (int)floor(u);                       // NaN converts to 0
+        ii = max(0, min(ii, n - 2));
+        i = ii;
+        t = u - (double)ii;
+        inv_h = A.inv_h[d];
+        hc = A.fv.h[d];
+    } else {
+        const double *__restrict__ xs = A.fv.axis[d];
+        int lo = 0, hi = n - 1;                       // largest i with xs[i] <= x, clamped to [0, n-2]
+        if (x >= xs[n - 1]) lo = n - 2;
+        else if (x >= xs[0]) {
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(xs + mid) <= x) lo = mid; else hi = mid; }
+        }
+        lo = min(lo, n - 2);
+        const double x0 = __ldg(xs + lo), x1 = __ldg(xs + lo + 1);
+        hc = x1 - x0;
+        inv_h = 1.0 / hc;
+        t = (x - x0) * inv_h;
+        i = lo;
+    }
+}
+
+// Trilinear value and analytic gradient of one component from its 8 corner samples:
+// lerp along x, then y, then z; the differences formed on the way are the gradient numerators.
+template <bool WITH_J>
+__device__ __forceinline__ void trilinear(double c000, double c100, double c010, double c110, double c001, double c101,
+                                          double c011, double c111, double tx, double ty, double tz, double &val,
+                                          double &gx, double &gy, double &gz)
+{
+    const double dx00 = c100 - c000, dx10 = c110 - c010, dx01 = c101 - c001, dx11 = c111 - c011;
+    const double v00 = fma(tx, dx00, c000), v10 = fma(tx, dx10, c010), v01 = fma(tx, dx01, c001), v11 = fma(tx, dx11, c011);
+    const double dy0 = v10 - v00, dy1 = v11 - v01;
+    const double v0 = fma(ty, dy0, v00), v1 = fma(ty, dy1, v01);
+    const double dz = v1 - v0;
+    val = fma(tz, dz, v0);
+    if (WITH_J) {
+        gz = dz;
+        gy = fma(tz, dy1 - dy0, dy0);
+        const double gx0 = fma(ty, dx10 - dx00, dx00), gx1 = fma(ty, dx11 - dx01, dx01);
+        gx = fma(tz, gx1 - gx0, gx0);
+    }
+}
+
+// Evaluate(x) -> b[3], J[9] (J[c*3+d] = d b_c / d x_d), optionally m = |B| and the cell size (O1 of DESIGN.md).
+template <typename S, bool STRETCHED, bool INTERP, bool WITH_J, bool WITH_M>
+__device__ __forceinline__ void evaluate(const TraceArgs &A, const double x[3], double b[3], double J[9], double &m, double &hmin)
+{
+    using S4 = typename Sample4<S>::type;
+    int i, j, k; double tx, ty, tz, ihx, ihy, ihz, hx, hy, hz;
+    locate<STRETCHED>(A, 0, A.fv.nx, x[0], i, tx, ihx, hx);
+    locate<STRETCHED>(A, 1, A.fv.ny, x[1], j, ty, ihy, hy);
+    locate<STRETCHED>(A, 2, A.fv.nz, x[2], k, tz, ihz, hz);
+    hmin = fmin(hx, fmin(hy, hz));
+    const int nx = A.fv.nx, sxy = A.fv.nx * A.fv.ny;
+    const S4 *__restrict__ p = (const S4 *)A.fv.samples + ((size_t)k * A.fv.ny + j) * nx + i;
+    const S4 s000 = load_sample(p), s100 = load_sample(p + 1), s010 = load_sample(p + nx), s110 = load_sample(p + nx + 1);
+    const S4 s001 = load_sample(p + sxy), s101 = load_sample(p + sxy + 1), s011 = load_sample(p + sxy + nx),
+             s111 = load_sample(p + sxy + nx + 1);
+    double v[3], g[9];
+    trilinear<WITH_J>(s000.x, s100.x, s010.x, s110.x, s001.x, s101.x, s011.x, s111.x, tx, ty, tz, v[0], g[0], g[1], g[2]);
+    trilinear<WITH_J>(s000.y, s100.y, s010.y, s110.y, s001.y, s101.y, s011.y, s111.y, tx, ty, tz, v[1], g[3], g[4], g[5]);
+    trilinear<WITH_J>(s000.z, s100.z, s010.z, s110.z, s001.z, s101.z, s011.z, s111.z, tx, ty, tz, v[2], g[6], g[7], g[8]);
+    if (WITH_J) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { g[c * 3 + 0] *= ihx; g[c * 3 + 1] *= ihy; g[c * 3 + 2] *= ihz; }
+    }
+    if (!INTERP) {
+        // paper mode: the interpolant of the pre-normalised samples is used as is
+#pragma unroll
+        for (int c = 0; c < 3; ++c) b[c] = v[c];
+        if (WITH_J) {
+#pragma unroll
+            for (int q = 0; q < 9; ++q) J[q] = g[q];
+        }
+        if (WITH_M) {
+            double dummy0, dummy1, dummy2;
+            trilinear<false>(s000.w, s100.w, s010.w, s110.w, s001.w, s101.w, s011.w, s111.w, tx, ty, tz, m, dummy0, dummy1, dummy2);
+        }
+    } else {
+        // reading A2: interpolate B, then normalise: b = B/|B|, J = (G - u (u^T G))/|B|, m = |B|
+        const double n2 = fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0]));
+        const double nn = sqrt(n2);
+        if (nn < 1e-300) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) b[c] = 0.0;
+            if (WITH_J) {
+#pragma unroll
+                for (int q = 0; q < 9; ++q) J[q] = 0.0;
+            }
+            m = 0.0;
+        } else {
+            const double inv = 1.0 / nn;
+            const double u0 = v[0] * inv, u1 = v[1] * inv, u2 = v[2] * inv;
+            b[0] = u0; b[1] = u1; b[2] = u2;
+            if (WITH_J) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const double uG = fma(u2, g[6 + d], fma(u1, g[3 + d], u0 * g[d]));
+                    J[d] = (g[d] - u0 * uG) * inv;
+                    J[3 + d] = (g[3 + d] - u1 * uG) * inv;
+                    J[6 + d] = (g[6 + d] - u2 * uG) * inv;
+                }
+            }
+            m = nn;
+        }
+    }
+}
+
+__device__ __forceinline__ double norm3(const double v[3]) { return sqrt(fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0]))); }
+__device__ __forceinline__ double dot3(const double a[3], const double b[3]) { return fma(a[2], b[2], fma(a[1], b[1], a[0] * b[0])); }
+
+__device__ __forceinline__ bool inside_box(const TraceArgs &A, const double x[3])
+{
+    return x[0] >= A.box_lo[0] && x[0] <= A.box_hi[0] && x[1] >= A.box_lo[1] && x[1] <= A.box_hi[1] &&
+           x[2] >= A.box_lo[2] && x[2] <= A.box_hi[2];
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// One work item = one direction of one field line, advanced by a small state machine so that every lane of a warp
+// runs the same code whatever its phase:
+//   phase 0      trial RK step of size h; accepted if the trial point is inside the closed trace box
+//   phase 1..3   landing (reading A4): step of size hp from the same state, then one Newton update of hp from the
+//                field at the trial end (evaluated as a "5th stage" through the same evaluate call site)
+//   phase 4      final step of size hp, snap onto the face, done
+// NV = 9 with deviation vectors (QSL_TRACE_LQ), 3 without (QSL_TRACE_L): x and L are bit-identical in both modes.
+template <typename S, bool DEV, bool STRETCHED, bool INTERP>
+struct LineState {
+    static constexpr int NV = DEV ? 9 : 3;
+    double y[NV];        // x, delta1, delta2
+    double L, lam, hp, bound;
+    uint32_t nsteps;
+    int phase, axis, face;
+    double sgn;
+    long long slot;      // record index dir*n + pos
+
+    // Initialises from work item q.  Returns false if the item ended at once (seed outside / null at seed).
+    __device__ bool init(const TraceArgs &A, long long q)
+    {
+        long long pos; int dir;
+        if (A.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= A.n ? 1 : 0; pos = q - (long long)dir * A.n; }
+        slot = (long long)dir * A.n + pos;
+        sgn = dir ? -1.0 : 1.0;
+        const uint32_t si = A.perm[pos];
+        double x[3] = { A.seeds[3 * (size_t)si], A.seeds[3 * (size_t)si + 1], A.seeds[3 * (size_t)si + 2] };
+        L = 0.0; lam = 0.0; nsteps = 0; phase = 0; axis = 0; face = 255; hp = 0.0; bound = 0.0;
+#pragma unroll
+        for (int c = 0; c < NV; ++c) y[c] = c < 3 ? x[c] : 0.0;
+        if (!inside_box(A, x)) { finish(A, REC_SEED_OUTSIDE); return false; }
+        double b[3], J[9], m, hmin;
+        evaluate<S, STRETCHED, INTERP, false, false>(A, x, b, J, m, hmin);
+        const double nb = norm3(b);
+        if (!(nb >= A.null_eps)) { finish(A, REC_NULL_AT_SEED); return false; }
+        if (DEV) {
+            // O2 (PAPER.md:160 eq. 9, :163): a^, b^ orthonormal with B^(x0); reading A7: e = axis of smallest |u_d|
+            const double inv = 1.0 / nb;
+            const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
+            int e = 0;
+            if (fabs(u[1]) < fabs(u[e])) e = 1;
+            if (fabs(u[2]) < fabs(u[e == 1 ? 1 : 0])) e = 2;
+            const double ue = e == 0 ? u[0] : (e == 1 ? u[1] : u[2]);
+            double a[3] = { -u[0] * ue, -u[1] * ue, -u[2] * ue };
+            if (e == 0) a[0] += 1.0; else if (e == 1) a[1] += 1.0; else a[2] += 1.0;
+            const double ia = 1.0 / norm3(a);
+            a[0] *= ia; a[1] *= ia; a[2] *= ia;
+            y[3 % NV] = a[0]; y[4 % NV] = a[1]; y[5 % NV] = a[2];
+            y[6 % NV] = u[1] * a[2] - u[2] * a[1];
+            y[7 % NV] = u[2] * a[0] - u[0] * a[2];
+            y[8 % NV] = u[0] * a[1] - u[1] * a[0];
+        }
+        return true;
+    }
+
+    __device__ void finish(const TraceArgs &A, uint32_t flags)
+    {
+        double *r = A.rec + (size_t)slot * REC_DOUBLES;
+        double out[REC_DOUBLES];
+#pragma unroll
+        for (int c = 0; c < 9; ++c) out[c] = c < NV ? y[c % NV] : 0.0;
+        out[9] = L;
+        const uint32_t w1 = (uint32_t)face | flags;
+        out[10] = __hiloint2double((int)w1, (int)nsteps);
+        out[11] = lam;
+        double2 *r2 = reinterpret_cast<double2 *>(r);
+#pragma unroll
+        for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
+    }
+
+    // Advances the line by one attempt (one trial step, one landing iteration, or the final landing step).
+    // Returns true when the line has ended (its record is written).
+    __device__ bool advance(const TraceArgs &A)
+    {
+        double acc[NV], accL = 0.0, ys[NV], yn[NV], Ln = L;
+        double hs = phase == 0 ? 0.0 : hp, h = 0.0;
+        const int last = A.method == QSL_EULER ? 0 : 3;
+#pragma unroll
+        for (int c = 0; c < NV; ++c) { acc[c] = 0.0; ys[c] = y[c]; yn[c] = y[c]; }
+#pragma unroll 1
+        for (int st = 0;; ++st) {
+            double b[3], J[9], m, hmin;
+            evaluate<S, STRETCHED, INTERP, DEV, false>(A, ys, b, J, m, hmin);
+            const double bn = norm3(b);
+            if (st == 0 && phase == 0) {
+                // O4: stall / caps are tested on k1 before the step; h from the cell containing x
+                if (!(bn >= A.null_eps)) { finish(A, REC_STALL); return true; }
+                if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, REC_CAP); return true; }
+                h = STRETCHED ? A.step_frac * hmin : A.h_uniform;
+                if (lam + h > A.max_length) h = A.max_length - lam;
+                hs = h;
+            }
+            if (st > last) {
+                // landing, "5th stage": b at the trial end -> one Newton update of hp (clamped to [0, h_full])
+                const double bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
+                const double xd = axis == 0 ? yn[0] : (axis == 1 ? yn[1] : yn[2]);
+                const double g = sgn * bd, r = xd - bound;
+                if (g != 0.0) {
+                    double hn = hp - r / g;
+                    if (hn == hn) hp = fmin(fmax(hn, 0.0), hfull());
+                }
+                ++phase;
+                return false;
+            }
+            // stage derivative k = (s b, s J d1, s J d2, |b|)  (PAPER.md:79 eq. 1, :119 eq. 5; reading A3 for L)
+            double k[NV];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) k[c] = sgn * b[c];
+            if (DEV) {
+#pragma unroll
+                for (int v = 0; v < 2; ++v)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c)
+                        k[(3 + 3 * v + c) % NV] = sgn * fma(J[c * 3 + 2], ys[(3 + 3 * v + 2) % NV],
+                                                            fma(J[c * 3 + 1], ys[(3 + 3 * v + 1) % NV], J[c * 3] * ys[(3 + 3 * v) % NV]));
+            }
+            const double w = (st == 0 || st == last) ? 1.0 : 2.0;
+#pragma unroll
+            for (int c = 0; c < NV; ++c) acc[c] = fma(w, k[c], acc[c]);
+            accL = fma(w, bn, accL);
+            if (st == last) {
+                const double f = A.method == QSL_EULER ? hs : hs * (1.0 / 6.0);
+#pragma unroll
+                for (int c = 0; c < NV; ++c) yn[c] = fma(f, acc[c], y[c]);
+                Ln = fma(f, accL, L);
+                if (phase >= 1 && phase <= 3) {
+#pragma unroll
+                    for (int c = 0; c < NV; ++c) ys[c] = yn[c];
+                    continue;
+                }
+                break;
+            }
+            const double ch = st == 2 ? hs : 0.5 * hs;
+#pragma unroll
+            for (int c = 0; c < NV; ++c) ys[c] = fma(ch, k[c], y[c]);
+        }
+        if (phase == 0) {
+            if (inside_box(A, yn)) {
+#pragma unroll
+                for (int c = 0; c < NV; ++c) y[c] = yn[c];
+                L = Ln; lam += h; ++nsteps;
+                return false;
+            }
+            // first face crossed by the chord: smallest fraction, tie -> lowest axis (reading A4)
+            double phi = INFINITY; int ax = -1, fc = 255; double bd = 0.0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                if (yn[d] < A.box_lo[d]) {
+                    const double f = (A.box_lo[d] - y[d]) / (yn[d] - y[d]);
+                    if (f < phi) { phi = f; ax = d; fc = 2 * d; bd = A.box_lo[d]; }
+                } else if (yn[d] > A.box_hi[d]) {
+                    const double f = (A.box_hi[d] - y[d]) / (yn[d] - y[d]);
+                    if (f < phi) { phi = f; ax = d; fc = 2 * d + 1; bd = A.box_hi[d]; }
+                }
+            }
+            if (ax < 0) { finish(A, REC_STALL); return true; }   // non-finite trial point
+            axis = ax; face_pending = fc; bound = bd; hp = phi * h; hfull_ = h; phase = 1;
+            return false;
+        }
+        // phase 4: final landing step
+#pragma unroll
+        for (int c = 0; c < NV; ++c) y[c] = yn[c];
+        if (axis == 0) y[0] = bound; else if (axis == 1) y[1] = bound; else y[2] = bound;
+        L = Ln; lam += hp; ++nsteps; face = face_pending;
+        finish(A, 0);
+        return true;
+    }
+
+    int face_pending;
+    double hfull_;
+    __device__ __forceinline__ double hfull() const { return hfull_; }
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// Kernels.  REFILL = false: one work item per thread (grid covers 2n items).  REFILL = true: persistent warps, a lane
+// whose line ended pops the next item from a global counter (warp-aggregated atomic), so ragged line lengths do not
+// idle lanes (north_star, "persistent trace kernel with a global work queue that refills lanes as lines terminate").
+template <typename S, bool DEV, bool STRETCHED, bool INTERP, bool REFILL>
+__global__ void __launch_bounds__(128) trace_kernel(const TraceArgs A)
+{
+    LineState<S, DEV, STRETCHED, INTERP> ls;
+    const long long n_items = 2 * A.n;
+    unsigned long long my_steps = 0;
+    if (!REFILL) {
+        const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        if (q < n_items && ls.init(A, q)) {
+            while (!ls.advance(A)) {}
+        }
+        if (q < n_items) my_steps = ls.nsteps;
+    } else {
+        const unsigned lane = threadIdx.x & 31u;
+        bool have = false, drained = false;
+        while (true) {
+            if (!have && !drained) {
+                const unsigned m = __activemask();
+                const int leader = __ffs(m) - 1;
+                unsigned long long base = 0;
+                if ((int)lane == leader) base = atomicAdd(A.queue, (unsigned long long)__popc(m));
+                base = __shfl_sync(m, base, leader);
+                const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
+                if (q >= n_items) drained = true;
+                else { have = ls.init(A, q); if (!have) my_steps += 0; }
+            }
+            if (__all_sync(0xffffffffu, drained && !have)) break;
+            if (have) {
+                if (ls.advance(A)) { my_steps += ls.nsteps; have = false; }
+            }
+        }
+    }
+    if (A.total_steps) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) my_steps += __shfl_xor_sync(0xffffffffu, my_steps, o);
+        if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(A.total_steps, my_steps);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Epilogue: one thread per seed combines its forward and backward records.
+struct EpilogueArgs {
+    TraceArgs T;
+    int with_dev;
+    qsl_trace_out out;
+};
+
+struct EndProj { double a[3], b[3], m; };
+
+template <typename S, bool STRETCHED, bool INTERP>
+__device__ void project_end(const TraceArgs &A, const double *r, int face, bool bnd, EndProj &E)
+{
+    // delta_perp = delta - B^(B^ . delta) with B^ re-normalised at the end point.
+    // Reading A1 (bnd): slide along the field onto the end face instead, and weight by the normal field component.
+    double b[3], J[9], m, hmin;
+    evaluate<S, STRETCHED, INTERP, false, true>(A, r, b, J, m, hmin);
+    const double inv = 1.0 / norm3(b);
+    const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
+    const double *d1 = r + 3, *d2 = r + 6;
+    double c1, c2;
+    if (bnd && face != 255) {
+        const int ax = face >> 1;
+        const double un = ax == 0 ? u[0] : (ax == 1 ? u[1] : u[2]);
+        c1 = (ax == 0 ? d1[0] : (ax == 1 ? d1[1] : d1[2])) / un;
+        c2 = (ax == 0 ? d2[0] : (ax == 1 ? d2[1] : d2[2])) / un;
+        E.m = m * fabs(un);
+    } else {
+        c1 = dot3(u, d1); c2 = dot3(u, d2);
+        E.m = m;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { E.a[c] = d1[c] - u[c] * c1; E.b[c] = d2[c] - u[c] * c2; }
+}
+
+__device__ __forceinline__ double q_eq11(const EndProj &F, const EndProj &B, double m0)
+{
+    // PAPER.md:174 (eq. 11): Q = B_F B_B / B_0^2 [ a_F^2 b_B^2 + a_B^2 b_F^2 - 2 (a_B . b_B)(a_F . b_F) ]
+    const double aF2 = dot3(F.a, F.a), bF2 = dot3(F.b, F.b), aB2 = dot3(B.a, B.a), bB2 = dot3(B.b, B.b);
+    const double abF = dot3(F.a, F.b), abB = dot3(B.a, B.b);
+    return (F.m * B.m) / (m0 * m0) * ((aF2 * bB2 + aB2 * bF2) - 2.0 * (abB * abF));
+}
+
+template <typename S, bool STRETCHED, bool INTERP>
+__global__ void __launch_bounds__(128) epilogue_kernel(const EpilogueArgs E)
+{
+    const TraceArgs &A = E.T;
+    const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= A.n) return;
+    const size_t si = A.perm[pos];
+    double rf[REC_DOUBLES], rb[REC_DOUBLES];
+    {
+        const double2 *pf = reinterpret_cast<const double2 *>(A.rec + (size_t)pos * REC_DOUBLES);
+        const double2 *pb = reinterpret_cast<const double2 *>(A.rec + (size_t)(A.n + pos) * REC_DOUBLES);
+#pragma unroll
+        for (int c = 0; c < REC_DOUBLES / 2; ++c) {
+            const double2 a = pf[c], b = pb[c];
+            rf[2 * c] = a.x; rf[2 * c + 1] = a.y; rb[2 * c] = b.x; rb[2 * c + 1] = b.y;
+        }
+    }
+    const uint32_t wf = (uint32_t)__double2hiint(rf[10]), wb = (uint32_t)__double2hiint(rb[10]);
+    const uint32_t nsf = (uint32_t)__double2loint(rf[10]), nsb = (uint32_t)__double2loint(rb[10]);
+    int ff = (int)(wf & 255u), fb = (int)(wb & 255u);
+    uint32_t st = 0;
+    if (wf & REC_SEED_OUTSIDE) st |= QSL_ST_SEED_OUTSIDE;
+    if (wf & REC_NULL_AT_SEED) st |= QSL_ST_NULL_AT_SEED;
+    const qsl_trace_out &O = E.out;
+    const double qnan = __longlong_as_double(0x7ff8000000000000ll);
+    if (st) {
+        for (int c = 0; c < 3; ++c) { if (O.end_f) O.end_f[3 * si + c] = qnan; if (O.end_b) O.end_b[3 * si + c] = qnan; }
+        if (O.L) O.L[si] = qnan;
+        if (O.q_perp) O.q_perp[si] = qnan;
+        if (O.q_bnd) O.q_bnd[si] = qnan;
+        if (O.face_f) O.face_f[si] = 255;
+        if (O.face_b) O.face_b[si] = 255;
+        if (O.nsteps_f) O.nsteps_f[si] = 0;
+        if (O.nsteps_b) O.nsteps_b[si] = 0;
+        if (O.dev_f) for (int c = 0; c < 6; ++c) O.dev_f[6 * si + c] = qnan;
+        if (O.dev_b) for (int c = 0; c < 6; ++c) O.dev_b[6 * si + c] = qnan;
+        if (O.status) O.status[si] = st;
+        return;
+    }
+    if (wf & REC_STALL) st |= QSL_ST_STALL_F;
+    if (wb & REC_STALL) st |= QSL_ST_STALL_B;
+    if (wf & REC_CAP) st |= QSL_ST_CAP_F;
+    if (wb & REC_CAP) st |= QSL_ST_CAP_B;
+    if ((ff != 255 && ff != 4) || (fb != 255 && fb != 4)) st |= QSL_ST_OPEN;
+    for (int c = 0; c < 3; ++c) { if (O.end_f) O.end_f[3 * si + c] = rf[c]; if (O.end_b) O.end_b[3 * si + c] = rb[c]; }
+    if (O.L) O.L[si] = rf[9] + rb[9];
+    if (O.face_f) O.face_f[si] = (unsigned char)ff;
+    if (O.face_b) O.face_b[si] = (unsigned char)fb;
+    if (O.nsteps_f) O.nsteps_f[si] = nsf;
+    if (O.nsteps_b) O.nsteps_b[si] = nsb;
+    if (O.status) O.status[si] = st;
+    if (!E.with_dev) {
+        if (O.q_perp) O.q_perp[si] = qnan;
+        if (O.q_bnd) O.q_bnd[si] = qnan;
+        if (O.dev_f) for (int c = 0; c < 6; ++c) O.dev_f[6 * si + c] = qnan;
+        if (O.dev_b) for (int c = 0; c < 6; ++c) O.dev_b[6 * si + c] = qnan;
+        return;
+    }
+    if (O.dev_f) for (int c = 0; c < 6; ++c) O.dev_f[6 * si + c] = rf[3 + c];
+    if (O.dev_b) for (int c = 0; c < 6; ++c) O.dev_b[6 * si + c] = rb[3 + c];
+    if (O.q_perp || O.q_bnd) {
+        // B_0 = |B| at the seed
+        const double x0[3] = { A.seeds[3 * si], A.seeds[3 * si + 1], A.seeds[3 * si + 2] };
+        double b0[3], J[9], m0, hmin;
+        evaluate<S, STRETCHED, INTERP, false, true>(A, x0, b0, J, m0, hmin);
+        EndProj PF, PB;
+        if (O.q_perp) {
+            project_end<S, STRETCHED, INTERP>(A, rf, ff, false, PF);
+            project_end<S, STRETCHED, INTERP>(A, rb, fb, false, PB);
+            O.q_perp[si] = q_eq11(PF, PB, m0);
+        }
+        if (O.q_bnd) {
+            project_end<S, STRETCHED, INTERP>(A, rf, ff, true, PF);
+            project_end<S, STRETCHED, INTERP>(A, rb, fb, true, PB);
+            O.q_bnd[si] = q_eq11(PF, PB, m0);
+        }
+    }
+}
+
+}  // namespace qsl

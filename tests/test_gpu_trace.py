@@ -1,0 +1,130 @@
+"""GPU parity: qsl_field_create / qsl_trace (through the C ABI) against the CPU oracle, element by element."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1609_00724_b200 as qsl
+import qsl_inputs as qi
+from tests.parity import compare_trace, cpu_field, gpu_field, run_both
+
+pytestmark = pytest.mark.gpu
+
+ALL_FLAGS = [0, qsl.QSL_FLAG_NO_REFILL, qsl.QSL_FLAG_NO_SORT, qsl.QSL_FLAG_NO_REFILL | qsl.QSL_FLAG_NO_SORT]
+
+
+@pytest.mark.parametrize("sample_type", ["f32", "f64"])
+@pytest.mark.parametrize("interp", [qsl.QSL_NORMALIZE_FIRST, qsl.QSL_INTERP_FIRST])
+def test_field_pack_bit_exact(sample_type, interp):
+    g = qi.Grid.uniform((19, 13, 11), (0, 0, 0), (1, 1, 0.5))
+    rng = np.random.default_rng(20)
+    B = [rng.normal(size=g.shape) for _ in range(3)]
+    B[0][1, 2, 3] = B[1][1, 2, 3] = B[2][1, 2, 3] = 0.0           # a null node
+    fg = gpu_field(g, B, sample_type, interp)
+    fc = cpu_field(g, B, sample_type, interp)
+    packed = fg.export().cpu().numpy().astype(np.float64).reshape(-1)
+    assert np.array_equal(packed, fc.packed)
+    assert fg.nbytes >= packed.size * (4 if sample_type == "f32" else 8)
+
+
+@pytest.mark.parametrize("flags", ALL_FLAGS)
+def test_cfg1_full_size_all_launch_modes(flags):
+    """BASELINE.json configs[0] at full size (16384 seeds, paper mode NORMALIZE_FIRST), every scheduling variant."""
+    cfg = qi.make_config("cfg1")
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", cfg["seeds"], cfg["box_lo"], cfg["box_hi"], max_steps=cfg["max_steps"],
+                    flags=flags, want_dev=True)
+    rep = compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], label="cfg1 flags=%d" % flags)
+    assert rep["same_steps"] == 1.0
+    # the basis (a^, b^) is only unique where the smallest |u_d| is unique (reading A7): here off the diagonals |x0| = |y0|
+    s = cfg["seeds"]
+    uniq = np.abs(np.abs(s[:, 0]) - np.abs(s[:, 1])) > 1e-9
+    assert uniq.mean() > 0.98
+    assert np.abs(g["dev_f"][uniq] - c["dev_f"][uniq]).max() < 1e-9 * np.abs(c["dev_f"]).max()
+
+
+def test_cfg1_closed_form_interp_first():
+    """The CUDA path itself against the closed forms of the hyperbolic field (north_star): Q = e^{2kh} + e^{-2kh}."""
+    cfg = qi.make_config("cfg1")
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", cfg["seeds"], cfg["box_lo"], cfg["box_hi"], interp_mode=qsl.QSL_INTERP_FIRST)
+    compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], label="cfg1 interp-first")
+    s = cfg["seeds"]; k = 2.0
+    top = np.abs(s[:, 0]) <= math.exp(-k)
+    qb = np.where(top, 2 * math.cosh(2 * k), k * (s[:, 0] ** 2 + s[:, 1] ** 2) + 1 / (k * s[:, 0] ** 2))
+    assert np.abs(g["q_bnd"] / qb - 1).max() < 1e-9
+    assert np.allclose(g["q_bnd"][top], 54.61646567, rtol=1e-9)
+
+
+@pytest.mark.parametrize("sample_type", ["f32", "f64"])
+@pytest.mark.parametrize("mode", [qsl.QSL_TRACE_L, qsl.QSL_TRACE_LQ])
+def test_quadrupole_volume_seeds(sample_type, mode):
+    """cfg3-like: quadrupole, bidirectional lines from a vertical slice, ragged lengths, both storage types."""
+    cfg = qi.make_config("cfg3", scale=0.25)                         # 32^3 grid
+    rng = np.random.default_rng(21)
+    seeds = cfg["seeds"][rng.choice(len(cfg["seeds"]), 3000, replace=False)]
+    g, c = run_both(cfg["grid"], cfg["B"], sample_type, seeds, cfg["box_lo"], cfg["box_hi"], mode=mode,
+                    max_steps=cfg["max_steps"])
+    compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], with_q=mode == qsl.QSL_TRACE_LQ, label="quad")
+
+
+def test_P12_gpu_L_mode_bit_identical_to_LQ():
+    cfg = qi.make_config("cfg3", scale=0.25)
+    seeds = cfg["seeds"][::41]
+    fg = gpu_field(cfg["grid"], cfg["B"], "f64", 0)
+    s = torch.from_numpy(seeds).cuda()
+    a = qsl.qsl_trace(fg, s, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=qsl.QSL_TRACE_LQ, max_steps=cfg["max_steps"]))
+    b = qsl.qsl_trace(fg, s, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=qsl.QSL_TRACE_L, max_steps=cfg["max_steps"]))
+    for k in ("end_f", "end_b", "L", "face_f", "face_b", "nsteps_f", "nsteps_b", "status"):
+        assert torch.equal(a[k], b[k]), k
+    assert torch.isnan(b["q_perp"]).all()
+
+
+def test_stretched_grid_and_euler():
+    g = qi.Grid.from_axes(qi.stretched_axis(40, -1, 1, 3.0), qi.stretched_axis(36, -1, 1, 0.4), qi.stretched_axis(44, 0, 1, 5.0))
+    B = qi.hyperbolic_field(g, 2.0)
+    rng = np.random.default_rng(22)
+    seeds = np.stack([rng.uniform(-0.5, 0.5, 500), rng.uniform(-0.5, 0.5, 500), rng.uniform(0, 0.9, 500)], 1)
+    lo, hi = (-1, -1, 0), (1, 1, 1)
+    for interp in (0, 1):
+        gg, c = run_both(g, B, "f64", seeds, lo, hi, interp_mode=interp)
+        compare_trace(gg, c, lo, hi, label="stretched interp=%d" % interp)
+    gg, c = run_both(g, B, "f64", seeds, lo, hi, method=qsl.QSL_EULER, step_frac=0.2)
+    compare_trace(gg, c, lo, hi, label="stretched euler")
+
+
+def test_edge_cases_status_caps_empty():
+    cfg = qi.make_config("cfg1", scale=0.25)
+    lo, hi = cfg["box_lo"], cfg["box_hi"]
+    seeds = np.array([[0.0, 0.0, 0.5], [2.0, 0.0, 0.5], [0.1, 0.1, 0.2], [1.0, 1.0, 1.0], [-1.0, 0.3, 0.0], [0.3, 0.2, 0.0]])
+    for kw in (dict(max_steps=3), dict(max_length=0.1), dict()):
+        g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, lo, hi, **kw)
+        compare_trace(g, c, lo, hi, frac=1.0, label=str(kw))
+        assert np.array_equal(g["status"], c["status"])
+    # raised lower boundary
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, (-1, -1, 0.25), hi)
+    compare_trace(g, c, (-1, -1, 0.25), hi, frac=1.0, label="raised")
+    # null field
+    gz = qi.Grid.uniform((8, 8, 8), lo, hi)
+    g, c = run_both(gz, tuple(np.zeros(gz.shape) for _ in range(3)), "f64", seeds[:3], lo, hi)
+    assert np.array_equal(g["status"], c["status"]) and np.isnan(g["q_perp"]).all()
+    # n = 0
+    fg = gpu_field(cfg["grid"], cfg["B"], "f64", 0)
+    out = qsl.qsl_trace(fg, torch.empty((0, 3), dtype=torch.float64, device="cuda"), qsl.make_trace_params(lo, hi))
+    assert out["L"].numel() == 0
+    # a ragged tail: n not a multiple of the block or warp size
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", cfg["seeds"][:131], lo, hi)
+    compare_trace(g, c, lo, hi, frac=1.0, label="tail")
+
+
+def test_bad_arguments_are_reported_not_crashed():
+    cfg = qi.make_config("cfg1", scale=0.25)
+    fg = gpu_field(cfg["grid"], cfg["B"], "f64", 0)
+    s = torch.zeros((4, 3), dtype=torch.float64, device="cuda")
+    with pytest.raises(qsl.QslError):
+        qsl.qsl_trace(fg, s, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], step_frac=0.0))
+    with pytest.raises(qsl.QslError):
+        qsl.qsl_trace(fg, s, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], method=7))
+    with pytest.raises(qsl.QslError):
+        z = torch.zeros(8, dtype=torch.float64, device="cuda")
+        qsl.qsl_field_create(1, 2, 4, z, z, z, lo=(0, 0, 0), hi=(1, 1, 1))
