@@ -151,6 +151,12 @@ int qsl_refine(int ndim, int level, long long n, const unsigned int *coords, con
                const qsl_lattice *lat, long long capacity, unsigned int *child_coords, double *child_seeds,
                long long *child_base, long long *n_children, void *stream);
 
+/* ---- test hook ------------------------------------------------------------------------------------------------- */
+/* Stable ascending sort of n (key, value) pairs (DEVICE, in place) on the low key_bits (1..32) of the keys: the
+ * hand-written LSD radix sort that qsl_trace uses to Morton-order its seeds (PAPER.md:196-198 orders samples along a
+ * space-filling curve), exposed so that tests can check it on its own.                                              */
+int qsl_debug_sort_pairs(unsigned int *keys, unsigned int *vals, long long n, int key_bits, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

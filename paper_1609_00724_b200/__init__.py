@@ -8,3 +8,4 @@ from .binding import (  # noqa: F401
     QslError, Field, lib, LIB_PATH, make_lattice, make_trace_params, qsl_field_create, qsl_trace, qsl_fledge_dense,
     qsl_fledge_sparse, qsl_select, qsl_refine, DEFAULT_OUTPUTS,
 )
+from .driver import adaptive_map  # noqa: F401,E402

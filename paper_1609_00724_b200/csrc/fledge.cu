@@ -1,0 +1,198 @@
+// FLEDGE maps.  PAPER.md:190: "the gradient magnitude from the Sobel operator (i.e. a 2D or 3D
+// gradient of FLL convolved with a simple smoothing function) applied to a 2D or 3D map of the length of field lines".
+// Reading A10: un-normalised weights, difference [-1,0,+1] along the axis, smoothing [1,2,1] along the others, edges
+// replicated.  The stencil is separable: every lane folds the other axes of its own column in registers, then the
+// axis-0 taps are exchanged between neighbouring lanes with warp shuffles (no shared memory).
+#include <math.h>
+
+#include "qsl_internal.cuh"
+
+namespace qsl {
+
+constexpr int FL_THREADS = 128;
+constexpr int FL_VALID = 30;   // outputs per warp: lanes 1..30; lanes 0 and 31 carry the halo columns
+
+// Folds the axis-1 / axis-2 taps of one column.  a[o2][o1] are the clamped neighbours of the column.
+// A: smooth x smooth, B: diff along axis 1 (smooth along 2), C: diff along axis 2 (smooth along 1).
+template <int NDIM>
+__device__ __forceinline__ void fold_column(const double a[3][3], double &A, double &B, double &C)
+{
+    if (NDIM == 2) {
+        A = (a[0][0] + a[0][2]) + 2.0 * a[0][1];
+        B = a[0][2] - a[0][0];
+        C = 0.0;
+    } else {
+        double s1[3], d1[3];
+#pragma unroll
+        for (int o2 = 0; o2 < 3; ++o2) {
+            s1[o2] = (a[o2][0] + a[o2][2]) + 2.0 * a[o2][1];
+            d1[o2] = a[o2][2] - a[o2][0];
+        }
+        A = (s1[0] + s1[2]) + 2.0 * s1[1];
+        B = (d1[0] + d1[2]) + 2.0 * d1[1];
+        C = s1[2] - s1[0];
+    }
+}
+
+// Axis-0 taps across lanes: G0 = A(i+1) - A(i-1), G1 = B(i-1) + 2 B(i) + B(i+1), G2 likewise from C.
+template <int NDIM>
+__device__ __forceinline__ double combine_lanes(double A, double B, double C)
+{
+    const unsigned full = 0xffffffffu;
+    const double Am = __shfl_up_sync(full, A, 1), Ap = __shfl_down_sync(full, A, 1);
+    const double Bm = __shfl_up_sync(full, B, 1), Bp = __shfl_down_sync(full, B, 1);
+    const double G0 = Ap - Am, G1 = (Bm + Bp) + 2.0 * B;
+    double ss = fma(G1, G1, G0 * G0);
+    if (NDIM == 3) {
+        const double Cm = __shfl_up_sync(full, C, 1), Cp = __shfl_down_sync(full, C, 1);
+        const double G2 = (Cm + Cp) + 2.0 * C;
+        ss = fma(G2, G2, ss);
+    }
+    return sqrt(ss);
+}
+
+template <int NDIM>
+__global__ void __launch_bounds__(FL_THREADS) fledge_dense_kernel(long long d0, long long d1, long long d2,
+                                                                  const double *__restrict__ L, double *__restrict__ S)
+{
+    const unsigned lane = threadIdx.x & 31u;
+    const long long strips = (d0 + FL_VALID - 1) / FL_VALID;
+    const long long tasks = strips * d1 * d2;
+    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long t = (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); t < tasks; t += warps) {
+        const long long strip = t % strips, row = t / strips;
+        const long long c1 = row % d1, c2 = row / d1;
+        const long long col = strip * FL_VALID - 1 + lane;               // lane 0 / 31 = halo
+        const long long cc = min(max(col, 0ll), d0 - 1);                 // edge replication
+        double a[3][3];
+#pragma unroll
+        for (int o2 = 0; o2 < (NDIM == 3 ? 3 : 1); ++o2) {
+            const long long z = NDIM == 3 ? min(max(c2 + o2 - 1, 0ll), d2 - 1) : 0;
+#pragma unroll
+            for (int o1 = 0; o1 < 3; ++o1) {
+                const long long y = min(max(c1 + o1 - 1, 0ll), d1 - 1);
+                a[o2][o1] = __ldg(L + (z * d1 + y) * d0 + cc);
+            }
+        }
+        double A, B, C;
+        fold_column<NDIM>(a, A, B, C);
+        double s = combine_lanes<NDIM>(A, B, C);
+        // the centre tap has weight 0 in every G_d; O6 still lets a non-finite L anywhere in the stencil poison S
+        if (!isfinite(a[NDIM == 3 ? 1 : 0][1])) s = __longlong_as_double(0x7ff8000000000000ll);
+        if (lane >= 1 && lane <= FL_VALID && col < d0) S[(c2 * d1 + c1) * d0 + col] = s;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Sparse levels: the same stencil on the virtual lattice n_d 2^level; a neighbour that was not refined takes the L
+// of its nearest existing ancestor.  Cells are found by walking down from the dense level 0 through the child_base
+// links written by qsl_refine (child_base[l][i] = index at level l+1 of the first child of cell i, or -1).
+constexpr int MAX_LEVELS = 16;
+struct SparseArgs {
+    int ndim, level;
+    long long n0[3];
+    long long count;
+    const uint32_t *coords;                 // cells of `level`
+    const double *L[MAX_LEVELS];            // L[0] = dense level 0
+    const long long *child_base[MAX_LEVELS];
+    double *S;
+};
+
+template <int NDIM>
+__device__ __forceinline__ double lookup_L(const SparseArgs &A, long long c0, long long c1, long long c2)
+{
+    const int lev = A.level;
+    long long idx = ((NDIM == 3 ? (c2 >> lev) : 0) * A.n0[1] + (c1 >> lev)) * A.n0[0] + (c0 >> lev);
+    for (int l = 1; l <= lev; ++l) {
+        const long long base = __ldg(A.child_base[l - 1] + idx);
+        if (base < 0) return __ldg(A.L[l - 1] + idx);
+        const int sh = lev - l;
+        int bits = (int)((c0 >> sh) & 1) | ((int)((c1 >> sh) & 1) << 1);
+        if (NDIM == 3) bits |= (int)((c2 >> sh) & 1) << 2;
+        idx = base + bits;
+    }
+    return __ldg(A.L[lev] + idx);
+}
+
+template <int NDIM>
+__global__ void __launch_bounds__(FL_THREADS) fledge_sparse_kernel(const SparseArgs A)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= A.count) return;
+    const long long dims[3] = { A.n0[0] << A.level, A.n0[1] << A.level, NDIM == 3 ? A.n0[2] << A.level : 1 };
+    const long long c0 = A.coords[i * NDIM], c1 = A.coords[i * NDIM + 1], c2 = NDIM == 3 ? A.coords[i * NDIM + 2] : 0;
+    double As[3], Bs[3], Cs[3], centre = 0.0;
+#pragma unroll
+    for (int o0 = 0; o0 < 3; ++o0) {
+        const long long x = min(max(c0 + o0 - 1, 0ll), dims[0] - 1);
+        double a[3][3];
+#pragma unroll
+        for (int o2 = 0; o2 < (NDIM == 3 ? 3 : 1); ++o2) {
+            const long long z = NDIM == 3 ? min(max(c2 + o2 - 1, 0ll), dims[2] - 1) : 0;
+#pragma unroll
+            for (int o1 = 0; o1 < 3; ++o1) {
+                const long long y = min(max(c1 + o1 - 1, 0ll), dims[1] - 1);
+                a[o2][o1] = lookup_L<NDIM>(A, x, y, z);
+            }
+        }
+        fold_column<NDIM>(a, As[o0], Bs[o0], Cs[o0]);
+        if (o0 == 1) centre = a[NDIM == 3 ? 1 : 0][1];
+    }
+    const double G0 = As[2] - As[0], G1 = (Bs[0] + Bs[2]) + 2.0 * Bs[1];
+    double ss = fma(G1, G1, G0 * G0);
+    if (NDIM == 3) {
+        const double G2 = (Cs[0] + Cs[2]) + 2.0 * Cs[1];
+        ss = fma(G2, G2, ss);
+    }
+    A.S[i] = isfinite(centre) ? sqrt(ss) : __longlong_as_double(0x7ff8000000000000ll);
+}
+
+}  // namespace qsl
+
+using namespace qsl;
+
+extern "C" int qsl_fledge_dense(int ndim, const long long dims[3], const double *L, double *S, void *stream)
+{
+    if ((ndim != 2 && ndim != 3) || !dims || !L || !S) return QSL_EINVAL;
+    const long long d0 = dims[0], d1 = dims[1], d2 = ndim == 3 ? dims[2] : 1;
+    if (d0 < 1 || d1 < 1 || d2 < 1) return QSL_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const long long strips = (d0 + FL_VALID - 1) / FL_VALID;
+    const long long tasks = strips * d1 * d2;
+    const int wpb = FL_THREADS / 32;
+    long long blocks = (tasks + wpb - 1) / wpb;
+    const long long cap = (long long)sm_count() * 32;      // a multiple of the SM count; warps stride over the tasks
+    if (blocks > cap) blocks = cap;
+    if (ndim == 2) fledge_dense_kernel<2><<<(unsigned)blocks, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
+    else fledge_dense_kernel<3><<<(unsigned)blocks, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
+    QSL_CUDA(cudaGetLastError());
+    return QSL_OK;
+}
+
+extern "C" int qsl_fledge_sparse(const qsl_levels *lv, int level, double *S, void *stream)
+{
+    if (!lv || !lv->lat || !S || level < 1 || level >= MAX_LEVELS || lv->nlevels < level + 1) return QSL_EINVAL;
+    if (!lv->L0 || !lv->count || !lv->coords || !lv->L || !lv->child_base) return QSL_EINVAL;
+    const int ndim = lv->lat->ndim;
+    if (ndim != 2 && ndim != 3) return QSL_EINVAL;
+    SparseArgs A;
+    A.ndim = ndim; A.level = level;
+    for (int d = 0; d < 3; ++d) A.n0[d] = d < ndim ? lv->lat->n[d] : 1;
+    for (int d = 0; d < ndim; ++d)
+        if (A.n0[d] < 1 || (A.n0[d] << level) > 0xffffffffll) return QSL_ERANGE;
+    A.count = lv->count[level];
+    if (A.count < 0) return QSL_EINVAL;
+    if (A.count == 0) return QSL_OK;
+    A.coords = lv->coords[level];
+    A.L[0] = lv->L0;
+    for (int l = 1; l <= level; ++l) { A.L[l] = lv->L[l]; if (!A.L[l]) return QSL_EINVAL; }
+    for (int l = 0; l < level; ++l) { A.child_base[l] = lv->child_base[l]; if (!A.child_base[l]) return QSL_EINVAL; }
+    if (!A.coords) return QSL_EINVAL;
+    A.S = S;
+    cudaStream_t s = (cudaStream_t)stream;
+    const long long blocks = (A.count + FL_THREADS - 1) / FL_THREADS;
+    if (ndim == 2) fledge_sparse_kernel<2><<<(unsigned)blocks, FL_THREADS, 0, s>>>(A);
+    else fledge_sparse_kernel<3><<<(unsigned)blocks, FL_THREADS, 0, s>>>(A);
+    QSL_CUDA(cudaGetLastError());
+    return QSL_OK;
+}

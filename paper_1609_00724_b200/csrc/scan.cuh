@@ -40,7 +40,7 @@ __device__ __forceinline__ unsigned long long block_exclusive_scan(unsigned long
     return before + inc - v;
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) scan_tile_sums(long long n, const uint32_t *__restrict__ in,
+static __global__ void __launch_bounds__(SCAN_THREADS) scan_tile_sums(long long n, const uint32_t *__restrict__ in,
                                                                unsigned long long *__restrict__ tile_sums)
 {
     const long long base = (long long)blockIdx.x * SCAN_TILE;
@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_tile_sums(long long n, cons
 }
 
 // Single block: exclusive scan of m values in place; writes the grand total to *total_out (if not NULL).
-__global__ void __launch_bounds__(1024) scan_single_block(long long m, unsigned long long *__restrict__ v,
+static __global__ void __launch_bounds__(1024) scan_single_block(long long m, unsigned long long *__restrict__ v,
                                                           unsigned long long *__restrict__ total_out)
 {
     unsigned long long carry = 0;
@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(1024) scan_single_block(long long m, unsigned 
     if (threadIdx.x == 0 && total_out) *total_out = carry;
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) scan_tiles(long long n, const uint32_t *__restrict__ in,
+static __global__ void __launch_bounds__(SCAN_THREADS) scan_tiles(long long n, const uint32_t *__restrict__ in,
                                                            const unsigned long long *__restrict__ tile_offsets,
                                                            unsigned long long *__restrict__ out)
 {

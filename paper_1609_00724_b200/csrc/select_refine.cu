@@ -1,0 +1,223 @@
+// Threshold and refinement.
+// refine where the field-line-length jump "surpasses a certain threshold"; new samples are
+// inserted where it does.  BASELINE.json configs[2]: "where the FLEDGE value exceeds the 95th percentile".
+// Reading A11: tau = nearest-rank order statistic of the finite level-0 values; strict >; 2x refinement per axis.
+//   qsl_select: exact radix select on the order-preserving 64-bit image of the doubles (8 passes of 8 bits), all on device.
+//   qsl_refine: flag -> exclusive scan -> stable stream compaction; every flagged cell emits its 2^D children.
+#include <math.h>
+
+#include "qsl_internal.cuh"
+#include "scan.cuh"
+
+namespace qsl {
+
+// ---------------------------------------------------------------------------------------------------------------
+// radix select
+struct SelectState {
+    unsigned long long prefix;      // high digits of the answer found so far
+    unsigned long long rank;        // 0-based rank still to be located inside the current bucket
+    unsigned long long n_finite;
+    unsigned int hist[256];
+};
+
+__device__ __forceinline__ unsigned long long ordered_key(double v)
+{
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double key_to_double(unsigned long long k)
+{
+    const unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    return __longlong_as_double((long long)b);
+}
+
+__global__ void __launch_bounds__(256) select_hist_kernel(long long n, const double *__restrict__ S, int pass,
+                                                          SelectState *__restrict__ st)
+{
+    __shared__ unsigned int h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const int shift = 56 - 8 * pass;
+    const unsigned long long prefix = st->prefix;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const double v = S[i];
+        if (!isfinite(v)) continue;
+        const unsigned long long k = ordered_key(v);
+        if (pass == 0 || (k >> (shift + 8)) == (prefix >> (shift + 8))) atomicAdd(&h[(k >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    if (h[threadIdx.x]) atomicAdd(&st->hist[threadIdx.x], h[threadIdx.x]);
+}
+
+__global__ void __launch_bounds__(256) select_pick_kernel(int pass, double p, SelectState *__restrict__ st, double *__restrict__ tau)
+{
+    const unsigned int mine = st->hist[threadIdx.x];
+    unsigned long long total;
+    const unsigned long long before = block_exclusive_scan((unsigned long long)mine, total);
+    if (pass == 0 && threadIdx.x == 0) {
+        st->n_finite = total;
+        long long r = (long long)ceil(p * (double)total);         // nearest rank: the ceil(p N)-th smallest
+        if (r < 1) r = 1;
+        if (r > (long long)total) r = (long long)total;
+        st->rank = total ? (unsigned long long)(r - 1) : 0ull;
+    }
+    __syncthreads();
+    const unsigned long long rank = st->rank;
+    const bool hit = mine != 0 && rank >= before && rank < before + mine;
+    __syncthreads();
+    if (hit) {
+        const int shift = 56 - 8 * pass;
+        st->prefix |= (unsigned long long)threadIdx.x << shift;
+        st->rank = rank - before;
+    }
+    st->hist[threadIdx.x] = 0;
+    __syncthreads();
+    if (pass == 7 && threadIdx.x == 0)
+        *tau = st->n_finite ? key_to_double(st->prefix) : __longlong_as_double(0x7ff8000000000000ll);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// refine
+struct RefineArgs {
+    int ndim, level;
+    long long n;
+    const uint32_t *coords;          // NULL: dense level-0 lattice in index order
+    const double *S;
+    const double *tau;
+    long long n0[3];
+    double origin[3], e[3][3];
+    long long capacity;
+    uint32_t *child_coords;
+    double *child_seeds;
+    long long *child_base;
+};
+
+__global__ void __launch_bounds__(256) refine_flag_kernel(long long n, const double *__restrict__ S, const double *__restrict__ tau,
+                                                          uint32_t *__restrict__ flags)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) flags[i] = S[i] > *tau ? 1u : 0u;                // NaN never flags
+}
+
+template <int NDIM>
+__global__ void __launch_bounds__(256) refine_emit_kernel(const RefineArgs A, const uint32_t *__restrict__ flags,
+                                                          const unsigned long long *__restrict__ offs)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= A.n) return;
+    if (!flags[i]) { if (A.child_base) A.child_base[i] = -1; return; }
+    const long long first = (long long)offs[i] << NDIM;
+    if (A.child_base) A.child_base[i] = first;
+    uint32_t c[3];
+    if (A.coords) {
+#pragma unroll
+        for (int d = 0; d < NDIM; ++d) c[d] = A.coords[i * NDIM + d];
+    } else {
+        c[0] = (uint32_t)(i % A.n0[0]);
+        c[1] = (uint32_t)((i / A.n0[0]) % A.n0[1]);
+        c[2] = (uint32_t)(i / (A.n0[0] * A.n0[1]));
+    }
+    double inv_den[3];
+#pragma unroll
+    for (int d = 0; d < NDIM; ++d) inv_den[d] = (double)(A.n0[d] << (A.level + 1));
+#pragma unroll
+    for (int ch = 0; ch < (1 << NDIM); ++ch) {
+        const long long m = first + ch;
+        if (m >= A.capacity) return;
+        double w[3] = { 0.0, 0.0, 0.0 };
+#pragma unroll
+        for (int d = 0; d < NDIM; ++d) {
+            const uint32_t cc = 2u * c[d] + (uint32_t)((ch >> d) & 1);
+            A.child_coords[m * NDIM + d] = cc;
+            w[d] = __ddiv_rn((double)cc + 0.5, inv_den[d]);      // one IEEE division, as in the definition
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            double pos = __fma_rn(w[0], A.e[0][k], A.origin[k]);
+            pos = __fma_rn(w[1], A.e[1][k], pos);
+            if (NDIM == 3) pos = __fma_rn(w[2], A.e[2][k], pos);
+            A.child_seeds[3 * m + k] = pos;
+        }
+    }
+}
+
+}  // namespace qsl
+
+using namespace qsl;
+
+extern "C" int qsl_select(long long n, const double *S, double p, double *tau, void *stream)
+{
+    if (n < 0 || (n > 0 && !S) || !tau || !(p >= 0.0 && p <= 1.0)) return QSL_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    void *stp = nullptr;
+    int rc = scratch_alloc(&stp, sizeof(SelectState), s);
+    if (rc != QSL_OK) return rc;
+    SelectState *st = (SelectState *)stp;
+    cudaError_t e = cudaMemsetAsync(st, 0, sizeof(SelectState), s);
+    long long blocks = (n + 255) / 256;
+    const long long cap = (long long)sm_count() * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    for (int pass = 0; pass < 8 && e == cudaSuccess; ++pass) {
+        select_hist_kernel<<<(unsigned)blocks, 256, 0, s>>>(n, S, pass, st);
+        select_pick_kernel<<<1, 256, 0, s>>>(pass, p, st, tau);
+        e = cudaGetLastError();
+    }
+    scratch_free(stp, s);
+    if (e != cudaSuccess) return record_cuda(e);
+    return QSL_OK;
+}
+
+extern "C" int qsl_refine(int ndim, int level, long long n, const unsigned int *coords, const double *S, const double *tau,
+                          const qsl_lattice *lat, long long capacity, unsigned int *child_coords, double *child_seeds,
+                          long long *child_base, long long *n_children, void *stream)
+{
+    if ((ndim != 2 && ndim != 3) || level < 0 || level > 14 || n < 0 || !lat || !tau || !n_children || capacity < 0) return QSL_EINVAL;
+    if (n > 0 && (!S || (capacity > 0 && (!child_coords || !child_seeds)))) return QSL_EINVAL;
+    if (lat->ndim != ndim) return QSL_EINVAL;
+    if (!coords) {
+        const long long dense = lat->n[0] * lat->n[1] * (ndim == 3 ? lat->n[2] : 1);
+        if (level != 0 || n != dense) return QSL_EINVAL;
+    }
+    for (int d = 0; d < ndim; ++d)
+        if (lat->n[d] < 1 || (lat->n[d] << (level + 1)) > 0xffffffffll) return QSL_ERANGE;
+    *n_children = 0;
+    if (n == 0) return QSL_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    RefineArgs A;
+    A.ndim = ndim; A.level = level; A.n = n; A.coords = coords; A.S = S; A.tau = tau;
+    for (int d = 0; d < 3; ++d) {
+        A.n0[d] = d < ndim ? lat->n[d] : 1;
+        A.origin[d] = lat->origin[d];
+        A.e[0][d] = lat->e0[d]; A.e[1][d] = lat->e1[d]; A.e[2][d] = lat->e2[d];
+    }
+    A.capacity = capacity; A.child_coords = child_coords; A.child_seeds = child_seeds; A.child_base = child_base;
+
+    void *flags = nullptr, *offs = nullptr, *tiles = nullptr, *total = nullptr;
+    const long long ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+    int rc = scratch_alloc(&flags, sizeof(uint32_t) * (size_t)n, s);
+    if (rc == QSL_OK) rc = scratch_alloc(&offs, sizeof(unsigned long long) * (size_t)n, s);
+    if (rc == QSL_OK) rc = scratch_alloc(&tiles, sizeof(unsigned long long) * (size_t)ntiles, s);
+    if (rc == QSL_OK) rc = scratch_alloc(&total, sizeof(unsigned long long), s);
+    unsigned long long h_total = 0;
+    if (rc == QSL_OK) {
+        const unsigned blocks = (unsigned)((n + 255) / 256);
+        refine_flag_kernel<<<blocks, 256, 0, s>>>(n, S, tau, (uint32_t *)flags);
+        cudaError_t e = exclusive_scan_u32(n, (const uint32_t *)flags, (unsigned long long *)offs, (unsigned long long *)tiles,
+                                           (unsigned long long *)total, s);
+        if (e == cudaSuccess) {
+            if (ndim == 2) refine_emit_kernel<2><<<blocks, 256, 0, s>>>(A, (const uint32_t *)flags, (const unsigned long long *)offs);
+            else refine_emit_kernel<3><<<blocks, 256, 0, s>>>(A, (const uint32_t *)flags, (const unsigned long long *)offs);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&h_total, total, sizeof(h_total), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) rc = record_cuda(e);
+    }
+    scratch_free(flags, s); scratch_free(offs, s); scratch_free(tiles, s); scratch_free(total, s);
+    if (rc != QSL_OK) return rc;
+    *n_children = (long long)(h_total << ndim);
+    if (*n_children > capacity) return QSL_ERANGE;
+    return QSL_OK;
+}

@@ -84,3 +84,32 @@ def compare_trace(g, c, box_lo, box_hi, *, with_q=True, frac=0.999, label=""):
             assert rep[key + "_dlog_max"] <= 1e-3, (label, rep)
     assert g["total_steps"] == int(g["nsteps_f"].astype(np.int64).sum() + g["nsteps_b"].astype(np.int64).sum()), label
     return rep
+
+
+# ------------------------------------------------------------------------------------------------- level loop (a9)
+def oracle_pipeline(cfg, sample_type=None, interp_mode=0):
+    """The adaptive level loop (O6, O7 + traces) run entirely by the oracle.  Returns per-level products."""
+    st = sample_type or cfg["sample_type"]
+    fc = cpu_field(cfg["grid"], cfg["B"], st, interp_mode)
+    lat = cfg["lattice"]; ndim = lat.ndim
+    kw = dict(max_steps=cfg["max_steps"], step_frac=cfg["step_frac"], null_eps=cfg["null_eps"])
+    o0 = oracle.trace(fc, cfg["seeds"], cfg["box_lo"], cfg["box_hi"], mode=oracle.TRACE_L, **kw)
+    shape = tuple(int(v) for v in lat.n[:ndim][::-1])
+    L0 = o0["L"].reshape(shape)
+    S0 = oracle.fledge_dense(L0, ndim).reshape(-1)
+    tau = oracle.select(S0, cfg["p"])
+    n = lat.count
+    c0 = np.stack(np.unravel_index(np.arange(n), shape), 1)[:, ::-1].astype(np.uint32)   # dense index order
+    res = dict(L0=o0["L"], S0=S0, tau=tau, coords=[c0], seeds=[cfg["seeds"]], out=[o0], S=[S0])
+    coords, S, Ls = c0, S0, [o0["L"]]
+    for level in range(cfg["levels"]):
+        cc, cs = oracle.refine(ndim, level, coords, S, tau, lat)
+        res["coords"].append(cc); res["seeds"].append(cs)
+        if len(cc) == 0:
+            break
+        o = oracle.trace(fc, cs, cfg["box_lo"], cfg["box_hi"], mode=oracle.TRACE_LQ, **kw)
+        res["out"].append(o); Ls.append(o["L"])
+        if level + 1 < cfg["levels"]:
+            S = oracle.fledge_sparse(ndim, lat.n[:ndim], level + 1, o0["L"], res["coords"], Ls)
+            res["S"].append(S); coords = cc
+    return res
