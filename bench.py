@@ -1,0 +1,385 @@
+#!/usr/bin/env python
+"""bench.py -- field lines/s (with Q) and RK steps/s of the libqsl hot path on B200, with its roofline fraction.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: seed ordering, the persistent trace
+kernel (a3-a5), the Q/L epilogue (a6) and, for the refinement workloads cfg3 / cfg5, FLEDGE, threshold, compaction and
+the level loop (a7-a9).  The default workload is BASELINE.json configs[1] (cfg2: quadrupole, fp64 128^3 field,
+1024^2 photospheric seeds, L + Q); DESIGN.md "Measurement" states what every key means.
+
+`value`   lines/s with the seeds and the packed field already resident in HBM (CUDA events on the launch stream).
+`e2e`     the same through the public binding with HOST buffers: pinned seeds -> device, trace, results -> pinned host.
+`roofline` the trace kernel against the FP64 (or FP32) pipe peak measured on this device by qsl_peak_fma.
+`cpu_baseline` the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload, rank 0, N = 1 only.
+`--impl reference` times only that oracle (the reference arm of the contract).
+
+Under torchrun every rank traces its own replica of the workload (lines are independent: weak scaling, no data-path
+collective); the time is the max over ranks and `value` the lines all ranks traced divided by it.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# Algorithmic FP-pipe work per accepted RK4 step of one line:
+# pipe instructions (an FMA, add or multiply each occupies one issue slot) and true flops (FMA = 2).
+PIPE_SLOTS_PER_STEP = {"LQ": 490, "L": 245}
+FLOPS_PER_STEP = {"LQ": 800, "L": 400}
+# dram__bytes_read.sum + dram__bytes_write.sum of one trace-kernel launch of the default workload, from the committed
+# ncu --set full capture (profiles/); None until a capture of the current kernel exists.
+NCU_TRACE_KERNEL_DRAM_BYTES = {}
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+class ClockSampler:
+    """Samples SM clock and clock-event reasons of one GPU during the timed region (NVML, every 100 ms)."""
+
+    BAD = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown"}
+    NOTE = {0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz, self._stop, self._t = [], set(), None, threading.Event(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in {**self.BAD, **self.NOTE}.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._t = threading.Thread(target=self._loop, daemon=True)
+            self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._t is not None:
+            self._t.join(timeout=2)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, target_s=15.0):
+    """Times the CPU oracle on a bounded, deterministic sample of the workload's level-0 seeds (every k-th seed, k
+    chosen from a small pilot run so that the timed run is about `target_s` seconds).  Returns (lines/s, steps/s,
+    cores, description)."""
+    import oracle
+    st = oracle.F32 if cfg["sample_type"] == "f32" else oracle.F64
+    f = oracle.Field(cfg["grid"], cfg["B"], st, oracle.NORMALIZE_FIRST)
+    seeds = cfg["seeds"]
+    n = len(seeds)
+    mode = cfg["mode"]
+    kw = dict(step_frac=cfg["step_frac"], mode=mode, max_steps=cfg["max_steps"], null_eps=cfg["null_eps"])
+    cores = os.cpu_count() or 1
+
+    def run(stride):
+        s = np.ascontiguousarray(seeds[::stride])
+        t0 = time.perf_counter()
+        o = oracle.trace(f, s, cfg["box_lo"], cfg["box_hi"], **kw)
+        return len(s), int(o["total_steps"]), time.perf_counter() - t0
+
+    pilot_stride = max(1, n // 4096)
+    m, steps, dt = run(pilot_stride)
+    rate = m / max(dt, 1e-6)                                   # lines/s of the pilot
+    stride = max(1, int(math.ceil(n / max(rate * target_s, 1.0))))
+    if stride < pilot_stride:
+        m, steps, dt = run(stride)
+    else:
+        stride = pilot_stride
+    desc = "every %d-th level-0 seed of %s (%d of %d lines, %d RK4 steps, %.1f s wall, OpenMP over lines, mode %s)" % (
+        stride, cfg["name"], m, n, steps, dt, "L+Q" if mode == 1 else "L")
+    return m / dt, steps / dt, cores, desc
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample of the workload."""
+    import oracle
+    st = oracle.F32 if cfg["sample_type"] == "f32" else oracle.F64
+    f = oracle.Field(cfg["grid"], cfg["B"], st, oracle.NORMALIZE_FIRST)
+    seeds = cfg["seeds"]
+    n = len(seeds)
+    kw = dict(step_frac=cfg["step_frac"], mode=cfg["mode"], max_steps=cfg["max_steps"], null_eps=cfg["null_eps"])
+    # size the per-step sample from a pilot so that warmup + steps finish in about two minutes
+    pilot = np.ascontiguousarray(seeds[::max(1, n // 2048)])
+    t0 = time.perf_counter()
+    oracle.trace(f, pilot, cfg["box_lo"], cfg["box_hi"], **kw)
+    rate = len(pilot) / max(time.perf_counter() - t0, 1e-6)
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    stride = max(1, int(math.ceil(n / max(rate * budget, 1.0))))
+    sample = np.ascontiguousarray(seeds[::stride])
+    for _ in range(args.warmup):
+        oracle.trace(f, sample, cfg["box_lo"], cfg["box_hi"], **kw)
+    t0 = time.perf_counter()
+    steps = 0
+    for _ in range(args.steps):
+        steps += int(oracle.trace(f, sample, cfg["box_lo"], cfg["box_hi"], **kw)["total_steps"])
+    dt = time.perf_counter() - t0
+    lines_s = len(sample) * args.steps / dt
+    cores = os.cpu_count() or 1
+    desc = "every %d-th level-0 seed of %s per step (%d lines/step), OpenMP over lines" % (stride, cfg["name"], len(sample))
+    line = {
+        "impl": "reference", "metric": "field lines/s (with Q)", "value": lines_s, "unit": "lines/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, args, sample=desc),
+        "rk_steps_per_s": steps / dt,
+        "cpu_baseline": {"value": lines_s, "unit": "lines/s", "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": lines_s, "unit": "lines/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, args, **extra):
+    g = cfg["grid"]
+    lat = cfg["lattice"]
+    c = {"workload": "%s: %s" % (cfg["name"], WORKLOADS[cfg["name"]]),
+         "field_grid": [g.nx, g.ny, g.nz], "field_samples": cfg["sample_type"],
+         "seed_lattice": [int(v) for v in lat.n], "n_seeds": int(len(cfg["seeds"])),
+         "trace_mode": "L+Q" if cfg["mode"] == 1 else "L", "refine_levels": int(cfg["levels"]),
+         "step_rule": "RK4, h = 0.25 x smallest cell edge", "parallelism": "replicas x%d" % args.gpus,
+         "l2": "flushed between timed steps (256 MiB write)"}
+    c.update(extra)
+    return c
+
+
+WORKLOADS = {
+    "cfg1": "BASELINE.json configs[0], hyperbolic field fp64 64^3, 128^2 seeds, L+Q",
+    "cfg2": "BASELINE.json configs[1], quadrupole fp64 128^3, 1024^2 photospheric seeds (|Bz|>1e-3), L+Q",
+    "cfg3": "BASELINE.json configs[2], quadrupole fp64 128^3, 2048x1024 vertical slice, FLEDGE + 4 refinement levels",
+    "cfg4": "BASELINE.json configs[3], LFFF fp32 samples 256^3, 256^3 seeds, L+Q",
+    "cfg5": "BASELINE.json configs[4], quadrupole+LFFF fp32 samples 512x512x256, 3-D FLEDGE + 3 refinement levels",
+}
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=sorted(WORKLOADS))
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink grid and seed lattice (debugging only)")
+    ap.add_argument("--flags", type=int, default=0, help="QSL_FLAG_* tuning flags (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+
+    import qsl_inputs as qi
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, qi.make_config(args.workload, args.scale))
+        return 0
+
+    import torch
+    import paper_1609_00724_b200 as qsl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libqsl has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = qi.make_config(args.workload, args.scale)
+    g = cfg["grid"]
+    dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda() for a in cfg["B"]]
+    st = qsl.QSL_F32 if cfg["sample_type"] == "f32" else qsl.QSL_F64
+    field = qsl.qsl_field_create(g.nx, g.ny, g.nz, *dev, lo=g.lo, hi=g.hi, sample_type=st)
+    del dev
+    seeds_host = torch.from_numpy(np.ascontiguousarray(cfg["seeds"])).pin_memory()
+    n = int(seeds_host.shape[0])
+    seeds = seeds_host.cuda()
+    mode = cfg["mode"]
+    levels = int(cfg["levels"])
+    mk = lambda m: qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=m, step_frac=cfg["step_frac"],
+                                         max_steps=cfg["max_steps"], null_eps=cfg["null_eps"], flags=args.flags)
+    pL, pLQ = mk(qsl.QSL_TRACE_L), mk(qsl.QSL_TRACE_LQ)
+    outs = ("end_f", "end_b", "L", "q_perp", "q_bnd", "face_f", "face_b", "status")
+    out_bufs = {}
+    tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    lat = cfg["lattice"]
+    qsl.qsl_profile_enable(True)
+
+    def step_device():
+        """One pass of the hot path, inputs resident.  Returns (lines traced, RK steps tensor)."""
+        if levels == 0:
+            res = qsl.qsl_trace(field, seeds, pLQ if mode == 1 else pL, outputs=outs, out=out_bufs, total_steps=tot)
+            out_bufs.update(res)
+            return n, tot
+        r = qsl.adaptive_map(field, lat, seeds, pL, pLQ, levels, cfg["p"])
+        return n + sum(int(s.shape[0]) for s in r["seeds"][1:]), r["total_steps"]
+
+    host_out = {}
+
+    def step_e2e():
+        """The same through HOST buffers: pinned seeds -> device, hot path, results -> pinned host."""
+        d = seeds_host.cuda(non_blocking=True)
+        if levels == 0:
+            res = qsl.qsl_trace(field, d, pLQ if mode == 1 else pL, outputs=outs, out=out_bufs, total_steps=tot)
+            results = [res[k] for k in outs]
+        else:
+            r = qsl.adaptive_map(field, lat, d, pL, pLQ, levels, cfg["p"])
+            results = [r["L0"], r["S0"]]
+            for lv in range(1, len(r["out"])):
+                if r["out"][lv] is not None:
+                    results += [r["coords"][lv], r["out"][lv]["L"], r["out"][lv]["q_perp"], r["out"][lv]["q_bnd"]]
+        nb = 0
+        for i, t in enumerate(results):
+            h = host_out.get(i)
+            if h is None or h.shape != t.shape:
+                h = host_out[i] = torch.empty(t.shape, dtype=t.dtype).pin_memory()
+            h.copy_(t, non_blocking=True)
+            nb += t.numel() * t.element_size()
+        return seeds_host.numel() * 8, nb
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------------------------------------
+    for _ in range(max(args.warmup, 3) if args.warmup > 0 else 0):
+        step_device()
+    barrier()
+    l0 = qsl.lib().qsl_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    lines = 0
+    rk = torch.zeros(1, dtype=torch.int64, device="cuda")
+    kern_ms = []
+    with ClockSampler(local) as clocks:
+        t_wall = time.perf_counter()
+        for a, b in ev:
+            flush.zero_()                      # L2 flush, outside the event pair
+            a.record()
+            m, s = step_device()
+            b.record()
+            rk += s
+            lines += m
+            if levels == 0:
+                kern_ms.append(qsl.qsl_profile_trace_kernel_ms())
+        barrier()
+        t_wall = time.perf_counter() - t_wall
+    launches = qsl.lib().qsl_launch_count() - l0
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev)
+    rk_steps = int(rk.item())
+    t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
+    agg = torch.tensor([float(lines), float(rk_steps)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(agg, op=dist.ReduceOp.SUM)
+    dev_ms_max = float(t.item())
+    lines_all, steps_all = float(agg[0].item()), float(agg[1].item())
+
+    # ---- end to end through host buffers ----------------------------------------------------------------------------
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2e_ms = 0.0
+    for _ in range(args.steps):
+        flush.zero_()
+        e0.record()
+        bi, bo = step_e2e()
+        e1.record()
+        e1.synchronize()
+        e2e_ms += e0.elapsed_time(e1)
+    barrier()
+    t2 = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+    e2e_ms_max = float(t2.item())
+
+    # ---- roofline of the dominant kernel (trace kernel) against the measured FP pipe peak ---------------------------
+    roofline = None
+    if rank == 0:
+        tag = "LQ" if mode == 1 else "L"
+        peak_fma = qsl.qsl_peak_fma(True)              # DFMA/s; arithmetic is fp64 whatever the sample type
+        peak = 2.0 * peak_fma / 1e12
+        if levels == 0 and kern_ms:
+            k_ms = sum(kern_ms) / len(kern_ms)
+            steps_per_launch = rk_steps / args.steps
+            achieved = 2.0 * PIPE_SLOTS_PER_STEP[tag] * steps_per_launch / (k_ms * 1e-3) / 1e12
+            roofline = {"bound": "alu", "kernel": "trace_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                        "frac": achieved / peak, "traffic": NCU_TRACE_KERNEL_DRAM_BYTES.get(args.workload),
+                        "kernel_ms": k_ms, "kernel_share_of_step": k_ms * args.steps / dev_ms,
+                        "convention": "FP64 pipe issue slots x 2 (FMA-equivalent flops): %d slots per RK4 step (%s); "
+                                      "peak = DFMA rate measured by qsl_peak_fma on this device" % (PIPE_SLOTS_PER_STEP[tag], tag),
+                        "true_flops_achieved_tflops": FLOPS_PER_STEP[tag] * steps_per_launch / (k_ms * 1e-3) / 1e12}
+        else:
+            # level loop: several trace launches of both modes per step; report the pipe fraction of the whole step
+            achieved = 2.0 * PIPE_SLOTS_PER_STEP["L"] * (rk_steps / args.steps) / (dev_ms / args.steps * 1e-3) / 1e12
+            roofline = {"bound": "alu", "kernel": "trace_kernel (all levels, whole step; lower bound: every step "
+                        "counted at the L-only cost)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                        "frac": achieved / peak, "traffic": None}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, sps, cores, desc = oracle_sample(cfg)
+        cpu = {"value": v, "unit": "lines/s", "cores": cores, "kind": "oracle", "sample": desc, "rk_steps_per_s": sps}
+
+    if rank == 0:
+        line = {
+            "metric": "field lines/s (with Q)", "value": lines_all / (dev_ms_max * 1e-3), "unit": "lines/s",
+            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3) if args.warmup > 0 else 0,
+            "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
+            "rk_steps_per_s": steps_all / (dev_ms_max * 1e-3), "rk_steps_per_step": rk_steps / args.steps,
+            "lines_per_step": lines / args.steps, "wall_s_timed_region": t_wall,
+            "clocks": clocks.summary(),
+            "e2e": {"value": lines_all / (e2e_ms_max * 1e-3), "unit": "lines/s", "h2d_bytes_per_step": bi,
+                    "d2h_bytes_per_step": bo, "ms_per_step": e2e_ms_max / args.steps},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

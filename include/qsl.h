@@ -157,6 +157,23 @@ int qsl_refine(int ndim, int level, long long n, const unsigned int *coords, con
  * space-filling curve), exposed so that tests can check it on its own.                                              */
 int qsl_debug_sort_pairs(unsigned int *keys, unsigned int *vals, long long n, int key_bits, void *stream);
 
+/* ---- measurement hooks (bench.py) ------------------------------------------------------------------ */
+/* qsl_profile_enable(1): every later qsl_trace records a CUDA event pair around its trace kernel (the dominant
+ * kernel) on the caller's stream.  qsl_profile_trace_kernel_ms waits for the most recent pair and returns the device
+ * time between them in milliseconds (host pointer); QSL_EINVAL if no trace ran with profiling on.                   */
+/* Number of kernels the library has launched in this process so far (bench.py's gpu_launches). */
+long long qsl_launch_count(void);
+int qsl_profile_enable(int on);
+int qsl_profile_trace_kernel_ms(double *ms);
+/* Roofline denominators measured on this device, each timed with CUDA events (2 warm-up launches, best of `reps`);
+ * both synchronise.  fma_per_s (host): fused multiply-adds per second of the plain FP pipe, fp64 != 0 -> DFMA, else
+ * FFMA, from 8 independent register-only chains per thread.  samples_per_s (host): divergent pseudo-random gathers per
+ * second of one 16-byte (float4) or 32-byte (double4) sample per lane over a zero-filled scratch buffer of
+ * footprint_bytes (rounded down to a power of two), i.e. the tracer's load shape with an L1-, L2- or HBM-resident
+ * field.  Errors: QSL_EINVAL, QSL_ENOMEM, QSL_ECUDA.                                                                */
+int qsl_peak_fma(int fp64, int reps, double *fma_per_s, void *stream);
+int qsl_peak_gather(int bytes_per_sample, long long footprint_bytes, int reps, double *samples_per_s, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -271,3 +271,32 @@ def qsl_refine(lattice, level: int, coords, S: torch.Tensor, tau: torch.Tensor, 
                             C.c_void_p(cs.data_ptr()), C.c_void_p(cb.data_ptr()), C.byref(m), _stream_ptr(stream)),
            "qsl_refine")
     return cc[: m.value], cs[: m.value], cb
+
+
+# ---- measurement hooks (bench.py) ----------------------------------------------------------------------------------
+def qsl_profile_enable(on: bool = True):
+    _require_cuda()
+    _check(lib().qsl_profile_enable(C.c_int(1 if on else 0)), "qsl_profile_enable")
+
+
+def qsl_profile_trace_kernel_ms() -> float:
+    ms = C.c_double(0.0)
+    _check(lib().qsl_profile_trace_kernel_ms(C.byref(ms)), "qsl_profile_trace_kernel_ms")
+    return ms.value
+
+
+def qsl_peak_fma(fp64: bool, reps: int = 5, stream=None) -> float:
+    """Measured FMA issue rate (FMA/s) of the plain FP pipe: DFMA if fp64 else FFMA."""
+    _require_cuda()
+    v = C.c_double(0.0)
+    _check(lib().qsl_peak_fma(C.c_int(1 if fp64 else 0), C.c_int(reps), C.byref(v), _stream_ptr(stream)), "qsl_peak_fma")
+    return v.value
+
+
+def qsl_peak_gather(bytes_per_sample: int, footprint_bytes: int, reps: int = 5, stream=None) -> float:
+    """Measured rate (samples/s) of divergent 16 B / 32 B gathers over a footprint of the given size."""
+    _require_cuda()
+    v = C.c_double(0.0)
+    _check(lib().qsl_peak_gather(C.c_int(bytes_per_sample), C.c_longlong(footprint_bytes), C.c_int(reps), C.byref(v),
+                                 _stream_ptr(stream)), "qsl_peak_gather")
+    return v.value

@@ -9,6 +9,7 @@
 namespace qsl {
 
 int g_last_cuda_error = 0;
+long long g_launches = 0;
 int record_cuda(cudaError_t e)
 {
     g_last_cuda_error = (int)e;
@@ -89,6 +90,7 @@ const char *qsl_strerror(int code)
     }
 }
 int qsl_last_cuda_error(void) { return g_last_cuda_error; }
+long long qsl_launch_count(void) { return g_launches; }
 int qsl_version(void) { return 100; }
 int qsl_compiled_arch(void)
 {
@@ -160,6 +162,7 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     }
     const int threads = 256;
     const int blocks = (int)((n + threads - 1) / threads < (long long)sm_count() * 16 ? (n + threads - 1) / threads : (long long)sm_count() * 16);
+    count_launch();
     if (d->sample_type == QSL_F32)
         pack_kernel<float4, float><<<blocks, threads, 0, s>>>(n, bx, by, bz, d->interp_mode, (float4 *)f->d_samples);
     else

@@ -163,6 +163,7 @@ extern "C" int qsl_fledge_dense(int ndim, const long long dims[3], const double 
     long long blocks = (tasks + wpb - 1) / wpb;
     const long long cap = (long long)sm_count() * 32;      // a multiple of the SM count; warps stride over the tasks
     if (blocks > cap) blocks = cap;
+    count_launch();
     if (ndim == 2) fledge_dense_kernel<2><<<(unsigned)blocks, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
     else fledge_dense_kernel<3><<<(unsigned)blocks, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
     QSL_CUDA(cudaGetLastError());
@@ -191,6 +192,7 @@ extern "C" int qsl_fledge_sparse(const qsl_levels *lv, int level, double *S, voi
     A.S = S;
     cudaStream_t s = (cudaStream_t)stream;
     const long long blocks = (A.count + FL_THREADS - 1) / FL_THREADS;
+    count_launch();
     if (ndim == 2) fledge_sparse_kernel<2><<<(unsigned)blocks, FL_THREADS, 0, s>>>(A);
     else fledge_sparse_kernel<3><<<(unsigned)blocks, FL_THREADS, 0, s>>>(A);
     QSL_CUDA(cudaGetLastError());

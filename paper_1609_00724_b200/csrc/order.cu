@@ -121,10 +121,12 @@ int radix_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_
         const unsigned blocks = (unsigned)((n_chunks + SORT_WARPS - 1) / SORT_WARPS);
         uint32_t *ki = keys, *vi = vals, *ko = keys_tmp, *vo = vals_tmp;
         for (int p = 0; p < passes && e == cudaSuccess; ++p) {
+            count_launch();
             sort_hist_kernel<<<blocks, SORT_THREADS, 0, s>>>(n, ki, 8 * p, n_chunks, (uint32_t *)counts);
             e = exclusive_scan_u32(table, (const uint32_t *)counts, (unsigned long long *)offsets, (unsigned long long *)tiles,
                                    (unsigned long long *)total, s);
             if (e != cudaSuccess) break;
+            count_launch();
             sort_scatter_kernel<<<blocks, SORT_THREADS, 0, s>>>(n, ki, vi, 8 * p, n_chunks, (const unsigned long long *)offsets, ko, vo);
             e = cudaGetLastError();
             uint32_t *t = ki; ki = ko; ko = t;
@@ -140,6 +142,7 @@ int morton_order(const FieldView &fv, long long n, const double *seeds, uint32_t
 {
     const unsigned blocks = (unsigned)((n + 255) / 256);
     if (!sort || n < 2) {
+        count_launch();
         iota_kernel<<<blocks, 256, 0, s>>>(n, perm);
         QSL_CUDA(cudaGetLastError());
         return QSL_OK;
@@ -155,6 +158,7 @@ int morton_order(const FieldView &fv, long long n, const double *seeds, uint32_t
     if (rc == QSL_OK) rc = scratch_alloc(&kt, sizeof(uint32_t) * (size_t)n, s);
     if (rc == QSL_OK) rc = scratch_alloc(&vt, sizeof(uint32_t) * (size_t)n, s);
     if (rc == QSL_OK) {
+        count_launch();
         morton_key_kernel<<<blocks, 256, 0, s>>>(fv, n, seeds, shift, (uint32_t *)keys, perm);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) rc = record_cuda(e);

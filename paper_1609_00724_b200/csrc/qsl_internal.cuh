@@ -23,6 +23,10 @@ void scratch_free(void *p, cudaStream_t s);
 
 int sm_count();
 
+// Number of kernels launched by the library so far (qsl_launch_count; bench.py's gpu_launches).
+extern long long g_launches;
+inline void count_launch() { ++g_launches; }
+
 // Device view of a packed field: AoS samples (v0, v1, v2, |B|), x fastest.
 struct FieldView {
     const void *samples;      // float4* or double4*

@@ -96,8 +96,11 @@ static inline cudaError_t exclusive_scan_u32(long long n, const uint32_t *in, un
 {
     const long long tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     if (tiles == 0) return cudaMemsetAsync(total, 0, sizeof(unsigned long long), s);
+    count_launch();
     scan_tile_sums<<<(unsigned)tiles, SCAN_THREADS, 0, s>>>(n, in, tile_sums);
+    count_launch();
     scan_single_block<<<1, 1024, 0, s>>>(tiles, tile_sums, total);
+    count_launch();
     scan_tiles<<<(unsigned)tiles, SCAN_THREADS, 0, s>>>(n, in, tile_sums, out);
     return cudaGetLastError();
 }

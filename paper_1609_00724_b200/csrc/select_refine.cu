@@ -160,7 +160,9 @@ extern "C" int qsl_select(long long n, const double *S, double p, double *tau, v
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
     for (int pass = 0; pass < 8 && e == cudaSuccess; ++pass) {
+        count_launch();
         select_hist_kernel<<<(unsigned)blocks, 256, 0, s>>>(n, S, pass, st);
+        count_launch();
         select_pick_kernel<<<1, 256, 0, s>>>(pass, p, st, tau);
         e = cudaGetLastError();
     }
@@ -203,10 +205,12 @@ extern "C" int qsl_refine(int ndim, int level, long long n, const unsigned int *
     unsigned long long h_total = 0;
     if (rc == QSL_OK) {
         const unsigned blocks = (unsigned)((n + 255) / 256);
+        count_launch();
         refine_flag_kernel<<<blocks, 256, 0, s>>>(n, S, tau, (uint32_t *)flags);
         cudaError_t e = exclusive_scan_u32(n, (const uint32_t *)flags, (unsigned long long *)offs, (unsigned long long *)tiles,
                                            (unsigned long long *)total, s);
         if (e == cudaSuccess) {
+            count_launch();
             if (ndim == 2) refine_emit_kernel<2><<<blocks, 256, 0, s>>>(A, (const uint32_t *)flags, (const unsigned long long *)offs);
             else refine_emit_kernel<3><<<blocks, 256, 0, s>>>(A, (const uint32_t *)flags, (const unsigned long long *)offs);
             e = cudaGetLastError();

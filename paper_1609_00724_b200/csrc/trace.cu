@@ -13,6 +13,31 @@ cudaError_t launch_epilogue_f64(const EpilogueArgs &E, cudaStream_t s);
 
 using namespace qsl;
 
+// Measurement hook: an event pair around the trace kernel (qsl_profile_enable / qsl_profile_trace_kernel_ms).
+static int g_profile = 0, g_profile_valid = 0;
+static cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+
+extern "C" int qsl_profile_enable(int on)
+{
+    if (on && !g_ev0) {
+        QSL_CUDA(cudaEventCreate(&g_ev0));
+        QSL_CUDA(cudaEventCreate(&g_ev1));
+    }
+    g_profile = on ? 1 : 0;
+    g_profile_valid = 0;
+    return QSL_OK;
+}
+
+extern "C" int qsl_profile_trace_kernel_ms(double *ms)
+{
+    if (!ms || !g_profile_valid) return QSL_EINVAL;
+    QSL_CUDA(cudaEventSynchronize(g_ev1));
+    float t = 0.f;
+    QSL_CUDA(cudaEventElapsedTime(&t, g_ev0, g_ev1));
+    *ms = (double)t;
+    return QSL_OK;
+}
+
 extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long long n, const double *seeds,
                          const qsl_trace_out *out, unsigned long long *total_steps, void *stream)
 {
@@ -53,8 +78,10 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         A.perm = (const uint32_t *)perm; A.rec = (double *)rec; A.queue = (unsigned long long *)queue;
         e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
         const bool dev = p->mode == QSL_TRACE_LQ;
+        if (e == cudaSuccess && g_profile) e = cudaEventRecord(g_ev0, s);
         if (e == cudaSuccess)
             e = f->sample_type == QSL_F32 ? launch_trace_f32(A, dev, refill, s) : launch_trace_f64(A, dev, refill, s);
+        if (e == cudaSuccess && g_profile) { e = cudaEventRecord(g_ev1, s); g_profile_valid = 1; }
         if (e == cudaSuccess) {
             EpilogueArgs E;
             E.T = A; E.with_dev = dev ? 1 : 0; E.out = *out;

@@ -11,6 +11,7 @@ static cudaError_t launch_trace_variant(const TraceArgs &A, bool refill, cudaStr
     const int threads = 128;
     if (!refill) {
         const long long blocks = (n_items + threads - 1) / threads;
+        count_launch();
         trace_kernel<S, DEV, STRETCHED, INTERP, false><<<(unsigned)blocks, threads, 0, s>>>(A);
     } else {
         int per_sm = 0;
@@ -20,6 +21,7 @@ static cudaError_t launch_trace_variant(const TraceArgs &A, bool refill, cudaStr
         long long blocks = (long long)sm_count() * per_sm;          // persistent: every CTA resident, grid = SMs x occupancy
         const long long need = (n_items + threads - 1) / threads;
         if (blocks > need) blocks = need;
+        count_launch();
         trace_kernel<S, DEV, STRETCHED, INTERP, true><<<(unsigned)blocks, threads, 0, s>>>(A);
     }
     return cudaGetLastError();
@@ -30,6 +32,7 @@ static cudaError_t launch_epilogue_variant(const EpilogueArgs &E, cudaStream_t s
 {
     const int threads = 128;
     const long long blocks = (E.T.n + threads - 1) / threads;
+    count_launch();
     epilogue_kernel<S, STRETCHED, INTERP><<<(unsigned)blocks, threads, 0, s>>>(E);
     return cudaGetLastError();
 }
