@@ -38,6 +38,7 @@ enum { QSL_F32 = 0, QSL_F64 = 1 };                       /* storage type of the 
 enum { QSL_NORMALIZE_FIRST = 0, QSL_INTERP_FIRST = 1 };  /* PAPER.md:178 (fn. 9) = NORMALIZE_FIRST, the default   */
 enum { QSL_RK4 = 0, QSL_EULER = 1 };                     /* PAPER.md:141; RK4: BASELINE.json configs (reading A5) */
 enum { QSL_TRACE_L = 0, QSL_TRACE_LQ = 1 };              /* L only (FLEDGE pass) | L and Q                        */
+enum { QSL_LAYOUT_CELL_TABLE = 0, QSL_LAYOUT_NODES_ONLY = 1 };  /* what qsl_field_create keeps in HBM (see qsl_grid_desc) */
 enum { QSL_ARITH_F64 = 0, QSL_ARITH_F32 = 1 };           /* arithmetic of the integrator (F32 only with F32 samples) */
 
 /* status bits of qsl_trace_out.status */
@@ -52,7 +53,7 @@ enum { QSL_ARITH_F64 = 0, QSL_ARITH_F32 = 1 };           /* arithmetic of the in
 /* tuning flags of qsl_trace_params.flags (results never depend on them) */
 #define QSL_FLAG_NO_SORT    1u    /* do not Morton-order the seeds before tracing                                  */
 #define QSL_FLAG_NO_REFILL  2u    /* one work item per thread instead of the persistent work queue                 */
-#define QSL_FLAG_KERNEL_V1  4u    /* baseline kernel: 8 AoS gathers per RK stage, no per-thread cell cache         */
+#define QSL_FLAG_KERNEL_V1  4u    /* corner kernel: 8 AoS sample gathers per RK stage instead of the per-cell table  */
 
 /* ---- field (PAPER.md:54 input cubes; :93-107 eq. 3-4 interpolation; :178 normalise-then-interpolate) --------- */
 typedef struct qsl_field qsl_field;          /* opaque, library-owned */
@@ -64,6 +65,11 @@ typedef struct {
     const double *xs, *ys, *zs;  /* HOST arrays of nx, ny, nz strictly increasing coordinates; only if stretched  */
     int sample_type;             /* QSL_F32 | QSL_F64: storage type of the packed samples                         */
     int interp_mode;             /* QSL_NORMALIZE_FIRST (paper) | QSL_INTERP_FIRST (reading A2)                   */
+    int layout;                  /* QSL_LAYOUT_CELL_TABLE (default): besides the packed node samples, keep per cell the
+                                    24 fp64 monomial coefficients of its trilinear interpolant (192 B per cell; 6x the
+                                    fp64 samples, 12x the fp32 samples) - what the fast trace kernel reads.
+                                    QSL_LAYOUT_NODES_ONLY: packed samples only; qsl_trace then gathers 8 corners per
+                                    RK stage (the slower QSL_FLAG_KERNEL_V1 path), for fields too large for the table */
 } qsl_grid_desc;
 
 /* Packs the three component cubes (DEVICE, fp64, nx*ny*nz each) into one AoS array of (b^x, b^y, b^z, |B|) samples

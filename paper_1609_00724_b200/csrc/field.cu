@@ -72,6 +72,55 @@ __global__ void __launch_bounds__(256) pack_kernel(long long n, const double *__
     }
 }
 
+// Per-cell polynomial table of the V2 trace kernel: the trilinear interpolant of each component c (eq. 3,
+// :101-107 eq. 4) inside cell (i, j, k), written in monomials of the physical offset d = x - x_cell,
+//     v_c(d) = sum_{m in {0,1}^3} a[c][m] dx^{m0} dy^{m1} dz^{m2},      m = m0 + 2 m1 + 4 m2,
+// so that value and analytic gradient cost 11 FMAs per component instead of 25 from the corners.
+// The coefficients are finite differences of the 8 corner samples (converted exactly to fp64) divided by the cell
+// edges; 24 doubles = 192 B per cell, component-major, cell index (k (ny-1) + j)(nx-1) + i.
+template <typename S4>
+__global__ void __launch_bounds__(256) cell_table_kernel(FieldView fv, double4 *__restrict__ cells)
+{
+    const int cx = fv.nx - 1, cy = fv.ny - 1, cz = fv.nz - 1;
+    const long long n_cells = (long long)cx * cy * cz;
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const S4 *__restrict__ smp = (const S4 *)fv.samples;
+    for (; p < n_cells; p += stride) {
+        const int i = (int)(p % cx), j = (int)((p / cx) % cy), k = (int)(p / ((long long)cx * cy));
+        const double ihx = 1.0 / (fv.axis[0][i + 1] - fv.axis[0][i]), ihy = 1.0 / (fv.axis[1][j + 1] - fv.axis[1][j]),
+                     ihz = 1.0 / (fv.axis[2][k + 1] - fv.axis[2][k]);
+        const size_t base = ((size_t)k * fv.ny + j) * fv.nx + i, sy = (size_t)fv.nx, sz = (size_t)fv.nx * fv.ny;
+        const S4 s[8] = { smp[base], smp[base + 1], smp[base + sy], smp[base + sy + 1],
+                          smp[base + sz], smp[base + sz + 1], smp[base + sz + sy], smp[base + sz + sy + 1] };
+        double a[24];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double v[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v[q] = c == 0 ? (double)s[q].x : (c == 1 ? (double)s[q].y : (double)s[q].z);
+            // finite differences along x, then y, then z (in place): v[m] becomes the coefficient of monomial m in t
+#pragma unroll
+            for (int q = 0; q < 8; q += 2) v[q + 1] -= v[q];
+#pragma unroll
+            for (int q = 0; q < 8; q += 4) { v[q + 2] -= v[q]; v[q + 3] -= v[q + 1]; }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) v[q + 4] -= v[q];
+            a[8 * c + 0] = v[0];
+            a[8 * c + 1] = v[1] * ihx;
+            a[8 * c + 2] = v[2] * ihy;
+            a[8 * c + 3] = v[3] * (ihx * ihy);
+            a[8 * c + 4] = v[4] * ihz;
+            a[8 * c + 5] = v[5] * (ihx * ihz);
+            a[8 * c + 6] = v[6] * (ihy * ihz);
+            a[8 * c + 7] = v[7] * ((ihx * ihy) * ihz);
+        }
+        double4 *o = cells + (size_t)p * 6;
+#pragma unroll
+        for (int q = 0; q < 6; ++q) o[q] = make_double4(a[4 * q], a[4 * q + 1], a[4 * q + 2], a[4 * q + 3]);
+    }
+}
+
 }  // namespace qsl
 
 using namespace qsl;
@@ -109,6 +158,7 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     if (d->nx < 2 || d->ny < 2 || d->nz < 2) return QSL_EINVAL;
     if (d->sample_type != QSL_F32 && d->sample_type != QSL_F64) return QSL_EINVAL;
     if (d->interp_mode != QSL_NORMALIZE_FIRST && d->interp_mode != QSL_INTERP_FIRST) return QSL_EINVAL;
+    if (d->layout != QSL_LAYOUT_CELL_TABLE && d->layout != QSL_LAYOUT_NODES_ONLY) return QSL_EINVAL;
     const long long n = (long long)d->nx * d->ny * d->nz;
     if (n >= (1ll << 31)) return QSL_ERANGE;   // node index is 32-bit inside the gather
     const int dims[3] = { d->nx, d->ny, d->nz };
@@ -127,6 +177,8 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     qsl_field *f = new (std::nothrow) qsl_field();
     if (!f) return QSL_ENOMEM;
     f->d_samples = nullptr;
+    f->d_cells = nullptr;
+    f->view.cells = nullptr;
     for (int a = 0; a < 3; ++a) f->d_axis[a] = nullptr;
     f->sample_type = d->sample_type;
     f->n_nodes = n;
@@ -169,6 +221,21 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
         pack_kernel<double4, double><<<blocks, threads, 0, s>>>(n, bx, by, bz, d->interp_mode, (double4 *)f->d_samples);
     e = cudaGetLastError();
     if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+    if (d->layout == QSL_LAYOUT_CELL_TABLE) {
+        const long long n_cells = (long long)(d->nx - 1) * (d->ny - 1) * (d->nz - 1);
+        const size_t cbytes = (size_t)n_cells * 24 * sizeof(double);
+        e = cudaMalloc(&f->d_cells, cbytes);
+        if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+        f->bytes += cbytes;
+        const long long want = (n_cells + threads - 1) / threads, cap = (long long)sm_count() * 16;
+        const int cblocks = (int)(want < cap ? want : cap);
+        count_launch();
+        if (d->sample_type == QSL_F32) cell_table_kernel<float4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
+        else cell_table_kernel<double4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+        f->view.cells = f->d_cells;
+    }
     *out = f;
     return QSL_OK;
 }
@@ -177,6 +244,7 @@ int qsl_field_destroy(qsl_field *f)
 {
     if (!f) return QSL_OK;
     if (f->d_samples) cudaFree(f->d_samples);
+    if (f->d_cells) cudaFree(f->d_cells);
     for (int a = 0; a < 3; ++a)
         if (f->d_axis[a]) cudaFree(f->d_axis[a]);
     delete f;

@@ -30,6 +30,7 @@ inline void count_launch() { ++g_launches; }
 // Device view of a packed field: AoS samples (v0, v1, v2, |B|), x fastest.
 struct FieldView {
     const void *samples;      // float4* or double4*
+    const void *cells;        // double4[6] per cell: monomial coefficients of the trilinear interpolant, or NULL
     int nx, ny, nz;
     int stretched;
     int interp_mode;
@@ -49,6 +50,7 @@ int morton_order(const FieldView &fv, long long n, const double *seeds, uint32_t
 struct qsl_field {
     qsl::FieldView view;
     void *d_samples;
+    void *d_cells;
     double *d_axis[3];
     int sample_type;
     long long n_nodes;

@@ -7,6 +7,7 @@
 namespace qsl {
 cudaError_t launch_trace_f32(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 cudaError_t launch_trace_f64(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
+cudaError_t launch_trace2(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 cudaError_t launch_epilogue_f32(const EpilogueArgs &E, cudaStream_t s);
 cudaError_t launch_epilogue_f64(const EpilogueArgs &E, cudaStream_t s);
 }  // namespace qsl
@@ -79,8 +80,10 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
         const bool dev = p->mode == QSL_TRACE_LQ;
         if (e == cudaSuccess && g_profile) e = cudaEventRecord(g_ev0, s);
+        const bool v2 = f->view.cells != nullptr && !(p->flags & QSL_FLAG_KERNEL_V1);
         if (e == cudaSuccess)
-            e = f->sample_type == QSL_F32 ? launch_trace_f32(A, dev, refill, s) : launch_trace_f64(A, dev, refill, s);
+            e = v2 ? launch_trace2(A, dev, refill, s)
+                   : (f->sample_type == QSL_F32 ? launch_trace_f32(A, dev, refill, s) : launch_trace_f64(A, dev, refill, s));
         if (e == cudaSuccess && g_profile) { e = cudaEventRecord(g_ev1, s); g_profile_valid = 1; }
         if (e == cudaSuccess) {
             EpilogueArgs E;

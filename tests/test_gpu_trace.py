@@ -12,7 +12,10 @@ from tests.parity import compare_trace, cpu_field, gpu_field, run_both
 
 pytestmark = pytest.mark.gpu
 
-ALL_FLAGS = [0, qsl.QSL_FLAG_NO_REFILL, qsl.QSL_FLAG_NO_SORT, qsl.QSL_FLAG_NO_REFILL | qsl.QSL_FLAG_NO_SORT]
+V1 = qsl.QSL_FLAG_KERNEL_V1
+ALL_FLAGS = [0, qsl.QSL_FLAG_NO_REFILL, qsl.QSL_FLAG_NO_SORT, qsl.QSL_FLAG_NO_REFILL | qsl.QSL_FLAG_NO_SORT,
+             V1, V1 | qsl.QSL_FLAG_NO_REFILL, V1 | qsl.QSL_FLAG_NO_SORT]
+KERNELS = [0, V1]          # per-cell table kernel (default) and corner-gather kernel
 
 
 @pytest.mark.parametrize("sample_type", ["f32", "f64"])
@@ -44,10 +47,12 @@ def test_cfg1_full_size_all_launch_modes(flags):
     assert np.abs(g["dev_f"][uniq] - c["dev_f"][uniq]).max() < 1e-9 * np.abs(c["dev_f"]).max()
 
 
-def test_cfg1_closed_form_interp_first():
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_cfg1_closed_form_interp_first(kernel):
     """The CUDA path itself against the closed forms of the hyperbolic field (north_star): Q = e^{2kh} + e^{-2kh}."""
     cfg = qi.make_config("cfg1")
-    g, c = run_both(cfg["grid"], cfg["B"], "f64", cfg["seeds"], cfg["box_lo"], cfg["box_hi"], interp_mode=qsl.QSL_INTERP_FIRST)
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", cfg["seeds"], cfg["box_lo"], cfg["box_hi"], interp_mode=qsl.QSL_INTERP_FIRST,
+                    flags=kernel)
     compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], label="cfg1 interp-first")
     s = cfg["seeds"]; k = 2.0
     top = np.abs(s[:, 0]) <= math.exp(-k)
@@ -56,64 +61,69 @@ def test_cfg1_closed_form_interp_first():
     assert np.allclose(g["q_bnd"][top], 54.61646567, rtol=1e-9)
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("sample_type", ["f32", "f64"])
 @pytest.mark.parametrize("mode", [qsl.QSL_TRACE_L, qsl.QSL_TRACE_LQ])
-def test_quadrupole_volume_seeds(sample_type, mode):
+def test_quadrupole_volume_seeds(sample_type, mode, kernel):
     """cfg3-like: quadrupole, bidirectional lines from a vertical slice, ragged lengths, both storage types."""
     cfg = qi.make_config("cfg3", scale=0.25)                         # 32^3 grid
     rng = np.random.default_rng(21)
     seeds = cfg["seeds"][rng.choice(len(cfg["seeds"]), 3000, replace=False)]
     g, c = run_both(cfg["grid"], cfg["B"], sample_type, seeds, cfg["box_lo"], cfg["box_hi"], mode=mode,
-                    max_steps=cfg["max_steps"])
+                    max_steps=cfg["max_steps"], flags=kernel)
     compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], with_q=mode == qsl.QSL_TRACE_LQ, label="quad")
 
 
-def test_P12_gpu_L_mode_bit_identical_to_LQ():
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_P12_gpu_L_mode_bit_identical_to_LQ(kernel):
     cfg = qi.make_config("cfg3", scale=0.25)
     seeds = cfg["seeds"][::41]
     fg = gpu_field(cfg["grid"], cfg["B"], "f64", 0)
     s = torch.from_numpy(seeds).cuda()
-    a = qsl.qsl_trace(fg, s, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=qsl.QSL_TRACE_LQ, max_steps=cfg["max_steps"]))
-    b = qsl.qsl_trace(fg, s, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=qsl.QSL_TRACE_L, max_steps=cfg["max_steps"]))
+    mk = lambda m: qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=m, max_steps=cfg["max_steps"], flags=kernel)
+    a = qsl.qsl_trace(fg, s, mk(qsl.QSL_TRACE_LQ))
+    b = qsl.qsl_trace(fg, s, mk(qsl.QSL_TRACE_L))
     for k in ("end_f", "end_b", "L", "face_f", "face_b", "nsteps_f", "nsteps_b", "status"):
         assert torch.equal(a[k], b[k]), k
     assert torch.isnan(b["q_perp"]).all()
 
 
-def test_stretched_grid_and_euler():
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_stretched_grid_and_euler(kernel):
     g = qi.Grid.from_axes(qi.stretched_axis(40, -1, 1, 3.0), qi.stretched_axis(36, -1, 1, 0.4), qi.stretched_axis(44, 0, 1, 5.0))
     B = qi.hyperbolic_field(g, 2.0)
     rng = np.random.default_rng(22)
     seeds = np.stack([rng.uniform(-0.5, 0.5, 500), rng.uniform(-0.5, 0.5, 500), rng.uniform(0, 0.9, 500)], 1)
     lo, hi = (-1, -1, 0), (1, 1, 1)
     for interp in (0, 1):
-        gg, c = run_both(g, B, "f64", seeds, lo, hi, interp_mode=interp)
+        gg, c = run_both(g, B, "f64", seeds, lo, hi, interp_mode=interp, flags=kernel)
         compare_trace(gg, c, lo, hi, label="stretched interp=%d" % interp)
-    gg, c = run_both(g, B, "f64", seeds, lo, hi, method=qsl.QSL_EULER, step_frac=0.2)
+    gg, c = run_both(g, B, "f64", seeds, lo, hi, method=qsl.QSL_EULER, step_frac=0.2, flags=kernel)
     compare_trace(gg, c, lo, hi, label="stretched euler")
 
 
-def test_edge_cases_status_caps_empty():
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_edge_cases_status_caps_empty(kernel):
     cfg = qi.make_config("cfg1", scale=0.25)
     lo, hi = cfg["box_lo"], cfg["box_hi"]
     seeds = np.array([[0.0, 0.0, 0.5], [2.0, 0.0, 0.5], [0.1, 0.1, 0.2], [1.0, 1.0, 1.0], [-1.0, 0.3, 0.0], [0.3, 0.2, 0.0]])
     for kw in (dict(max_steps=3), dict(max_length=0.1), dict()):
-        g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, lo, hi, **kw)
+        g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, lo, hi, flags=kernel, **kw)
         compare_trace(g, c, lo, hi, frac=1.0, label=str(kw))
         assert np.array_equal(g["status"], c["status"])
     # raised lower boundary (PAPER.md:232)
-    g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, (-1, -1, 0.25), hi)
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, (-1, -1, 0.25), hi, flags=kernel)
     compare_trace(g, c, (-1, -1, 0.25), hi, frac=1.0, label="raised")
     # null field
     gz = qi.Grid.uniform((8, 8, 8), lo, hi)
-    g, c = run_both(gz, tuple(np.zeros(gz.shape) for _ in range(3)), "f64", seeds[:3], lo, hi)
+    g, c = run_both(gz, tuple(np.zeros(gz.shape) for _ in range(3)), "f64", seeds[:3], lo, hi, flags=kernel)
     assert np.array_equal(g["status"], c["status"]) and np.isnan(g["q_perp"]).all()
     # n = 0
     fg = gpu_field(cfg["grid"], cfg["B"], "f64", 0)
     out = qsl.qsl_trace(fg, torch.empty((0, 3), dtype=torch.float64, device="cuda"), qsl.make_trace_params(lo, hi))
     assert out["L"].numel() == 0
     # a ragged tail: n not a multiple of the block or warp size
-    g, c = run_both(cfg["grid"], cfg["B"], "f64", cfg["seeds"][:131], lo, hi)
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", cfg["seeds"][:131], lo, hi, flags=kernel)
     compare_trace(g, c, lo, hi, frac=1.0, label="tail")
 
 
@@ -128,3 +138,22 @@ def test_bad_arguments_are_reported_not_crashed():
     with pytest.raises(qsl.QslError):
         z = torch.zeros(8, dtype=torch.float64, device="cuda")
         qsl.qsl_field_create(1, 2, 4, z, z, z, lo=(0, 0, 0), hi=(1, 1, 1))
+
+
+def test_nodes_only_layout_uses_corner_kernel_and_matches():
+    """QSL_LAYOUT_NODES_ONLY keeps no per-cell table (6x / 12x less HBM); qsl_trace then runs the corner kernel."""
+    cfg = qi.make_config("cfg3", scale=0.25)
+    seeds = cfg["seeds"][::37]
+    dev = [torch.from_numpy(np.ascontiguousarray(a).reshape(-1)).cuda() for a in cfg["B"]]
+    gr = cfg["grid"]
+    ft = qsl.qsl_field_create(gr.nx, gr.ny, gr.nz, *dev, lo=gr.lo, hi=gr.hi)
+    fn = qsl.qsl_field_create(gr.nx, gr.ny, gr.nz, *dev, lo=gr.lo, hi=gr.hi, layout=qsl.QSL_LAYOUT_NODES_ONLY)
+    n_nodes, n_cells = gr.nx * gr.ny * gr.nz, (gr.nx - 1) * (gr.ny - 1) * (gr.nz - 1)
+    assert fn.nbytes < n_nodes * 32 + 4096 and ft.nbytes >= n_nodes * 32 + n_cells * 192
+    s = torch.from_numpy(seeds).cuda()
+    p = qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], max_steps=cfg["max_steps"])
+    pv1 = qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], max_steps=cfg["max_steps"], flags=V1)
+    a, b = qsl.qsl_trace(fn, s, p), qsl.qsl_trace(ft, s, pv1)
+    for k in a:
+        assert torch.equal(a[k], b[k]) or (torch.isnan(a[k]) == torch.isnan(b[k])).all() and torch.equal(
+            torch.nan_to_num(a[k]), torch.nan_to_num(b[k])), k
