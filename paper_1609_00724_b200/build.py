@@ -15,6 +15,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqsl.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "-DQSL_TARGET_ARCH=100", "-I" + os.path.join(ROOT, "include"), "-I" + CSRC]
+NVCC_FLAGS += os.environ.get("QSL_NVCC_EXTRA", "").split()      # e.g. -DQSL_T2_MIN_BLOCKS=2 for tuning experiments
 
 
 def _nvcc() -> str:

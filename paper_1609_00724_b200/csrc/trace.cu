@@ -1,6 +1,7 @@
 // qsl_trace: host entry point.  Orders the seeds, runs the trace kernel over 2n work items
 // (one per direction), then the Q/L epilogue, all asynchronously on the caller's stream.
 #include <math.h>
+#include <string.h>
 
 #include "trace_kernels.cuh"
 
@@ -60,6 +61,7 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
     for (int d = 0; d < 3; ++d) {
         A.inv_h[d] = 1.0 / f->view.h[d];
         A.box_lo[d] = p->box_lo[d]; A.box_hi[d] = p->box_hi[d];
+        { unsigned long long bits; memcpy(&bits, &f->view.h[d], 8); A.h_hi[d] = (unsigned)(bits >> 32); }
     }
     A.h_uniform = p->step_frac * fmin(f->view.h[0], fmin(f->view.h[1], f->view.h[2]));
     A.step_frac = p->step_frac; A.max_length = p->max_length; A.null_eps = p->null_eps;

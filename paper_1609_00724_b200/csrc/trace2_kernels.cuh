@@ -21,11 +21,12 @@ __device__ __forceinline__ double4 load_cell4(const double4 *p)
     return r;
 }
 
-// 0 <= a < b for b > 0, as one unsigned 64-bit integer compare of the bit patterns (runs on the integer pipe, not on
-// the FP64 pipe).  False for negative a (sign bit set), -0.0 and NaN.
-__device__ __forceinline__ bool in_range_bits(double a, double b)
+// Sufficient test for 0 <= a < b (b > 0) on the high 32 bits of the bit patterns: one unsigned integer compare on
+// the integer pipe instead of two DSETP on the FP64 pipe.  False for negative a (sign bit set), -0.0, NaN, and for a
+// within 2^-20 (relative) below b: a false negative only costs a redundant relocate, which finds the right cell.
+__device__ __forceinline__ bool in_range_hi(double a, unsigned b_hi)
 {
-    return (unsigned long long)__double_as_longlong(a) < (unsigned long long)__double_as_longlong(b);
+    return (unsigned)__double2hiint(a) < b_hi;
 }
 
 template <bool DEV, bool STRETCHED, bool INTERP>
@@ -64,16 +65,26 @@ struct LineState2 {
         }
     }
 
-    // Evaluate(x) -> b[3], J[9] (J[3 c + d] = d b_c / d x_d); O1 of DESIGN.md.
-    template <bool WITH_J>
-    __device__ __forceinline__ void evaluate(const TraceArgs &A, const double x[3], double b[3], double J[9])
+    // Makes the cached cell the one containing x (reading A8: index clamped, offsets not) and returns the offsets
+    // d = x - x_cell.  Called for the NEXT stage point as soon as its position is known, i.e. before the deviation
+    // products, the norm and the RK bookkeeping of the current stage, so that the table loads of a cell change are in
+    // flight while ~50 FP64 instructions that no longer need the old coefficients execute.
+    __device__ __forceinline__ void enter_cell(const TraceArgs &A, const double x[3], double d[3])
     {
-        double dx = x[0] - x0[0], dy = x[1] - x0[1], dz = x[2] - x0[2];
-        const double hx = STRETCHED ? hc[0] : A.fv.h[0], hy = STRETCHED ? hc[1] : A.fv.h[1], hz = STRETCHED ? hc[2] : A.fv.h[2];
-        if (!(in_range_bits(dx, hx) && in_range_bits(dy, hy) && in_range_bits(dz, hz))) {
+        d[0] = x[0] - x0[0]; d[1] = x[1] - x0[1]; d[2] = x[2] - x0[2];
+        const unsigned hx = STRETCHED ? (unsigned)__double2hiint(hc[0]) : A.h_hi[0], hy = STRETCHED ? (unsigned)__double2hiint(hc[1]) : A.h_hi[1],
+                       hz = STRETCHED ? (unsigned)__double2hiint(hc[2]) : A.h_hi[2];
+        if (!(in_range_hi(d[0], hx) && in_range_hi(d[1], hy) && in_range_hi(d[2], hz))) {
             relocate(A, x);
-            dx = x[0] - x0[0]; dy = x[1] - x0[1]; dz = x[2] - x0[2];
+            d[0] = x[0] - x0[0]; d[1] = x[1] - x0[1]; d[2] = x[2] - x0[2];
         }
+    }
+
+    // Evaluate -> b[3], J[9] (J[3 c + d] = d b_c / d x_d) at offsets d inside the cached cell; O1 of DESIGN.md.
+    template <bool WITH_J>
+    __device__ __forceinline__ void poly(const double d[3], double b[3], double J[9])
+    {
+        const double dx = d[0], dy = d[1], dz = d[2];
         double v[3], g[9];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -138,8 +149,9 @@ struct LineState2 {
         for (int c = 0; c < NV; ++c) y[c] = c < 3 ? x[c] : 0.0;
         if (!inside_box(A, x)) { finish(A, REC_SEED_OUTSIDE); return false; }
         x0[0] = x0[1] = x0[2] = __longlong_as_double(0x7ff8000000000000ll);    // no cell cached yet
-        double b[3], J[9];
-        evaluate<false>(A, x, b, J);
+        double b[3], J[9], d[3];
+        enter_cell(A, x, d);
+        poly<false>(d, b, J);
         const double nb = norm3(b);
         if (!(nb >= A.null_eps)) { finish(A, REC_NULL_AT_SEED); return false; }
         if (DEV) {
@@ -164,7 +176,7 @@ struct LineState2 {
 
     __device__ void finish(const TraceArgs &A, uint32_t flags)
     {
-        double out[REC_DOUBLES];
+        double out[REC_DOUBLES] = {};
 #pragma unroll
         for (int c = 0; c < 9; ++c) out[c] = c < NV ? y[c % NV] : 0.0;
         out[9] = L;
@@ -176,106 +188,178 @@ struct LineState2 {
         for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
     }
 
-    // One attempt: a trial step (phase 0), a landing iteration (1..3) or the final landing step (4).  True when the
-    // line has ended.  The sign of the direction is folded into the step (hs = sgn h), so the stage derivative is
-    // (b, J d1, J d2, |b|) without the three + six multiplications by sgn; the rounding is unchanged (sgn = +-1).
+    // Stage derivative k = (b, J d1, J d2) at the stage point ys, without the direction sign (it is folded into the
+    // step: the rounding is unchanged since sgn = +-1).  PAPER.md:79 (eq. 1), :119 (eq. 5).
+    __device__ __forceinline__ void derivative(const double b[3], const double J[9], const double ys[NV], double k[NV])
+    {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) k[c] = b[c];
+        if (DEV) {
+#pragma unroll
+            for (int v = 0; v < 2; ++v)
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    k[(3 + 3 * v + c) % NV] = fma(J[c * 3 + 2], ys[(3 + 3 * v + 2) % NV],
+                                                  fma(J[c * 3 + 1], ys[(3 + 3 * v + 1) % NV], J[c * 3] * ys[(3 + 3 * v) % NV]));
+        }
+    }
+
+    // One attempt = exactly four field evaluations for every lane, whatever its phase, so a warp never diverges on the
+    // integrator itself:
+    //   phase 0     trial RK4 step of size h from y; accepted if the trial end is inside the closed trace box, else the
+    //               chord fraction gives the first landing step size hp (reading A4) and the lane enters phase 1
+    //   phase 1     step of size hp from the same y (k1 is recomputed by the first evaluation and stashed in the lane's
+    //               record slot, which is not yet in use); the trial end xt is stashed too
+    //   phase 2..4  the first evaluation is spent at xt instead of y: one Newton update of hp from b(xt); k1 comes back
+    //               from the stash; step of size hp; phase 4 snaps the end onto the face and finishes the line
+    // i.e. hp0 -> step, Newton, step, Newton, step, Newton, final step: the three Newton updates of O4.
+    // Within a stage the order is: polynomial (b, J) -> position of the next stage point -> enter_cell for it (table
+    // loads in flight) -> deviation products, |b|, accumulators.
     __device__ bool advance(const TraceArgs &A)
     {
-        double acc[NV], accL = 0.0, ys[NV];
-        double hs = phase == 0 ? 0.0 : hp, h = 0.0;
-        const int last = A.method == QSL_EULER ? 0 : 3;
-#pragma unroll
-        for (int c = 0; c < NV; ++c) { acc[c] = 0.0; ys[c] = y[c]; }
-        double Ln = L;
-#pragma unroll 1
-        for (int st = 0;; ++st) {
-            double b[3], J[9];
-            evaluate<DEV>(A, ys, b, J);
-            const double bn = norm3(b);
-            if (st == 0 && phase == 0) {
+        double *stash = A.rec + (size_t)slot * REC_DOUBLES;
+        double b[3], J[9], k[NV], d[3], bn, hs, h = 0.0;
+        double acc[NV], accL, ys[NV];
+        {
+            double p0[3] = { y[0], y[1], y[2] };
+            if (phase >= 2) { p0[0] = stash[NV + 1]; p0[1] = stash[NV + 2]; p0[2] = stash[NV + 3]; }
+            enter_cell(A, p0, d);
+            poly<DEV>(d, b, J);
+            bn = norm3(b);
+            derivative(b, J, y, k);
+            if (phase == 0) {
                 // O4: stall / caps are tested on k1 before the step; h from the cell containing x
                 if (!(bn >= A.null_eps)) { finish(A, REC_STALL); return true; }
                 if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, REC_CAP); return true; }
                 h = STRETCHED ? A.step_frac * fmin(hc[0], fmin(hc[1], hc[2])) : A.h_uniform;
                 if (lam + h > A.max_length) h = A.max_length - lam;
                 hs = h;
-            }
-            if (st > last) {
-                // landing, "5th stage": b at the trial end -> one Newton update of hp (clamped to [0, h_full])
-                const double bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
-                const double xd = axis == 0 ? ys[0] : (axis == 1 ? ys[1] : ys[2]);
-                const double gg = sgn * bd, r = xd - bound;
-                if (gg != 0.0) {
-                    const double hn = hp - r / gg;
-                    if (hn == hn) hp = fmin(fmax(hn, 0.0), hfull);
+            } else {
+                if (phase == 1) {
+#pragma unroll
+                    for (int c = 0; c < NV; ++c) stash[c] = k[c];
+                    stash[NV] = bn;
+                } else {
+                    // Newton update of hp from the field at the previous trial end (clamped to [0, h_full])
+                    const double bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
+                    const double xd = axis == 0 ? p0[0] : (axis == 1 ? p0[1] : p0[2]);
+                    const double gg = sgn * bd, r = xd - bound;
+                    if (gg != 0.0) {
+                        const double hn = hp - r / gg;
+                        if (hn == hn) hp = fmin(fmax(hn, 0.0), hfull);
+                    }
+#pragma unroll
+                    for (int c = 0; c < NV; ++c) k[c] = stash[c];
+                    bn = stash[NV];
                 }
-                ++phase;
-                return false;
+                hs = hp;
             }
-            // stage derivative k = (b, J d1, J d2, |b|)  (PAPER.md:79 eq. 1, :119 eq. 5; reading A3 for L)
-            double k[NV];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) k[c] = b[c];
-            if (DEV) {
-#pragma unroll
-                for (int v = 0; v < 2; ++v)
-#pragma unroll
-                    for (int c = 0; c < 3; ++c)
-                        k[(3 + 3 * v + c) % NV] = fma(J[c * 3 + 2], ys[(3 + 3 * v + 2) % NV],
-                                                      fma(J[c * 3 + 1], ys[(3 + 3 * v + 1) % NV], J[c * 3] * ys[(3 + 3 * v) % NV]));
-            }
-            const double w = (st == 0 || st == last) ? 1.0 : 2.0;
-#pragma unroll
-            for (int c = 0; c < NV; ++c) acc[c] = fma(w, k[c], acc[c]);
-            accL = fma(w, bn, accL);
-            if (st == last) {
-                const double fL = A.method == QSL_EULER ? hs : hs * (1.0 / 6.0), f = sgn * fL;
-                // the trial end goes into ys (it is the "5th stage" point of the landing iterations)
-#pragma unroll
-                for (int c = 0; c < NV; ++c) ys[c] = fma(f, acc[c], y[c]);
-                Ln = fma(fL, accL, L);
-                if (phase >= 1 && phase <= 3) continue;
-                break;
-            }
-            const double ch = sgn * (st == 2 ? hs : 0.5 * hs);
-#pragma unroll
-            for (int c = 0; c < NV; ++c) ys[c] = fma(ch, k[c], y[c]);
         }
+        const double shs = sgn * hs;
+        if (A.method == QSL_EULER) {
+#pragma unroll
+            for (int c = 0; c < NV; ++c) ys[c] = fma(shs, k[c], y[c]);
+            accL = fma(hs, bn, L);
+        } else {
+            // RK4 (reading A5): k2 = f(y + h/2 k1), k3 = f(y + h/2 k2), k4 = f(y + h k3), y+ = y + h/6 (k1 + 2 k2 + 2 k3 + k4)
+            const double half = 0.5 * shs;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ys[c] = fma(half, k[c], y[c]);
+            enter_cell(A, ys, d);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) { acc[c] = k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
+            accL = bn;
+            // ---- stage 2
+            poly<DEV>(d, b, J);
+            {
+                double xn[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
+                enter_cell(A, xn, d);
+                bn = norm3(b);
+                derivative(b, J, ys, k);
+#pragma unroll
+                for (int c = 0; c < NV; ++c) { acc[c] = fma(2.0, k[c], acc[c]); ys[c] = c < 3 ? xn[c] : fma(half, k[c], y[c]); }
+                accL = fma(2.0, bn, accL);
+            }
+            // ---- stage 3
+            poly<DEV>(d, b, J);
+            {
+                double xn[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
+                enter_cell(A, xn, d);
+                bn = norm3(b);
+                derivative(b, J, ys, k);
+#pragma unroll
+                for (int c = 0; c < NV; ++c) { acc[c] = fma(2.0, k[c], acc[c]); ys[c] = c < 3 ? xn[c] : fma(shs, k[c], y[c]); }
+                accL = fma(2.0, bn, accL);
+            }
+            // ---- stage 4
+            poly<DEV>(d, b, J);
+            {
+                const double fL = hs * (1.0 / 6.0), f = sgn * fL;
+                double xn[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) xn[c] = fma(f, fma(1.0, b[c], acc[c]), y[c]);
+                // the trial end is where the next attempt starts if it is accepted: enter its cell now
+                enter_cell(A, xn, d);
+                bn = norm3(b);
+                derivative(b, J, ys, k);
+#pragma unroll
+                for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, fma(1.0, k[c], acc[c]), y[c]);
+                accL = fma(fL, fma(1.0, bn, accL), L);
+            }
+        }
+        // ys = trial end, accL = trial length
         if (phase == 0) {
             if (inside_box(A, ys)) {
 #pragma unroll
                 for (int c = 0; c < NV; ++c) y[c] = ys[c];
-                L = Ln; lam += h; ++nsteps;
+                L = accL; lam += h; ++nsteps;
                 return false;
             }
             // first face crossed by the chord: smallest fraction, tie -> lowest axis (reading A4)
             double phi = INFINITY; int ax = -1, fc = 255; double bd = 0.0;
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                if (ys[d] < A.box_lo[d]) {
-                    const double f = (A.box_lo[d] - y[d]) / (ys[d] - y[d]);
-                    if (f < phi) { phi = f; ax = d; fc = 2 * d; bd = A.box_lo[d]; }
-                } else if (ys[d] > A.box_hi[d]) {
-                    const double f = (A.box_hi[d] - y[d]) / (ys[d] - y[d]);
-                    if (f < phi) { phi = f; ax = d; fc = 2 * d + 1; bd = A.box_hi[d]; }
+            for (int dd = 0; dd < 3; ++dd) {
+                if (ys[dd] < A.box_lo[dd]) {
+                    const double f = (A.box_lo[dd] - y[dd]) / (ys[dd] - y[dd]);
+                    if (f < phi) { phi = f; ax = dd; fc = 2 * dd; bd = A.box_lo[dd]; }
+                } else if (ys[dd] > A.box_hi[dd]) {
+                    const double f = (A.box_hi[dd] - y[dd]) / (ys[dd] - y[dd]);
+                    if (f < phi) { phi = f; ax = dd; fc = 2 * dd + 1; bd = A.box_hi[dd]; }
                 }
             }
             if (ax < 0) { finish(A, REC_STALL); return true; }   // non-finite trial point
             axis = ax; face_pending = fc; bound = bd; hp = phi * h; hfull = h; phase = 1;
             return false;
         }
+        if (phase < 4) {
+            stash[NV + 1] = ys[0]; stash[NV + 2] = ys[1]; stash[NV + 3] = ys[2];
+            ++phase;
+            return false;
+        }
         // phase 4: final landing step
 #pragma unroll
         for (int c = 0; c < NV; ++c) y[c] = ys[c];
         if (axis == 0) y[0] = bound; else if (axis == 1) y[1] = bound; else y[2] = bound;
-        L = Ln; lam += hp; ++nsteps; face = face_pending;
+        L = accL; lam += hp; ++nsteps; face = face_pending;
         finish(A, 0);
         return true;
     }
 };
 
+// Resident CTAs per SM the register allocation is capped for: 3 x 128 threads (<= 168 registers) with the deviation
+// vectors, 4 x 128 (<= 128 registers) without; the FP64 dependency chains need the extra warps more than the registers.
+#ifndef QSL_T2_MIN_BLOCKS_LQ
+#define QSL_T2_MIN_BLOCKS_LQ 3
+#endif
+#ifndef QSL_T2_MIN_BLOCKS_L
+#define QSL_T2_MIN_BLOCKS_L 4
+#endif
 template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL>
-__global__ void __launch_bounds__(128) trace2_kernel(const TraceArgs A)
+__global__ void __launch_bounds__(128, DEV ? QSL_T2_MIN_BLOCKS_LQ : QSL_T2_MIN_BLOCKS_L) trace2_kernel(const TraceArgs A)
 {
     LineState2<DEV, STRETCHED, INTERP> ls;
     const long long n_items = 2 * A.n;

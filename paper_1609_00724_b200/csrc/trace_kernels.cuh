@@ -21,6 +21,7 @@ struct TraceArgs {
     double inv_h[3];             // 1 / uniform spacing
     double box_lo[3], box_hi[3];
     double h_uniform;            // step_frac * min_d h_d on a uniform grid
+    unsigned h_hi[3];            // high words of the uniform spacings (in-cell test of the V2 kernel)
     double step_frac, max_length, null_eps;
     long long max_steps;
     int method;
@@ -33,8 +34,8 @@ struct TraceArgs {
     unsigned long long *queue;   // work counter of the persistent kernel
 };
 
-// Per-direction record written once when a line ends: x[3], d1[3], d2[3], L, then (nsteps, face|flags) as two uint32.
-constexpr int REC_DOUBLES = 12;
+// Per-direction record written once when a line ends: x[3], d1[3], d2[3], L, (nsteps, face|flags) as two uint32, lambda.
+constexpr int REC_DOUBLES = 14;    // [12], [13] are only used as the landing stash of the V2 kernel
 constexpr uint32_t REC_STALL = 1u << 8, REC_CAP = 1u << 9, REC_SEED_OUTSIDE = 1u << 10, REC_NULL_AT_SEED = 1u << 11;
 
 template <typename S> struct Sample4;
@@ -233,7 +234,7 @@ struct LineState {
     __device__ void finish(const TraceArgs &A, uint32_t flags)
     {
         double *r = A.rec + (size_t)slot * REC_DOUBLES;
-        double out[REC_DOUBLES];
+        double out[REC_DOUBLES] = {};
 #pragma unroll
         for (int c = 0; c < 9; ++c) out[c] = c < NV ? y[c % NV] : 0.0;
         out[9] = L;
