@@ -8,7 +8,7 @@
 namespace qsl {
 cudaError_t launch_trace_f32(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 cudaError_t launch_trace_f64(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
-cudaError_t launch_trace2(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
+int launch_trace2(TraceArgs &A, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 cudaError_t launch_epilogue_f32(const EpilogueArgs &E, cudaStream_t s);
 cudaError_t launch_epilogue_f64(const EpilogueArgs &E, cudaStream_t s);
 }  // namespace qsl
@@ -70,6 +70,7 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
     const bool refill = !(p->flags & QSL_FLAG_NO_REFILL);
     A.interleave = refill ? 1 : 0;
     A.n = n; A.seeds = seeds; A.total_steps = total_steps;
+    A.basis = nullptr; A.stash = nullptr;
 
     void *perm = nullptr, *rec = nullptr, *queue = nullptr;
     int rc = scratch_alloc(&perm, sizeof(uint32_t) * (size_t)n, s);
@@ -81,18 +82,24 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         A.perm = (const uint32_t *)perm; A.rec = (double *)rec; A.queue = (unsigned long long *)queue;
         e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
         const bool dev = p->mode == QSL_TRACE_LQ;
-        if (e == cudaSuccess && g_profile) e = cudaEventRecord(g_ev0, s);
         const bool v2 = f->view.cells != nullptr && !(p->flags & QSL_FLAG_KERNEL_V1);
-        if (e == cudaSuccess)
-            e = v2 ? launch_trace2(A, dev, refill, s)
-                   : (f->sample_type == QSL_F32 ? launch_trace_f32(A, dev, refill, s) : launch_trace_f64(A, dev, refill, s));
-        if (e == cudaSuccess && g_profile) { e = cudaEventRecord(g_ev1, s); g_profile_valid = 1; }
+        if (e == cudaSuccess && v2) {
+            // the cell-table kernel allocates its own scratch and brackets its launch with the profiling events
+            rc = launch_trace2(A, dev, refill, g_profile ? g_ev0 : nullptr, g_profile ? g_ev1 : nullptr, s);
+            if (rc == QSL_OK && g_profile) g_profile_valid = 1;
+        } else if (e == cudaSuccess) {
+            if (g_profile) e = cudaEventRecord(g_ev0, s);
+            if (e == cudaSuccess)
+                e = f->sample_type == QSL_F32 ? launch_trace_f32(A, dev, refill, s) : launch_trace_f64(A, dev, refill, s);
+            if (e == cudaSuccess && g_profile) { e = cudaEventRecord(g_ev1, s); g_profile_valid = 1; }
+        }
+        if (rc != QSL_OK) e = cudaErrorUnknown;
         if (e == cudaSuccess) {
             EpilogueArgs E;
             E.T = A; E.with_dev = dev ? 1 : 0; E.out = *out;
             e = f->sample_type == QSL_F32 ? launch_epilogue_f32(E, s) : launch_epilogue_f64(E, s);
         }
-        if (e != cudaSuccess) rc = record_cuda(e);
+        if (e != cudaSuccess && rc == QSL_OK) rc = record_cuda(e);
     }
     scratch_free(perm, s); scratch_free(rec, s); scratch_free(queue, s);
     return rc;

@@ -4,37 +4,53 @@
 namespace qsl {
 
 template <bool DEV, bool STRETCHED, bool INTERP>
-static cudaError_t launch_trace2_variant(const TraceArgs &A, bool refill, cudaStream_t s)
+static int launch_trace2_variant(TraceArgs &A, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s)
 {
     const long long n_items = 2 * A.n;
-    const int threads = 128;
-    if (!refill) {
-        const long long blocks = (n_items + threads - 1) / threads;
-        count_launch();
-        trace2_kernel<DEV, STRETCHED, INTERP, false><<<(unsigned)blocks, threads, 0, s>>>(A);
-    } else {
+    const int threads = QSL_T2_THREADS;
+    long long blocks = (n_items + threads - 1) / threads;
+    if (refill) {
         int per_sm = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace2_kernel<DEV, STRETCHED, INTERP, true>, threads, 0);
-        if (e != cudaSuccess) return e;
+        QSL_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace2_kernel<DEV, STRETCHED, INTERP, true>, threads, 0));
         if (per_sm < 1) per_sm = 1;
-        long long blocks = (long long)sm_count() * per_sm;          // persistent: every CTA resident, grid = SMs x occupancy
-        const long long need = (n_items + threads - 1) / threads;
-        if (blocks > need) blocks = need;
-        count_launch();
-        trace2_kernel<DEV, STRETCHED, INTERP, true><<<(unsigned)blocks, threads, 0, s>>>(A);
+        const long long resident = (long long)sm_count() * per_sm;   // persistent: every CTA resident, grid = SMs x occupancy
+        if (blocks > resident) blocks = resident;
     }
-    return cudaGetLastError();
+    void *basis = nullptr, *stash = nullptr;
+    int rc = scratch_alloc(&stash, sizeof(double) * STASH_DOUBLES * (size_t)blocks * threads, s);
+    if (rc == QSL_OK && DEV) rc = scratch_alloc(&basis, sizeof(double) * 6 * (size_t)A.n, s);
+    cudaError_t e = cudaSuccess;
+    if (rc == QSL_OK) {
+        A.stash = (double *)stash;
+        if (DEV) {
+            count_launch();
+            seed_basis_kernel<STRETCHED, INTERP><<<(unsigned)((A.n + 127) / 128), 128, 0, s>>>(A, (double *)basis);
+            A.basis = (const double *)basis;
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess && ev0) e = cudaEventRecord(ev0, s);
+        if (e == cudaSuccess) {
+            count_launch();
+            if (refill) trace2_kernel<DEV, STRETCHED, INTERP, true><<<(unsigned)blocks, threads, 0, s>>>(A);
+            else trace2_kernel<DEV, STRETCHED, INTERP, false><<<(unsigned)blocks, threads, 0, s>>>(A);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, s);
+        if (e != cudaSuccess) rc = record_cuda(e);
+    }
+    scratch_free(basis, s); scratch_free(stash, s);
+    return rc;
 }
 
-cudaError_t launch_trace2(const TraceArgs &A, bool dev, bool refill, cudaStream_t s)
+int launch_trace2(TraceArgs &A, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s)
 {
     const bool st = A.fv.stretched != 0, in = A.fv.interp_mode == QSL_INTERP_FIRST;
 #define QSL_DISPATCH(D, ST, IN) \
-    if (dev == D && st == ST && in == IN) return launch_trace2_variant<D, ST, IN>(A, refill, s);
+    if (dev == D && st == ST && in == IN) return launch_trace2_variant<D, ST, IN>(A, refill, ev0, ev1, s);
     QSL_DISPATCH(false, false, false) QSL_DISPATCH(false, false, true) QSL_DISPATCH(false, true, false) QSL_DISPATCH(false, true, true)
     QSL_DISPATCH(true, false, false) QSL_DISPATCH(true, false, true) QSL_DISPATCH(true, true, false) QSL_DISPATCH(true, true, true)
 #undef QSL_DISPATCH
-    return cudaErrorInvalidValue;
+    return QSL_EINVAL;
 }
 
 }  // namespace qsl

@@ -21,29 +21,40 @@ __device__ __forceinline__ double4 load_cell4(const double4 *p)
     return r;
 }
 
-// Sufficient test for 0 <= a < b (b > 0) on the high 32 bits of the bit patterns: one unsigned integer compare on
-// the integer pipe instead of two DSETP on the FP64 pipe.  False for negative a (sign bit set), -0.0, NaN, and for a
-// within 2^-20 (relative) below b: a false negative only costs a redundant relocate, which finds the right cell.
-__device__ __forceinline__ bool in_range_hi(double a, unsigned b_hi)
+// |v| for the length integrand (reading A3) and the stall test: hardware reciprocal-square-root seed and one coupled
+// Newton step (relative error ~1e-13, five orders below the parity gate on L) instead of the IEEE sqrt sequence with its
+// fix-up branch; arguments outside [2^-767, 2^769) (zero, subnormal, huge, NaN) take the exact path.
+__device__ __forceinline__ double norm3_fast(const double v[3])
 {
-    return (unsigned)__double2hiint(a) < b_hi;
+    const double n2 = fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0]));
+    if ((unsigned)(__double2hiint(n2) - 0x10000000) >= 0x60000000u) return sqrt(n2);
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(n2));
+    const double s = n2 * r, hr = 0.5 * r;
+    const double e = fma(-s, hr, 0.5);                 // 0.5 (1 - n2 r^2)
+    const double s1 = fma(s, e, s), h1 = fma(hr, e, hr);
+    return fma(fma(-s1, s1, n2), h1, s1);
 }
+
+// Per-thread scratch of the landing (reading A4), in global memory: used only by the last five attempts of a line, so
+// it must not occupy registers during the thousands of plain steps.  Layout [slot * n_threads + thread].
+enum { ST_K1 = 0, ST_BN = 9, ST_XT = 10, ST_HP = 13, ST_BOUND = 14, ST_HFULL = 15, ST_AXIS_FACE = 16, STASH_DOUBLES = 17 };
 
 template <bool DEV, bool STRETCHED, bool INTERP>
 struct LineState2 {
     static constexpr int NV = DEV ? 9 : 3;
-    // cached cell: monomial coefficients a[8 c + m], origin, edges (edges only needed on stretched grids)
+    // cached cell: monomial coefficients a[8 c + m], origin (edges only on stretched grids)
     double a[24];
     double x0[3];
     double hc[3];
-    // line state (as LineState)
+    // line state
     double y[NV];
-    double L, lam, hp, bound, hfull;
-    uint32_t nsteps;
-    int phase, axis, face, face_pending;
-    double sgn;
-    long long slot;
+    double L, lam;
+    uint32_t nsteps, slot;
+    int phase;
+    bool back;
 
+    // Cell search (reading A8: index clamped, offsets not) and load of the cell's 24 coefficients (six 256-bit loads).
     __device__ __forceinline__ void relocate(const TraceArgs &A, const double x[3])
     {
         int i, j, k; double t, ih;
@@ -65,118 +76,118 @@ struct LineState2 {
         }
     }
 
-    // Makes the cached cell the one containing x (reading A8: index clamped, offsets not) and returns the offsets
-    // d = x - x_cell.  Called for the NEXT stage point as soon as its position is known, i.e. before the deviation
-    // products, the norm and the RK bookkeeping of the current stage, so that the table loads of a cell change are in
-    // flight while ~50 FP64 instructions that no longer need the old coefficients execute.
+    // Makes the cached cell the one containing x and returns the offsets d = x - x_cell.  Called for the NEXT stage
+    // point as soon as its position is known, so the table loads of a cell change are in flight while the ~50 FP64
+    // instructions of the current stage that no longer need the old coefficients execute.  The "still inside" test is a
+    // sufficient one on the high words of the bit patterns, 0 <= d < h: one unsigned integer compare per axis on the
+    // integer pipe instead of two DSETP on the FP64 pipe.  It is false for negative d (sign bit), -0.0, NaN and for d
+    // within 2^-20 (relative) below h: a false negative only costs a redundant search, which finds the right cell.
+    // (A branch-free variant with predicated neighbour loads was measured and dropped: profiles/r1c.)
     __device__ __forceinline__ void enter_cell(const TraceArgs &A, const double x[3], double d[3])
     {
         d[0] = x[0] - x0[0]; d[1] = x[1] - x0[1]; d[2] = x[2] - x0[2];
         const unsigned hx = STRETCHED ? (unsigned)__double2hiint(hc[0]) : A.h_hi[0], hy = STRETCHED ? (unsigned)__double2hiint(hc[1]) : A.h_hi[1],
                        hz = STRETCHED ? (unsigned)__double2hiint(hc[2]) : A.h_hi[2];
-        if (!(in_range_hi(d[0], hx) && in_range_hi(d[1], hy) && in_range_hi(d[2], hz))) {
+        if (!((unsigned)__double2hiint(d[0]) < hx && (unsigned)__double2hiint(d[1]) < hy && (unsigned)__double2hiint(d[2]) < hz)) {
             relocate(A, x);
             d[0] = x[0] - x0[0]; d[1] = x[1] - x0[1]; d[2] = x[2] - x0[2];
         }
     }
 
-    // Evaluate -> b[3], J[9] (J[3 c + d] = d b_c / d x_d) at offsets d inside the cached cell; O1 of DESIGN.md.
-    template <bool WITH_J>
-    __device__ __forceinline__ void poly(const double d[3], double b[3], double J[9])
+    // Field evaluation at offsets d inside the cached cell (O1 of DESIGN.md) fused with the deviation products:
+    // b[3] and, with DEV, k[3 + 3 v + c] = sum_e J[c][e] dl_v[e] for the two deviation vectors dl = ys[3..8]
+    // (eq. 5), component by component so that only one row of J is live at a time.
+    __device__ __forceinline__ void stage(const double d[3], const double *ys, double b[3], double *k)
     {
         const double dx = d[0], dy = d[1], dz = d[2];
-        double v[3], g[9];
+        if (!INTERP) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const double *q = a + 8 * c;
-            const double P = fma(q[7], dz, q[3]);      // coefficient of dx dy
-            const double Q = fma(q[5], dz, q[1]);      // coefficient of dx
-            const double R = fma(q[6], dz, q[2]);      // coefficient of dy
-            const double S = fma(q[4], dz, q[0]);
-            const double E = fma(P, dy, Q);            // d/dx
-            const double F = fma(R, dy, S);
-            v[c] = fma(E, dx, F);
-            if (WITH_J) {
+            for (int c = 0; c < 3; ++c) {
+                const double *q = a + 8 * c;
+                const double P = fma(q[7], dz, q[3]);      // coefficient of dx dy
+                const double Q = fma(q[5], dz, q[1]);      // coefficient of dx
+                const double R = fma(q[6], dz, q[2]);      // coefficient of dy
+                const double S = fma(q[4], dz, q[0]);
+                const double E = fma(P, dy, Q);            // d/dx
+                const double F = fma(R, dy, S);
+                b[c] = fma(E, dx, F);
+                if (DEV) {
+                    const double gy = fma(P, dx, R);
+                    const double gz = fma(fma(q[7], dy, q[5]), dx, fma(q[6], dy, q[4]));
+                    k[(3 + c) % NV] = fma(gz, ys[5 % NV], fma(gy, ys[4 % NV], E * ys[3 % NV]));
+                    k[(6 + c) % NV] = fma(gz, ys[8 % NV], fma(gy, ys[7 % NV], E * ys[6 % NV]));
+                }
+            }
+        } else {
+            // reading A2: interpolate B, then normalise: b = B/|B|, J = (G - u (u^T G))/|B|
+            double v[3], g[9], J[9];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double *q = a + 8 * c;
+                const double P = fma(q[7], dz, q[3]), Q = fma(q[5], dz, q[1]), R = fma(q[6], dz, q[2]), S = fma(q[4], dz, q[0]);
+                const double E = fma(P, dy, Q), F = fma(R, dy, S);
+                v[c] = fma(E, dx, F);
                 g[3 * c] = E;
                 g[3 * c + 1] = fma(P, dx, R);
                 g[3 * c + 2] = fma(fma(q[7], dy, q[5]), dx, fma(q[6], dy, q[4]));
             }
-        }
-        if (!INTERP) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) b[c] = v[c];
-            if (WITH_J) {
-#pragma unroll
-                for (int q = 0; q < 9; ++q) J[q] = g[q];
-            }
-        } else {
-            // reading A2: interpolate B, then normalise: b = B/|B|, J = (G - u (u^T G))/|B|
             const double nn = sqrt(fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0])));
             if (nn < 1e-300) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) b[c] = 0.0;
-                if (WITH_J) {
 #pragma unroll
-                    for (int q = 0; q < 9; ++q) J[q] = 0.0;
-                }
+                for (int q = 0; q < 9; ++q) J[q] = 0.0;
             } else {
                 const double inv = 1.0 / nn;
                 const double u0 = v[0] * inv, u1 = v[1] * inv, u2 = v[2] * inv;
                 b[0] = u0; b[1] = u1; b[2] = u2;
-                if (WITH_J) {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) {
-                        const double uG = fma(u2, g[6 + d], fma(u1, g[3 + d], u0 * g[d]));
-                        J[d] = (g[d] - u0 * uG) * inv;
-                        J[3 + d] = (g[3 + d] - u1 * uG) * inv;
-                        J[6 + d] = (g[6 + d] - u2 * uG) * inv;
-                    }
+                for (int e = 0; e < 3; ++e) {
+                    const double uG = fma(u2, g[6 + e], fma(u1, g[3 + e], u0 * g[e]));
+                    J[e] = (g[e] - u0 * uG) * inv;
+                    J[3 + e] = (g[3 + e] - u1 * uG) * inv;
+                    J[6 + e] = (g[6 + e] - u2 * uG) * inv;
                 }
+            }
+            if (DEV) {
+#pragma unroll
+                for (int w = 0; w < 2; ++w)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c)
+                        k[(3 + 3 * w + c) % NV] = fma(J[c * 3 + 2], ys[(3 + 3 * w + 2) % NV],
+                                                      fma(J[c * 3 + 1], ys[(3 + 3 * w + 1) % NV], J[c * 3] * ys[(3 + 3 * w) % NV]));
             }
         }
     }
 
+    // Starts work item q.  Returns false if the item ended at once (seed outside the trace box).  The orthonormal pair
+    // a^, b^ of O2 comes from seed_basis_kernel (one thread per seed, all lanes busy) instead of being built here by
+    // the one or two lanes of a warp that happen to be refilling; a null at the seed is caught by the first attempt.
     __device__ bool init(const TraceArgs &A, long long q)
     {
         long long pos; int dir;
         if (A.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= A.n ? 1 : 0; pos = q - (long long)dir * A.n; }
-        slot = (long long)dir * A.n + pos;
-        sgn = dir ? -1.0 : 1.0;
+        slot = (uint32_t)((long long)dir * A.n + pos);
+        back = dir != 0;
         const uint32_t si = A.perm[pos];
-        double x[3] = { A.seeds[3 * (size_t)si], A.seeds[3 * (size_t)si + 1], A.seeds[3 * (size_t)si + 2] };
-        L = 0.0; lam = 0.0; nsteps = 0; phase = 0; axis = 0; face = 255; face_pending = 255; hp = 0.0; bound = 0.0; hfull = 0.0;
+        const double x[3] = { A.seeds[3 * (size_t)si], A.seeds[3 * (size_t)si + 1], A.seeds[3 * (size_t)si + 2] };
+        L = 0.0; lam = 0.0; nsteps = 0; phase = 0;
 #pragma unroll
         for (int c = 0; c < NV; ++c) y[c] = c < 3 ? x[c] : 0.0;
-        if (!inside_box(A, x)) { finish(A, REC_SEED_OUTSIDE); return false; }
+        if (!inside_box(A, x)) { finish(A, 255, REC_SEED_OUTSIDE); return false; }
         x0[0] = x0[1] = x0[2] = __longlong_as_double(0x7ff8000000000000ll);    // no cell cached yet
-        double b[3], J[9], d[3];
-        enter_cell(A, x, d);
-        poly<false>(d, b, J);
-        const double nb = norm3(b);
-        if (!(nb >= A.null_eps)) { finish(A, REC_NULL_AT_SEED); return false; }
+        hc[0] = hc[1] = hc[2] = 0.0;
         if (DEV) {
-            // O2 (PAPER.md:160 eq. 9, :163): a^, b^ orthonormal with B^(x0); reading A7: e = axis of smallest |u_d|
-            const double inv = 1.0 / nb;
-            const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
-            int e = 0;
-            if (fabs(u[1]) < fabs(u[e])) e = 1;
-            if (fabs(u[2]) < fabs(u[e == 1 ? 1 : 0])) e = 2;
-            const double ue = e == 0 ? u[0] : (e == 1 ? u[1] : u[2]);
-            double av[3] = { -u[0] * ue, -u[1] * ue, -u[2] * ue };
-            if (e == 0) av[0] += 1.0; else if (e == 1) av[1] += 1.0; else av[2] += 1.0;
-            const double ia = 1.0 / norm3(av);
-            av[0] *= ia; av[1] *= ia; av[2] *= ia;
-            y[3 % NV] = av[0]; y[4 % NV] = av[1]; y[5 % NV] = av[2];
-            y[6 % NV] = u[1] * av[2] - u[2] * av[1];
-            y[7 % NV] = u[2] * av[0] - u[0] * av[2];
-            y[8 % NV] = u[0] * av[1] - u[1] * av[0];
+            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(A.basis + 6 * (size_t)pos);
+            const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
+            y[3 % NV] = b0.x; y[4 % NV] = b0.y; y[5 % NV] = b1.x; y[6 % NV] = b1.y; y[7 % NV] = b2.x; y[8 % NV] = b2.y;
         }
         return true;
     }
 
-    __device__ void finish(const TraceArgs &A, uint32_t flags)
+    __device__ void finish(const TraceArgs &A, int face, uint32_t flags)
     {
-        double out[REC_DOUBLES] = {};
+        double out[REC_DOUBLES];
 #pragma unroll
         for (int c = 0; c < 9; ++c) out[c] = c < NV ? y[c % NV] : 0.0;
         out[9] = L;
@@ -188,124 +199,120 @@ struct LineState2 {
         for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
     }
 
-    // Stage derivative k = (b, J d1, J d2) at the stage point ys, without the direction sign (it is folded into the
-    // step: the rounding is unchanged since sgn = +-1).  PAPER.md:79 (eq. 1), :119 (eq. 5).
-    __device__ __forceinline__ void derivative(const double b[3], const double J[9], const double ys[NV], double k[NV])
-    {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) k[c] = b[c];
-        if (DEV) {
-#pragma unroll
-            for (int v = 0; v < 2; ++v)
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-                    k[(3 + 3 * v + c) % NV] = fma(J[c * 3 + 2], ys[(3 + 3 * v + 2) % NV],
-                                                  fma(J[c * 3 + 1], ys[(3 + 3 * v + 1) % NV], J[c * 3] * ys[(3 + 3 * v) % NV]));
-        }
-    }
-
     // One attempt = exactly four field evaluations for every lane, whatever its phase, so a warp never diverges on the
     // integrator itself:
     //   phase 0     trial RK4 step of size h from y; accepted if the trial end is inside the closed trace box, else the
     //               chord fraction gives the first landing step size hp (reading A4) and the lane enters phase 1
-    //   phase 1     step of size hp from the same y (k1 is recomputed by the first evaluation and stashed in the lane's
-    //               record slot, which is not yet in use); the trial end xt is stashed too
+    //   phase 1     step of size hp from the same y (k1 is recomputed by the first evaluation and stashed); the trial end
+    //               xt is stashed too
     //   phase 2..4  the first evaluation is spent at xt instead of y: one Newton update of hp from b(xt); k1 comes back
     //               from the stash; step of size hp; phase 4 snaps the end onto the face and finishes the line
     // i.e. hp0 -> step, Newton, step, Newton, step, Newton, final step: the three Newton updates of O4.
-    // Within a stage the order is: polynomial (b, J) -> position of the next stage point -> enter_cell for it (table
-    // loads in flight) -> deviation products, |b|, accumulators.
+    // Within a stage the order is: polynomial + deviation products -> position of the next stage point -> enter_cell
+    // for it (table loads in flight) -> |b|, accumulators.  The direction sign is folded into the step size.
     __device__ bool advance(const TraceArgs &A)
     {
-        double *stash = A.rec + (size_t)slot * REC_DOUBLES;
-        double b[3], J[9], k[NV], d[3], bn, hs, h = 0.0;
+        // this thread's landing scratch and its stride: recomputed where needed (rare) rather than held in registers
+#define st (A.stash + ((size_t)blockIdx.x * blockDim.x + threadIdx.x))
+#define T ((size_t)gridDim.x * blockDim.x)
+        double b[3], k[NV], d[3], bn, hs, h = 0.0;
         double acc[NV], accL, ys[NV];
         {
             double p0[3] = { y[0], y[1], y[2] };
-            if (phase >= 2) { p0[0] = stash[NV + 1]; p0[1] = stash[NV + 2]; p0[2] = stash[NV + 3]; }
+            if (phase >= 2) { p0[0] = st[(ST_XT + 0) * T]; p0[1] = st[(ST_XT + 1) * T]; p0[2] = st[(ST_XT + 2) * T]; }
             enter_cell(A, p0, d);
-            poly<DEV>(d, b, J);
-            bn = norm3(b);
-            derivative(b, J, y, k);
+            stage(d, y, b, k);
+            bn = norm3_fast(b);
             if (phase == 0) {
                 // O4: stall / caps are tested on k1 before the step; h from the cell containing x
-                if (!(bn >= A.null_eps)) { finish(A, REC_STALL); return true; }
-                if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, REC_CAP); return true; }
+                if (!(bn >= A.null_eps)) { finish(A, 255, nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL); return true; }
+                if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, 255, REC_CAP); return true; }
                 h = STRETCHED ? A.step_frac * fmin(hc[0], fmin(hc[1], hc[2])) : A.h_uniform;
                 if (lam + h > A.max_length) h = A.max_length - lam;
                 hs = h;
             } else {
+                double hp = st[ST_HP * T];
                 if (phase == 1) {
 #pragma unroll
-                    for (int c = 0; c < NV; ++c) stash[c] = k[c];
-                    stash[NV] = bn;
+                    for (int c = 0; c < 3; ++c) st[(ST_K1 + c) * T] = b[c];
+#pragma unroll
+                    for (int c = 3; c < NV; ++c) st[(ST_K1 + c) * T] = k[c];
+                    st[ST_BN * T] = bn;
                 } else {
                     // Newton update of hp from the field at the previous trial end (clamped to [0, h_full])
+                    const int axis = __double2hiint(st[ST_AXIS_FACE * T]);
+                    const double bound = st[ST_BOUND * T], hfull = st[ST_HFULL * T];
                     const double bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
                     const double xd = axis == 0 ? p0[0] : (axis == 1 ? p0[1] : p0[2]);
-                    const double gg = sgn * bd, r = xd - bound;
+                    const double gg = back ? -bd : bd, r = xd - bound;
                     if (gg != 0.0) {
                         const double hn = hp - r / gg;
                         if (hn == hn) hp = fmin(fmax(hn, 0.0), hfull);
                     }
+                    st[ST_HP * T] = hp;
 #pragma unroll
-                    for (int c = 0; c < NV; ++c) k[c] = stash[c];
-                    bn = stash[NV];
+                    for (int c = 0; c < 3; ++c) b[c] = st[(ST_K1 + c) * T];
+#pragma unroll
+                    for (int c = 3; c < NV; ++c) k[c] = st[(ST_K1 + c) * T];
+                    bn = st[ST_BN * T];
                 }
                 hs = hp;
             }
         }
-        const double shs = sgn * hs;
+        const double shs = back ? -hs : hs;
         if (A.method == QSL_EULER) {
 #pragma unroll
-            for (int c = 0; c < NV; ++c) ys[c] = fma(shs, k[c], y[c]);
+            for (int c = 0; c < NV; ++c) ys[c] = fma(shs, c < 3 ? b[c] : k[c], y[c]);
             accL = fma(hs, bn, L);
         } else {
             // RK4 (reading A5): k2 = f(y + h/2 k1), k3 = f(y + h/2 k2), k4 = f(y + h k3), y+ = y + h/6 (k1 + 2 k2 + 2 k3 + k4)
             const double half = 0.5 * shs;
 #pragma unroll
-            for (int c = 0; c < 3; ++c) ys[c] = fma(half, k[c], y[c]);
+            for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
             enter_cell(A, ys, d);
 #pragma unroll
-            for (int c = 0; c < NV; ++c) { acc[c] = k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
+            for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
             accL = bn;
             // ---- stage 2
-            poly<DEV>(d, b, J);
+            stage(d, ys, b, k);
             {
                 double xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
                 enter_cell(A, xn, d);
-                bn = norm3(b);
-                derivative(b, J, ys, k);
+                bn = norm3_fast(b);
 #pragma unroll
-                for (int c = 0; c < NV; ++c) { acc[c] = fma(2.0, k[c], acc[c]); ys[c] = c < 3 ? xn[c] : fma(half, k[c], y[c]); }
+                for (int c = 0; c < NV; ++c) {
+                    const double kc = c < 3 ? b[c] : k[c];
+                    acc[c] = fma(2.0, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(half, kc, y[c]);
+                }
                 accL = fma(2.0, bn, accL);
             }
             // ---- stage 3
-            poly<DEV>(d, b, J);
+            stage(d, ys, b, k);
             {
                 double xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
                 enter_cell(A, xn, d);
-                bn = norm3(b);
-                derivative(b, J, ys, k);
+                bn = norm3_fast(b);
 #pragma unroll
-                for (int c = 0; c < NV; ++c) { acc[c] = fma(2.0, k[c], acc[c]); ys[c] = c < 3 ? xn[c] : fma(shs, k[c], y[c]); }
+                for (int c = 0; c < NV; ++c) {
+                    const double kc = c < 3 ? b[c] : k[c];
+                    acc[c] = fma(2.0, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(shs, kc, y[c]);
+                }
                 accL = fma(2.0, bn, accL);
             }
             // ---- stage 4
-            poly<DEV>(d, b, J);
+            stage(d, ys, b, k);
             {
-                const double fL = hs * (1.0 / 6.0), f = sgn * fL;
+                const double fL = hs * (1.0 / 6.0), f = back ? -fL : fL;
                 double xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(f, fma(1.0, b[c], acc[c]), y[c]);
                 // the trial end is where the next attempt starts if it is accepted: enter its cell now
                 enter_cell(A, xn, d);
-                bn = norm3(b);
-                derivative(b, J, ys, k);
+                bn = norm3_fast(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, fma(1.0, k[c], acc[c]), y[c]);
                 accL = fma(fL, fma(1.0, bn, accL), L);
@@ -331,27 +338,81 @@ struct LineState2 {
                     if (f < phi) { phi = f; ax = dd; fc = 2 * dd + 1; bd = A.box_hi[dd]; }
                 }
             }
-            if (ax < 0) { finish(A, REC_STALL); return true; }   // non-finite trial point
-            axis = ax; face_pending = fc; bound = bd; hp = phi * h; hfull = h; phase = 1;
+            if (ax < 0) { finish(A, 255, REC_STALL); return true; }   // non-finite trial point
+            const double yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
+            if (yd == bd) {
+                // the line starts on the face it leaves through (photospheric seeds): hp = 0, every Newton residual is
+                // exactly 0, so the landing of O4 ends where it started: one zero-length step
+                ++nsteps;
+                finish(A, fc, 0);
+                return true;
+            }
+            st[ST_HP * T] = phi * h; st[ST_BOUND * T] = bd; st[ST_HFULL * T] = h;
+            st[ST_AXIS_FACE * T] = __hiloint2double(ax, fc);
+            phase = 1;
             return false;
         }
         if (phase < 4) {
-            stash[NV + 1] = ys[0]; stash[NV + 2] = ys[1]; stash[NV + 3] = ys[2];
+            st[(ST_XT + 0) * T] = ys[0]; st[(ST_XT + 1) * T] = ys[1]; st[(ST_XT + 2) * T] = ys[2];
             ++phase;
             return false;
         }
         // phase 4: final landing step
+        const double af = st[ST_AXIS_FACE * T];
+        const int axis = __double2hiint(af), fc = __double2loint(af);
+        const double bound = st[ST_BOUND * T];
 #pragma unroll
         for (int c = 0; c < NV; ++c) y[c] = ys[c];
         if (axis == 0) y[0] = bound; else if (axis == 1) y[1] = bound; else y[2] = bound;
-        L = accL; lam += hp; ++nsteps; face = face_pending;
-        finish(A, 0);
+        L = accL; lam += st[ST_HP * T]; ++nsteps;
+        finish(A, fc, 0);
         return true;
+#undef st
+#undef T
     }
 };
 
+// O2 (PAPER.md:160 eq. 9, :163): a^, b^ orthonormal with B^(x0); reading A7: e = axis of the smallest |u_d|.  One thread
+// per seed in sorted order; writes (a^, b^) = 6 doubles per seed for the init of the trace kernel.
+template <bool STRETCHED, bool INTERP>
+__global__ void __launch_bounds__(128) seed_basis_kernel(const TraceArgs A, double *__restrict__ basis)
+{
+    const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= A.n) return;
+    const uint32_t si = A.perm[pos];
+    const double x[3] = { A.seeds[3 * (size_t)si], A.seeds[3 * (size_t)si + 1], A.seeds[3 * (size_t)si + 2] };
+    double o[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
+    if (inside_box(A, x)) {
+        LineState2<false, STRETCHED, INTERP> ls;
+        ls.relocate(A, x);
+        const double d[3] = { x[0] - ls.x0[0], x[1] - ls.x0[1], x[2] - ls.x0[2] };
+        double b[3];
+        ls.stage(d, nullptr, b, nullptr);
+        const double nb = norm3(b);
+        const double inv = 1.0 / nb;
+        const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
+        int e = 0;
+        if (fabs(u[1]) < fabs(u[e])) e = 1;
+        if (fabs(u[2]) < fabs(u[e == 1 ? 1 : 0])) e = 2;
+        const double ue = e == 0 ? u[0] : (e == 1 ? u[1] : u[2]);
+        double av[3] = { -u[0] * ue, -u[1] * ue, -u[2] * ue };
+        if (e == 0) av[0] += 1.0; else if (e == 1) av[1] += 1.0; else av[2] += 1.0;
+        const double ia = 1.0 / norm3(av);
+        av[0] *= ia; av[1] *= ia; av[2] *= ia;
+        o[0] = av[0]; o[1] = av[1]; o[2] = av[2];
+        o[3] = u[1] * av[2] - u[2] * av[1];
+        o[4] = u[2] * av[0] - u[0] * av[2];
+        o[5] = u[0] * av[1] - u[1] * av[0];
+    }
+    double2 *w = reinterpret_cast<double2 *>(basis + 6 * (size_t)pos);
+    w[0] = make_double2(o[0], o[1]); w[1] = make_double2(o[2], o[3]); w[2] = make_double2(o[4], o[5]);
+}
+
 // Resident CTAs per SM the register allocation is capped for: 3 x 128 threads (<= 168 registers) with the deviation
 // vectors, 4 x 128 (<= 128 registers) without; the FP64 dependency chains need the extra warps more than the registers.
+#ifndef QSL_T2_THREADS
+#define QSL_T2_THREADS 128
+#endif
 #ifndef QSL_T2_MIN_BLOCKS_LQ
 #define QSL_T2_MIN_BLOCKS_LQ 3
 #endif
@@ -359,7 +420,7 @@ struct LineState2 {
 #define QSL_T2_MIN_BLOCKS_L 4
 #endif
 template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL>
-__global__ void __launch_bounds__(128, DEV ? QSL_T2_MIN_BLOCKS_LQ : QSL_T2_MIN_BLOCKS_L) trace2_kernel(const TraceArgs A)
+__global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : QSL_T2_MIN_BLOCKS_L) trace2_kernel(const TraceArgs A)
 {
     LineState2<DEV, STRETCHED, INTERP> ls;
     const long long n_items = 2 * A.n;

@@ -21,7 +21,7 @@ struct TraceArgs {
     double inv_h[3];             // 1 / uniform spacing
     double box_lo[3], box_hi[3];
     double h_uniform;            // step_frac * min_d h_d on a uniform grid
-    unsigned h_hi[3];            // high words of the uniform spacings (in-cell test of the V2 kernel)
+    unsigned h_hi[3];            // high words of the uniform spacings (in-cell test of the cell-table kernel)
     double step_frac, max_length, null_eps;
     long long max_steps;
     int method;
@@ -32,10 +32,12 @@ struct TraceArgs {
     double *rec;                 // 2n per-direction records of REC_DOUBLES doubles, index = dir*n + pos
     unsigned long long *total_steps;
     unsigned long long *queue;   // work counter of the persistent kernel
+    const double *basis;         // cell-table kernel, QSL_TRACE_LQ: n*6 (a^, b^) per seed in sorted order (seed_basis_kernel)
+    double *stash;               // cell-table kernel: per-thread landing scratch, STASH_DOUBLES x n_threads
 };
 
 // Per-direction record written once when a line ends: x[3], d1[3], d2[3], L, (nsteps, face|flags) as two uint32, lambda.
-constexpr int REC_DOUBLES = 14;    // [12], [13] are only used as the landing stash of the V2 kernel
+constexpr int REC_DOUBLES = 12;
 constexpr uint32_t REC_STALL = 1u << 8, REC_CAP = 1u << 9, REC_SEED_OUTSIDE = 1u << 10, REC_NULL_AT_SEED = 1u << 11;
 
 template <typename S> struct Sample4;
