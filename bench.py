@@ -244,13 +244,15 @@ def main():
     qsl.qsl_profile_enable(True)
 
     def step_device():
-        """One pass of the hot path, inputs resident.  Returns (lines traced, RK steps tensor)."""
+        """One pass of the hot path, inputs resident.  Returns (lines traced, RK steps tensor [L-only, L+Q])."""
         if levels == 0:
             res = qsl.qsl_trace(field, seeds, pLQ if mode == 1 else pL, outputs=outs, out=out_bufs, total_steps=tot)
             out_bufs.update(res)
-            return n, tot
+            two = torch.zeros(2, dtype=torch.int64, device="cuda")
+            two[mode:mode + 1] = tot
+            return n, two
         r = qsl.adaptive_map(field, lat, seeds, pL, pLQ, levels, cfg["p"])
-        return n + sum(int(s.shape[0]) for s in r["seeds"][1:]), r["total_steps"]
+        return n + sum(int(s.shape[0]) for s in r["seeds"][1:]), r["steps_by_mode"]
 
     host_out = {}
 
@@ -287,8 +289,8 @@ def main():
     l0 = qsl.lib().qsl_launch_count()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     lines = 0
-    rk = torch.zeros(1, dtype=torch.int64, device="cuda")
-    kern_ms = []
+    rk = torch.zeros(2, dtype=torch.int64, device="cuda")
+    kern_ms, kern_n = [0.0, 0.0], [0, 0]
     with ClockSampler(local) as clocks:
         t_wall = time.perf_counter()
         for a, b in ev:
@@ -298,13 +300,15 @@ def main():
             b.record()
             rk += s
             lines += m
-            if levels == 0:
-                kern_ms.append(qsl.qsl_profile_trace_kernel_ms())
+            kms, kn = qsl.qsl_profile_trace_kernel_ms()      # waits for this step's trace kernels (after b.record())
+            for q in (0, 1):
+                kern_ms[q] += kms[q]; kern_n[q] += kn[q]
         barrier()
         t_wall = time.perf_counter() - t_wall
     launches = qsl.lib().qsl_launch_count() - l0
     dev_ms = sum(a.elapsed_time(b) for a, b in ev)
-    rk_steps = int(rk.item())
+    rk_by_mode = [int(v) for v in rk.tolist()]
+    rk_steps = sum(rk_by_mode)
     t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
     agg = torch.tensor([float(lines), float(rk_steps)], dtype=torch.float64, device="cuda")
     if dist is not None:
@@ -335,25 +339,25 @@ def main():
     # ---- roofline of the dominant kernel (trace kernel) against the measured FP pipe peak ---------------------------
     roofline = None
     if rank == 0:
-        tag = "LQ" if mode == 1 else "L"
         peak_fma = qsl.qsl_peak_fma(True)              # DFMA/s; arithmetic is fp64 whatever the sample type
         peak = 2.0 * peak_fma / 1e12
-        if levels == 0 and kern_ms:
-            k_ms = sum(kern_ms) / len(kern_ms)
-            steps_per_launch = rk_steps / args.steps
-            achieved = 2.0 * PIPE_SLOTS_PER_STEP[tag] * steps_per_launch / (k_ms * 1e-3) / 1e12
-            roofline = {"bound": "alu", "kernel": "trace_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                        "frac": achieved / peak, "traffic": NCU_TRACE_KERNEL_DRAM_BYTES.get(args.workload),
-                        "kernel_ms": k_ms, "kernel_share_of_step": k_ms * args.steps / dev_ms,
-                        "convention": "FP64 pipe issue slots x 2 (FMA-equivalent flops): %d slots per RK4 step (%s); "
-                                      "peak = DFMA rate measured by qsl_peak_fma on this device" % (PIPE_SLOTS_PER_STEP[tag], tag),
-                        "true_flops_achieved_tflops": FLOPS_PER_STEP[tag] * steps_per_launch / (k_ms * 1e-3) / 1e12}
-        else:
-            # level loop: several trace launches of both modes per step; report the pipe fraction of the whole step
-            achieved = 2.0 * PIPE_SLOTS_PER_STEP["L"] * (rk_steps / args.steps) / (dev_ms / args.steps * 1e-3) / 1e12
-            roofline = {"bound": "alu", "kernel": "trace_kernel (all levels, whole step; lower bound: every step "
-                        "counted at the L-only cost)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                        "frac": achieved / peak, "traffic": None}
+        # algorithmic FP64 issue slots of all trace-kernel launches of the timed region (both modes) / their device time
+        slots = PIPE_SLOTS_PER_STEP["L"] * rk_by_mode[0] + PIPE_SLOTS_PER_STEP["LQ"] * rk_by_mode[1]
+        flops = FLOPS_PER_STEP["L"] * rk_by_mode[0] + FLOPS_PER_STEP["LQ"] * rk_by_mode[1]
+        k_ms = kern_ms[0] + kern_ms[1]
+        achieved = 2.0 * slots / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "trace2_kernel (cell-table trace kernel; all %d launches of the timed region)"
+                    % (kern_n[0] + kern_n[1]), "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                    "frac": achieved / peak, "traffic": NCU_TRACE_KERNEL_DRAM_BYTES.get(args.workload),
+                    "kernel_ms": k_ms / args.steps, "kernel_share_of_step": k_ms / dev_ms,
+                    "launches_per_step": (kern_n[0] + kern_n[1]) / args.steps,
+                    "by_mode": {m: {"rk_steps_per_step": rk_by_mode[q] / args.steps, "kernel_ms_per_step": kern_ms[q] / args.steps,
+                                    "frac": (2.0 * PIPE_SLOTS_PER_STEP[m] * rk_by_mode[q] / (kern_ms[q] * 1e-3) / 1e12 / peak)
+                                    if kern_ms[q] > 0 else None} for q, m in enumerate(("L", "LQ"))},
+                    "convention": "FP64 pipe issue slots x 2 (FMA-equivalent flops): %d slots per RK4 step with Q, %d "
+                                  "without; peak = DFMA rate measured by qsl_peak_fma on this device"
+                                  % (PIPE_SLOTS_PER_STEP["LQ"], PIPE_SLOTS_PER_STEP["L"]),
+                    "true_flops_achieved_tflops": flops / (k_ms * 1e-3) / 1e12}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

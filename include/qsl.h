@@ -165,12 +165,13 @@ int qsl_debug_sort_pairs(unsigned int *keys, unsigned int *vals, long long n, in
 
 /* ---- measurement hooks (bench.py) ------------------------------------------------------------------ */
 /* qsl_profile_enable(1): every later qsl_trace records a CUDA event pair around its trace kernel (the dominant
- * kernel) on the caller's stream.  qsl_profile_trace_kernel_ms waits for the most recent pair and returns the device
- * time between them in milliseconds (host pointer); QSL_EINVAL if no trace ran with profiling on.                   */
+ * kernel) on the caller's stream (up to 256 launches between two reads).  qsl_profile_trace_kernel_ms waits for the pairs
+ * recorded since the previous read (or enable), returns their summed device time in milliseconds and their number per
+ * trace mode (host arrays indexed by QSL_TRACE_L, QSL_TRACE_LQ) and forgets them; QSL_EINVAL if there were none.      */
 /* Number of kernels the library has launched in this process so far (bench.py's gpu_launches). */
 long long qsl_launch_count(void);
 int qsl_profile_enable(int on);
-int qsl_profile_trace_kernel_ms(double *ms);
+int qsl_profile_trace_kernel_ms(double ms[2], long long launches[2]);
 /* Roofline denominators measured on this device, each timed with CUDA events (2 warm-up launches, best of `reps`);
  * both synchronise.  fma_per_s (host): fused multiply-adds per second of the plain FP pipe, fp64 != 0 -> DFMA, else
  * FFMA, from 8 independent register-only chains per thread.  samples_per_s (host): divergent pseudo-random gathers per

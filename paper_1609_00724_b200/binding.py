@@ -281,10 +281,13 @@ def qsl_profile_enable(on: bool = True):
     _check(lib().qsl_profile_enable(C.c_int(1 if on else 0)), "qsl_profile_enable")
 
 
-def qsl_profile_trace_kernel_ms() -> float:
-    ms = C.c_double(0.0)
-    _check(lib().qsl_profile_trace_kernel_ms(C.byref(ms)), "qsl_profile_trace_kernel_ms")
-    return ms.value
+def qsl_profile_trace_kernel_ms():
+    """(ms, launches): device time and number of the trace-kernel launches since the previous read, each a 2-tuple
+    indexed by trace mode (QSL_TRACE_L, QSL_TRACE_LQ)."""
+    ms = (C.c_double * 2)()
+    n = (C.c_longlong * 2)()
+    _check(lib().qsl_profile_trace_kernel_ms(ms, n), "qsl_profile_trace_kernel_ms")
+    return (ms[0], ms[1]), (int(n[0]), int(n[1]))
 
 
 def qsl_peak_fma(fp64: bool, reps: int = 5, stream=None) -> float:

@@ -15,28 +15,42 @@ cudaError_t launch_epilogue_f64(const EpilogueArgs &E, cudaStream_t s);
 
 using namespace qsl;
 
-// Measurement hook: an event pair around the trace kernel (qsl_profile_enable / qsl_profile_trace_kernel_ms).
-static int g_profile = 0, g_profile_valid = 0;
-static cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+// Measurement hook: an event pair around every trace-kernel launch (qsl_profile_enable / qsl_profile_trace_kernel_ms).
+constexpr int PROF_MAX = 256;
+static int g_profile = 0, g_prof_n = 0;
+static cudaEvent_t g_ev0[PROF_MAX], g_ev1[PROF_MAX];
+static int g_prof_mode[PROF_MAX], g_prof_made = 0;
 
 extern "C" int qsl_profile_enable(int on)
 {
-    if (on && !g_ev0) {
-        QSL_CUDA(cudaEventCreate(&g_ev0));
-        QSL_CUDA(cudaEventCreate(&g_ev1));
-    }
     g_profile = on ? 1 : 0;
-    g_profile_valid = 0;
+    g_prof_n = 0;
     return QSL_OK;
 }
 
-extern "C" int qsl_profile_trace_kernel_ms(double *ms)
+// Next free event pair (created on first use), or -1 when the pool is full (the launch is then not timed).
+static int prof_slot(int mode)
 {
-    if (!ms || !g_profile_valid) return QSL_EINVAL;
-    QSL_CUDA(cudaEventSynchronize(g_ev1));
-    float t = 0.f;
-    QSL_CUDA(cudaEventElapsedTime(&t, g_ev0, g_ev1));
-    *ms = (double)t;
+    if (!g_profile || g_prof_n >= PROF_MAX) return -1;
+    if (g_prof_n >= g_prof_made) {
+        if (cudaEventCreate(&g_ev0[g_prof_made]) != cudaSuccess || cudaEventCreate(&g_ev1[g_prof_made]) != cudaSuccess) return -1;
+        ++g_prof_made;
+    }
+    g_prof_mode[g_prof_n] = mode;
+    return g_prof_n++;
+}
+
+extern "C" int qsl_profile_trace_kernel_ms(double ms[2], long long launches[2])
+{
+    if (!ms || !launches || g_prof_n == 0) return QSL_EINVAL;
+    ms[0] = ms[1] = 0.0; launches[0] = launches[1] = 0;
+    for (int i = 0; i < g_prof_n; ++i) {
+        QSL_CUDA(cudaEventSynchronize(g_ev1[i]));
+        float t = 0.f;
+        QSL_CUDA(cudaEventElapsedTime(&t, g_ev0[i], g_ev1[i]));
+        ms[g_prof_mode[i]] += (double)t; ++launches[g_prof_mode[i]];
+    }
+    g_prof_n = 0;
     return QSL_OK;
 }
 
@@ -85,13 +99,14 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         const bool v2 = f->view.cells != nullptr && !(p->flags & QSL_FLAG_KERNEL_V1);
         if (e == cudaSuccess && v2) {
             // the cell-table kernel allocates its own scratch and brackets its launch with the profiling events
-            rc = launch_trace2(A, dev, refill, g_profile ? g_ev0 : nullptr, g_profile ? g_ev1 : nullptr, s);
-            if (rc == QSL_OK && g_profile) g_profile_valid = 1;
+            const int ps = prof_slot(p->mode);
+            rc = launch_trace2(A, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
         } else if (e == cudaSuccess) {
-            if (g_profile) e = cudaEventRecord(g_ev0, s);
+            const int ps = prof_slot(p->mode);
+            if (ps >= 0) e = cudaEventRecord(g_ev0[ps], s);
             if (e == cudaSuccess)
                 e = f->sample_type == QSL_F32 ? launch_trace_f32(A, dev, refill, s) : launch_trace_f64(A, dev, refill, s);
-            if (e == cudaSuccess && g_profile) { e = cudaEventRecord(g_ev1, s); g_profile_valid = 1; }
+            if (e == cudaSuccess && ps >= 0) e = cudaEventRecord(g_ev1[ps], s);
         }
         if (rc != QSL_OK) e = cudaErrorUnknown;
         if (e == cudaSuccess) {

@@ -18,14 +18,15 @@ def adaptive_map(field, lattice, seeds0, params_L, params_LQ, n_levels: int, p: 
 
     seeds0: CUDA float64 (n0*n1*n2, 3) level-0 seeds in dense index order.
     Returns a dict: L0 (dense map), S0, tau (CUDA float64[1]) and per-level lists coords / seeds / out (trace outputs) /
-    S / child_base, plus `total_steps` (CUDA int64[1], summed over all levels).
+    S / child_base, plus `total_steps` (CUDA int64[1], summed over all levels) and `steps_by_mode` (CUDA int64[2]: RK
+    steps of the L-only level-0 pass and of the L+Q passes over the refined seeds).
     """
     ndim = int(lattice.ndim)
     shape = tuple(int(v) for v in lattice.n[:ndim][::-1])
     steps = torch.zeros(1, dtype=torch.int64, device="cuda")
-    acc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    acc = torch.zeros(2, dtype=torch.int64, device="cuda")
     o0 = B.qsl_trace(field, seeds0, params_L, outputs=("L", "status"), total_steps=steps, stream=stream)
-    acc += steps
+    acc[0:1] += steps
     L0 = o0["L"]
     S0 = B.qsl_fledge_dense(L0.view(shape), ndim, stream=stream).view(-1)
     tau = B.qsl_select(S0, p, stream=stream)
@@ -40,12 +41,13 @@ def adaptive_map(field, lattice, seeds0, params_L, params_LQ, n_levels: int, p: 
             res["out"].append(None); res["S"].append(None)
             break
         o = B.qsl_trace(field, cs, params_LQ, outputs=outputs, total_steps=steps, stream=stream)
-        acc += steps
+        acc[1:2] += steps
         res["out"].append(o)
         Ls.append(o["L"])
         if level + 1 < n_levels:
             S = B.qsl_fledge_sparse(lattice, level + 1, L0, res["coords"], Ls, res["child_base"], stream=stream)
             res["S"].append(S)
             coords = cc
-    res["total_steps"] = acc
+    res["steps_by_mode"] = acc
+    res["total_steps"] = acc.sum(0, keepdim=True)
     return res
