@@ -283,15 +283,21 @@ def main():
         torch.cuda.synchronize()
 
     # ---- device-resident timing -------------------------------------------------------------------------------------
+    # NVML is initialised and its sampling thread started before the warm-up: its first calls take driver locks that
+    # would otherwise delay the launches of the first timed step; the samples of the warm-up are dropped below.
+    clocks = ClockSampler(local)
+    clocks.__enter__()
     for _ in range(max(args.warmup, 3) if args.warmup > 0 else 0):
         step_device()
     barrier()
+    qsl.qsl_profile_enable(True)               # drop the warm-up launches from the trace-kernel event pool
     l0 = qsl.lib().qsl_launch_count()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     lines = 0
     rk = torch.zeros(2, dtype=torch.int64, device="cuda")
     kern_ms, kern_n = [0.0, 0.0], [0, 0]
-    with ClockSampler(local) as clocks:
+    try:
+        clocks.samples.clear(); clocks.reasons.clear()
         t_wall = time.perf_counter()
         for a, b in ev:
             flush.zero_()                      # L2 flush, outside the event pair
@@ -305,6 +311,8 @@ def main():
                 kern_ms[q] += kms[q]; kern_n[q] += kn[q]
         barrier()
         t_wall = time.perf_counter() - t_wall
+    finally:
+        clocks.__exit__()
     launches = qsl.lib().qsl_launch_count() - l0
     dev_ms = sum(a.elapsed_time(b) for a, b in ev)
     rk_by_mode = [int(v) for v in rk.tolist()]
@@ -372,6 +380,7 @@ def main():
             "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
             "rk_steps_per_s": steps_all / (dev_ms_max * 1e-3), "rk_steps_per_step": rk_steps / args.steps,
             "lines_per_step": lines / args.steps, "wall_s_timed_region": t_wall,
+            "ms_each_step": [round(a.elapsed_time(b), 3) for a, b in ev],
             "clocks": clocks.summary(),
             "e2e": {"value": lines_all / (e2e_ms_max * 1e-3), "unit": "lines/s", "h2d_bytes_per_step": bi,
                     "d2h_bytes_per_step": bo, "ms_per_step": e2e_ms_max / args.steps},
