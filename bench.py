@@ -39,7 +39,7 @@ PIPE_SLOTS_PER_STEP = {"LQ": 490, "L": 245}
 FLOPS_PER_STEP = {"LQ": 800, "L": 400}
 # dram__bytes_read.sum + dram__bytes_write.sum of one trace-kernel launch of the default workload, from the committed
 # ncu --set full capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRACE_KERNEL_DRAM_BYTES = {}
+NCU_TRACE_KERNEL_DRAM_BYTES = {"cfg2": 789848320}   # profiles/r1b_cell_table_kernel.md
 
 
 def _env_int(name, default):
@@ -202,6 +202,9 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=sorted(WORKLOADS))
     ap.add_argument("--scale", type=float, default=1.0, help="shrink grid and seed lattice (debugging only)")
     ap.add_argument("--flags", type=int, default=0, help="QSL_FLAG_* tuning flags (debugging only)")
+    ap.add_argument("--arith", default="f64", choices=["f64", "f32"],
+                    help="arithmetic of the integrator; f32 = QSL_ARITH_F32 throughput mode (fp32-sampled workloads only; "
+                         "parity is gated in f64, DESIGN.md reading A6)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -226,7 +229,11 @@ def main():
     g = cfg["grid"]
     dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda() for a in cfg["B"]]
     st = qsl.QSL_F32 if cfg["sample_type"] == "f32" else qsl.QSL_F64
-    field = qsl.qsl_field_create(g.nx, g.ny, g.nz, *dev, lo=g.lo, hi=g.hi, sample_type=st)
+    f32 = args.arith == "f32"
+    if f32 and cfg["sample_type"] != "f32":
+        raise SystemExit("--arith f32 needs an fp32-sampled workload (cfg4, cfg5)")
+    field = qsl.qsl_field_create(g.nx, g.ny, g.nz, *dev, lo=g.lo, hi=g.hi, sample_type=st,
+                                 layout=qsl.QSL_LAYOUT_CELL_TABLE_F32 if f32 else qsl.QSL_LAYOUT_CELL_TABLE)
     del dev
     seeds_host = torch.from_numpy(np.ascontiguousarray(cfg["seeds"])).pin_memory()
     n = int(seeds_host.shape[0])
@@ -234,7 +241,8 @@ def main():
     mode = cfg["mode"]
     levels = int(cfg["levels"])
     mk = lambda m: qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=m, step_frac=cfg["step_frac"],
-                                         max_steps=cfg["max_steps"], null_eps=cfg["null_eps"], flags=args.flags)
+                                         max_steps=cfg["max_steps"], null_eps=cfg["null_eps"], flags=args.flags,
+                                         arith=qsl.QSL_ARITH_F32 if f32 else qsl.QSL_ARITH_F64)
     pL, pLQ = mk(qsl.QSL_TRACE_L), mk(qsl.QSL_TRACE_LQ)
     outs = ("end_f", "end_b", "L", "q_perp", "q_bnd", "face_f", "face_b", "status")
     out_bufs = {}
@@ -347,24 +355,25 @@ def main():
     # ---- roofline of the dominant kernel (trace kernel) against the measured FP pipe peak ---------------------------
     roofline = None
     if rank == 0:
-        peak_fma = qsl.qsl_peak_fma(True)              # DFMA/s; arithmetic is fp64 whatever the sample type
+        peak_fma = qsl.qsl_peak_fma(not f32)           # DFMA/s (FFMA/s with --arith f32), measured on this device
         peak = 2.0 * peak_fma / 1e12
         # algorithmic FP64 issue slots of all trace-kernel launches of the timed region (both modes) / their device time
         slots = PIPE_SLOTS_PER_STEP["L"] * rk_by_mode[0] + PIPE_SLOTS_PER_STEP["LQ"] * rk_by_mode[1]
         flops = FLOPS_PER_STEP["L"] * rk_by_mode[0] + FLOPS_PER_STEP["LQ"] * rk_by_mode[1]
         k_ms = kern_ms[0] + kern_ms[1]
         achieved = 2.0 * slots / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "trace2_kernel (cell-table trace kernel; all %d launches of the timed region)"
-                    % (kern_n[0] + kern_n[1]), "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+        roofline = {"bound": "alu", "kernel": "%s (cell-table trace kernel; all %d launches of the timed region)"
+                    % ("trace3_kernel, fp32 arithmetic" if f32 else "trace2_kernel", kern_n[0] + kern_n[1]), "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                     "frac": achieved / peak, "traffic": NCU_TRACE_KERNEL_DRAM_BYTES.get(args.workload),
                     "kernel_ms": k_ms / args.steps, "kernel_share_of_step": k_ms / dev_ms,
                     "launches_per_step": (kern_n[0] + kern_n[1]) / args.steps,
                     "by_mode": {m: {"rk_steps_per_step": rk_by_mode[q] / args.steps, "kernel_ms_per_step": kern_ms[q] / args.steps,
                                     "frac": (2.0 * PIPE_SLOTS_PER_STEP[m] * rk_by_mode[q] / (kern_ms[q] * 1e-3) / 1e12 / peak)
                                     if kern_ms[q] > 0 else None} for q, m in enumerate(("L", "LQ"))},
-                    "convention": "FP64 pipe issue slots x 2 (FMA-equivalent flops): %d slots per RK4 step with Q, %d "
-                                  "without; peak = DFMA rate measured by qsl_peak_fma on this device"
-                                  % (PIPE_SLOTS_PER_STEP["LQ"], PIPE_SLOTS_PER_STEP["L"]),
+                    "convention": "%s pipe issue slots x 2 (FMA-equivalent flops): %d slots per RK4 step with Q, %d "
+                                  "without; peak = %s rate measured by qsl_peak_fma on this device"
+                                  % ("FP32" if f32 else "FP64", PIPE_SLOTS_PER_STEP["LQ"], PIPE_SLOTS_PER_STEP["L"],
+                                     "FFMA" if f32 else "DFMA"),
                     "true_flops_achieved_tflops": flops / (k_ms * 1e-3) / 1e12}
 
     cpu = None
@@ -377,7 +386,7 @@ def main():
             "metric": "field lines/s (with Q)", "value": lines_all / (dev_ms_max * 1e-3), "unit": "lines/s",
             "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3) if args.warmup > 0 else 0,
             "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
+            "dtype": "f32" if f32 else "f64", "data": "synthetic", "config": workload_config(cfg, args),
             "rk_steps_per_s": steps_all / (dev_ms_max * 1e-3), "rk_steps_per_step": rk_steps / args.steps,
             "lines_per_step": lines / args.steps, "wall_s_timed_region": t_wall,
             "ms_each_step": [round(a.elapsed_time(b), 3) for a, b in ev],

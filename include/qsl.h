@@ -38,7 +38,8 @@ enum { QSL_F32 = 0, QSL_F64 = 1 };                       /* storage type of the 
 enum { QSL_NORMALIZE_FIRST = 0, QSL_INTERP_FIRST = 1 };  /* PAPER.md:178 (fn. 9) = NORMALIZE_FIRST, the default   */
 enum { QSL_RK4 = 0, QSL_EULER = 1 };                     /* PAPER.md:141; RK4: BASELINE.json configs (reading A5) */
 enum { QSL_TRACE_L = 0, QSL_TRACE_LQ = 1 };              /* L only (FLEDGE pass) | L and Q                        */
-enum { QSL_LAYOUT_CELL_TABLE = 0, QSL_LAYOUT_NODES_ONLY = 1 };  /* what qsl_field_create keeps in HBM (see qsl_grid_desc) */
+enum { QSL_LAYOUT_CELL_TABLE = 0, QSL_LAYOUT_NODES_ONLY = 1,    /* what qsl_field_create keeps in HBM (see qsl_grid_desc) */
+       QSL_LAYOUT_CELL_TABLE_F32 = 2, QSL_LAYOUT_CELL_TABLES_BOTH = 3 };
 enum { QSL_ARITH_F64 = 0, QSL_ARITH_F32 = 1 };           /* arithmetic of the integrator (F32 only with F32 samples) */
 
 /* status bits of qsl_trace_out.status */
@@ -69,7 +70,11 @@ typedef struct {
                                     24 fp64 monomial coefficients of its trilinear interpolant (192 B per cell; 6x the
                                     fp64 samples, 12x the fp32 samples) - what the fast trace kernel reads.
                                     QSL_LAYOUT_NODES_ONLY: packed samples only; qsl_trace then gathers 8 corners per
-                                    RK stage (the slower QSL_FLAG_KERNEL_V1 path), for fields too large for the table */
+                                    RK stage (the slower QSL_FLAG_KERNEL_V1 path), for fields too large for the table.
+                                    QSL_LAYOUT_CELL_TABLE_F32: the same coefficients rounded to fp32 (96 B per cell),
+                                    the table of QSL_ARITH_F32; fp32 samples on a uniform grid only (else QSL_EINVAL);
+                                    QSL_ARITH_F64 traces of such a field run the corner kernel.
+                                    QSL_LAYOUT_CELL_TABLES_BOTH: the fp64 and the fp32 table                          */
 } qsl_grid_desc;
 
 /* Packs the three component cubes (DEVICE, fp64, nx*ny*nz each) into one AoS array of (b^x, b^y, b^z, |B|) samples

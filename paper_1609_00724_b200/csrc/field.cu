@@ -78,8 +78,9 @@ __global__ void __launch_bounds__(256) pack_kernel(long long n, const double *__
 // so that value and analytic gradient cost 11 FMAs per component instead of 25 from the corners.
 // The coefficients are finite differences of the 8 corner samples (converted exactly to fp64) divided by the cell
 // edges; 24 doubles = 192 B per cell, component-major, cell index (k (ny-1) + j)(nx-1) + i.
-template <typename S4>
-__global__ void __launch_bounds__(256) cell_table_kernel(FieldView fv, double4 *__restrict__ cells)
+// O4 = double4 (192 B per cell, the fp64 kernels) or float4 (coefficients rounded to fp32, 96 B per cell, QSL_ARITH_F32).
+template <typename S4, typename O4>
+__global__ void __launch_bounds__(256) cell_table_kernel(FieldView fv, O4 *__restrict__ cells)
 {
     const int cx = fv.nx - 1, cy = fv.ny - 1, cz = fv.nz - 1;
     const long long n_cells = (long long)cx * cy * cz;
@@ -115,9 +116,13 @@ __global__ void __launch_bounds__(256) cell_table_kernel(FieldView fv, double4 *
             a[8 * c + 6] = v[6] * (ihy * ihz);
             a[8 * c + 7] = v[7] * ((ihx * ihy) * ihz);
         }
-        double4 *o = cells + (size_t)p * 6;
+        O4 *o = cells + (size_t)p * 6;
 #pragma unroll
-        for (int q = 0; q < 6; ++q) o[q] = make_double4(a[4 * q], a[4 * q + 1], a[4 * q + 2], a[4 * q + 3]);
+        for (int q = 0; q < 6; ++q) {
+            O4 w;
+            w.x = (decltype(w.x))a[4 * q]; w.y = (decltype(w.x))a[4 * q + 1]; w.z = (decltype(w.x))a[4 * q + 2]; w.w = (decltype(w.x))a[4 * q + 3];
+            o[q] = w;
+        }
     }
 }
 
@@ -158,7 +163,10 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     if (d->nx < 2 || d->ny < 2 || d->nz < 2) return QSL_EINVAL;
     if (d->sample_type != QSL_F32 && d->sample_type != QSL_F64) return QSL_EINVAL;
     if (d->interp_mode != QSL_NORMALIZE_FIRST && d->interp_mode != QSL_INTERP_FIRST) return QSL_EINVAL;
-    if (d->layout != QSL_LAYOUT_CELL_TABLE && d->layout != QSL_LAYOUT_NODES_ONLY) return QSL_EINVAL;
+    if (d->layout < QSL_LAYOUT_CELL_TABLE || d->layout > QSL_LAYOUT_CELL_TABLES_BOTH) return QSL_EINVAL;
+    const bool want64 = d->layout == QSL_LAYOUT_CELL_TABLE || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH;
+    const bool want32 = d->layout == QSL_LAYOUT_CELL_TABLE_F32 || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH;
+    if (want32 && (d->sample_type != QSL_F32 || d->stretched)) return QSL_EINVAL;   // fp32 arithmetic: fp32 samples, uniform grid
     const long long n = (long long)d->nx * d->ny * d->nz;
     if (n >= (1ll << 31)) return QSL_ERANGE;   // node index is 32-bit inside the gather
     const int dims[3] = { d->nx, d->ny, d->nz };
@@ -178,6 +186,7 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     if (!f) return QSL_ENOMEM;
     f->d_samples = nullptr;
     f->d_cells = nullptr;
+    f->d_cells32 = nullptr;
     f->view.cells = nullptr;
     for (int a = 0; a < 3; ++a) f->d_axis[a] = nullptr;
     f->sample_type = d->sample_type;
@@ -221,7 +230,7 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
         pack_kernel<double4, double><<<blocks, threads, 0, s>>>(n, bx, by, bz, d->interp_mode, (double4 *)f->d_samples);
     e = cudaGetLastError();
     if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
-    if (d->layout == QSL_LAYOUT_CELL_TABLE) {
+    if (want64) {
         const long long n_cells = (long long)(d->nx - 1) * (d->ny - 1) * (d->nz - 1);
         const size_t cbytes = (size_t)n_cells * 24 * sizeof(double);
         e = cudaMalloc(&f->d_cells, cbytes);
@@ -230,11 +239,25 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
         const long long want = (n_cells + threads - 1) / threads, cap = (long long)sm_count() * 16;
         const int cblocks = (int)(want < cap ? want : cap);
         count_launch();
-        if (d->sample_type == QSL_F32) cell_table_kernel<float4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
-        else cell_table_kernel<double4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
+        if (d->sample_type == QSL_F32) cell_table_kernel<float4, double4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
+        else cell_table_kernel<double4, double4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
         e = cudaGetLastError();
         if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
         f->view.cells = f->d_cells;
+    }
+    if (want32) {
+        const long long n_cells = (long long)(d->nx - 1) * (d->ny - 1) * (d->nz - 1);
+        if (n_cells >= (1ll << 31)) { qsl_field_destroy(f); return QSL_ERANGE; }   // 32-bit cell index in the fp32 kernel
+        const size_t cbytes = (size_t)n_cells * 24 * sizeof(float);
+        e = cudaMalloc(&f->d_cells32, cbytes);
+        if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+        f->bytes += cbytes;
+        const long long want = (n_cells + threads - 1) / threads, cap = (long long)sm_count() * 16;
+        const int cblocks = (int)(want < cap ? want : cap);
+        count_launch();
+        cell_table_kernel<float4, float4><<<cblocks, threads, 0, s>>>(f->view, (float4 *)f->d_cells32);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
     }
     *out = f;
     return QSL_OK;
@@ -245,6 +268,7 @@ int qsl_field_destroy(qsl_field *f)
     if (!f) return QSL_OK;
     if (f->d_samples) cudaFree(f->d_samples);
     if (f->d_cells) cudaFree(f->d_cells);
+    if (f->d_cells32) cudaFree(f->d_cells32);
     for (int a = 0; a < 3; ++a)
         if (f->d_axis[a]) cudaFree(f->d_axis[a]);
     delete f;

@@ -51,6 +51,7 @@ struct qsl_field {
     qsl::FieldView view;
     void *d_samples;
     void *d_cells;
+    void *d_cells32;          // fp32 coefficient table of the QSL_ARITH_F32 kernel, or NULL
     double *d_axis[3];
     int sample_type;
     long long n_nodes;

@@ -9,6 +9,7 @@ namespace qsl {
 cudaError_t launch_trace_f32(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 cudaError_t launch_trace_f64(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 int launch_trace2(TraceArgs &A, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
+int launch_trace3(const TraceArgs &T, const void *cells32, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 cudaError_t launch_epilogue_f32(const EpilogueArgs &E, cudaStream_t s);
 cudaError_t launch_epilogue_f64(const EpilogueArgs &E, cudaStream_t s);
 }  // namespace qsl
@@ -61,7 +62,9 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
     if (p->method != QSL_RK4 && p->method != QSL_EULER) return QSL_EINVAL;
     if (p->mode != QSL_TRACE_L && p->mode != QSL_TRACE_LQ) return QSL_EINVAL;
     if (p->arith != QSL_ARITH_F64 && p->arith != QSL_ARITH_F32) return QSL_EINVAL;
-    if (p->arith == QSL_ARITH_F32) return QSL_EINVAL;   // throughput mode not built yet
+    // fp32 arithmetic (reading A6): needs the fp32 coefficient table (QSL_LAYOUT_CELL_TABLE_F32 / _BOTH), which
+    // qsl_field_create only builds for fp32 samples on a uniform grid
+    if (p->arith == QSL_ARITH_F32 && !f->d_cells32) return QSL_EINVAL;
     if (!(p->step_frac > 0.0) || p->max_steps < 1 || !(p->max_length > 0.0) || !(p->null_eps >= 0.0)) return QSL_EINVAL;
     for (int d = 0; d < 3; ++d)
         if (!(p->box_hi[d] >= p->box_lo[d])) return QSL_EINVAL;
@@ -97,7 +100,10 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
         const bool dev = p->mode == QSL_TRACE_LQ;
         const bool v2 = f->view.cells != nullptr && !(p->flags & QSL_FLAG_KERNEL_V1);
-        if (e == cudaSuccess && v2) {
+        if (e == cudaSuccess && p->arith == QSL_ARITH_F32) {
+            const int ps = prof_slot(p->mode);
+            rc = launch_trace3(A, f->d_cells32, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
+        } else if (e == cudaSuccess && v2) {
             // the cell-table kernel allocates its own scratch and brackets its launch with the profiling events
             const int ps = prof_slot(p->mode);
             rc = launch_trace2(A, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);

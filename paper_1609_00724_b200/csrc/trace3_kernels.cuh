@@ -1,0 +1,479 @@
+// fp32-arithmetic trace kernel (QSL_ARITH_F32, reading A6 of DESIGN.md: the throughput mode for fp32-sampled fields).
+// The same method and state machine as trace2_kernels.cuh (PAPER.md:79 eq. 1, :119 eq. 5, :141, :163; readings A3-A5),
+// re-designed for single precision instead of re-typed:
+//
+//  * the position is never held as an absolute fp32 coordinate (ulp(1.0f) = 6e-8 is 1.5e-5 of a 1/255 cell): a line
+//    carries the integer index C of the cell whose polynomial is cached and the fp32 offset of its point from that
+//    cell's origin.  Offsets are < 2 h, so their rounding is ~1e-10 of the box, and a cell change is an integer
+//    neighbour step plus one subtraction of h - no floating-point search;
+//  * the per-cell table holds the 24 monomial coefficients as fp32 (96 B = 3 sectors per cell, half the fp64 table);
+//  * the trace box is given in cell coordinates (cell index + offset per face), so the "inside the box" test is an
+//    integer compare for every cell that does not touch a face of the box;
+//  * L and lambda are accumulated in fp64 (two DADD per step): summing ~1e3 increments of ~1e-3 in fp32 would by itself
+//    cost 1e-6 of L.
+// End records are written in fp64 (origin of the cell + offset), so the epilogue (eq. 11) is shared.
+#pragma once
+#include "trace_kernels.cuh"
+
+namespace qsl {
+
+struct Trace3Args {
+    TraceArgs T;
+    const float4 *cells32;       // 6 float4 per cell: monomial coefficients a[8 c + m] of the trilinear interpolant
+    float hf[3];                 // cell edges
+    float h_step;                // step_frac * min_d h_d
+    int cmax[3];                 // n_d - 2: last cell index per axis
+    int cell_sy, cell_sz;        // table strides in cells
+    int cl[3], ch[3];            // cells containing box_lo / box_hi (box_hi on a node belongs to the cell below it)
+    unsigned cw[3];              // max(ch - cl - 1, 0): number of cells strictly between them
+    float off_lo[3], off_hi[3];  // offsets of box_lo / box_hi from the origins of cells cl / ch
+    float null_eps;
+    float *stash;                // per-thread landing scratch, STASH3_FLOATS x n_threads
+};
+
+enum { S3_K1 = 0, S3_BN = 9, S3_DXT = 10, S3_HP = 13, S3_HFULL = 14, S3_AXIS_FACE = 15, STASH3_FLOATS = 16 };
+
+// |v| in fp32: hardware reciprocal square root and one Newton step (relative error ~1e-7); zero, subnormal, huge and
+// NaN arguments take the IEEE path.
+__device__ __forceinline__ float norm3f_fast(const float v[3])
+{
+    const float n2 = fmaf(v[2], v[2], fmaf(v[1], v[1], v[0] * v[0]));
+    if ((unsigned)(__float_as_int(n2) - 0x10000000) >= 0x60000000u) return sqrtf(n2);
+    const float r = rsqrtf(n2);
+    const float s = n2 * r;
+    return fmaf(fmaf(-s, s, n2), 0.5f * r, s);
+}
+
+template <bool DEV, bool INTERP>
+struct LineState3 {
+    static constexpr int NV = DEV ? 9 : 3;
+    float a[24];             // cached cell: monomial coefficients
+    int C[3];                // its index = the frame of every offset below
+    float y[NV];             // y[0..2]: offset of the line's point from the origin of cell C; delta1, delta2
+    double L, lam;
+    uint32_t nsteps, slot;
+    int phase;
+    bool back;
+
+    __device__ __forceinline__ void load_cell(const Trace3Args &A)
+    {
+        const float4 *__restrict__ p = A.cells32 + ((size_t)((unsigned)C[2] * (unsigned)A.cell_sz + (unsigned)C[1] * (unsigned)A.cell_sy + (unsigned)C[0])) * 6;
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            const float4 v = __ldg(p + q);
+            a[4 * q] = v.x; a[4 * q + 1] = v.y; a[4 * q + 2] = v.z; a[4 * q + 3] = v.w;
+        }
+    }
+
+    // Makes the cached cell the one containing the point at offsets p (reading A8: the index is clamped to the grid,
+    // the offset is not) by a neighbour step per axis, and moves the frame of p and of the line's own point with it.
+    // Consecutive evaluation points are at most half a cell apart (|b| <= 1, h = step_frac cell), so one step suffices.
+    // The "still inside" test is one unsigned compare per axis on the bit pattern: 0 <= p < h.
+    __device__ __forceinline__ void enter_cell(const Trace3Args &A, float p[3])
+    {
+        const unsigned u0 = (unsigned)__float_as_int(p[0]), u1 = (unsigned)__float_as_int(p[1]), u2 = (unsigned)__float_as_int(p[2]);
+        if (!(u0 < (unsigned)__float_as_int(A.hf[0]) && u1 < (unsigned)__float_as_int(A.hf[1]) && u2 < (unsigned)__float_as_int(A.hf[2]))) {
+            int s[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d)
+                s[d] = p[d] < 0.f ? (C[d] > 0 ? -1 : 0) : (p[d] >= A.hf[d] ? (C[d] < A.cmax[d] ? 1 : 0) : 0);
+            if (s[0] | s[1] | s[2]) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    C[d] += s[d];
+                    const float sh = (float)s[d] * A.hf[d];
+                    p[d] -= sh; y[d] -= sh;
+                }
+                load_cell(A);
+            }
+        }
+    }
+
+    // Field evaluation at offsets d inside the cached cell fused with the deviation products (as LineState2::stage).
+    __device__ __forceinline__ void stage(const float d[3], const float *ys, float b[3], float *k)
+    {
+        const float dx = d[0], dy = d[1], dz = d[2];
+        float v[3], g[9];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float *q = a + 8 * c;
+            const float P = fmaf(q[7], dz, q[3]), Q = fmaf(q[5], dz, q[1]), R = fmaf(q[6], dz, q[2]), S = fmaf(q[4], dz, q[0]);
+            const float E = fmaf(P, dy, Q), F = fmaf(R, dy, S);
+            v[c] = fmaf(E, dx, F);
+            if (DEV || INTERP) {
+                g[3 * c] = E;
+                g[3 * c + 1] = fmaf(P, dx, R);
+                g[3 * c + 2] = fmaf(fmaf(q[7], dy, q[5]), dx, fmaf(q[6], dy, q[4]));
+            }
+        }
+        if (!INTERP) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) b[c] = v[c];
+        } else {
+            // reading A2: b = B/|B|, J = (G - u (u^T G))/|B|
+            const float nn = sqrtf(fmaf(v[2], v[2], fmaf(v[1], v[1], v[0] * v[0])));
+            if (nn < 1e-37f) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) b[c] = 0.f;
+#pragma unroll
+                for (int q = 0; q < 9; ++q) g[q] = 0.f;
+            } else {
+                const float inv = 1.0f / nn;
+                const float u[3] = { v[0] * inv, v[1] * inv, v[2] * inv };
+#pragma unroll
+                for (int c = 0; c < 3; ++c) b[c] = u[c];
+                if (DEV) {
+#pragma unroll
+                    for (int e = 0; e < 3; ++e) {
+                        const float uG = fmaf(u[2], g[6 + e], fmaf(u[1], g[3 + e], u[0] * g[e]));
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) g[3 * c + e] = (g[3 * c + e] - u[c] * uG) * inv;
+                    }
+                }
+            }
+        }
+        if (DEV) {
+#pragma unroll
+            for (int w = 0; w < 2; ++w)
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    k[(3 + 3 * w + c) % NV] = fmaf(g[3 * c + 2], ys[(5 + 3 * w) % NV], fmaf(g[3 * c + 1], ys[(4 + 3 * w) % NV], g[3 * c] * ys[(3 + 3 * w) % NV]));
+        }
+    }
+
+    // Starts work item q (false if it ended at once: seed outside the trace box).  The seed's cell is found once, in
+    // fp64, exactly as O1 does (floor of (x - lo)/h, clamped); the basis a^, b^ of O2 comes from seed_basis3_kernel.
+    __device__ bool init(const Trace3Args &A, long long q)
+    {
+        const TraceArgs &T = A.T;
+        long long pos; int dir;
+        if (T.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= T.n ? 1 : 0; pos = q - (long long)dir * T.n; }
+        slot = (uint32_t)((long long)dir * T.n + pos);
+        back = dir != 0;
+        const uint32_t si = T.perm[pos];
+        const double x[3] = { T.seeds[3 * (size_t)si], T.seeds[3 * (size_t)si + 1], T.seeds[3 * (size_t)si + 2] };
+        L = 0.0; lam = 0.0; nsteps = 0; phase = 0;
+        if (!inside_box(T, x)) {
+            double out[REC_DOUBLES];
+#pragma unroll
+            for (int c = 0; c < REC_DOUBLES; ++c) out[c] = c < 3 ? x[c] : 0.0;
+            out[10] = __hiloint2double((int)(255u | REC_SEED_OUTSIDE), 0);
+            double2 *r2 = reinterpret_cast<double2 *>(T.rec + (size_t)slot * REC_DOUBLES);
+#pragma unroll
+            for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
+            return false;
+        }
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double u = (x[d] - T.fv.lo[d]) * T.inv_h[d];
+            int i = (int)floor(u);
+            i = max(0, min(i, A.cmax[d]));
+            C[d] = i;
+            y[d] = (float)(x[d] - fma((double)i, T.fv.h[d], T.fv.lo[d]));
+        }
+#pragma unroll
+        for (int c = 3; c < NV; ++c) y[c] = 0.f;
+        if (DEV) {
+            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(T.basis + 6 * (size_t)pos);
+            const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
+            y[3 % NV] = (float)b0.x; y[4 % NV] = (float)b0.y; y[5 % NV] = (float)b1.x;
+            y[6 % NV] = (float)b1.y; y[7 % NV] = (float)b2.x; y[8 % NV] = (float)b2.y;
+        }
+        load_cell(A);
+        return true;
+    }
+
+    // Writes the per-direction record in fp64: position = origin of the frame cell + offset; `snap` >= 0 puts the
+    // coordinate of that axis exactly on the face it landed on.
+    __device__ void finish(const Trace3Args &A, int face, uint32_t flags, int snap)
+    {
+        const TraceArgs &T = A.T;
+        double out[REC_DOUBLES];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) out[d] = fma((double)C[d], T.fv.h[d], T.fv.lo[d]) + (double)y[d];
+        if (snap >= 0) {
+            const double bd = (face & 1) ? (snap == 0 ? T.box_hi[0] : (snap == 1 ? T.box_hi[1] : T.box_hi[2]))
+                                         : (snap == 0 ? T.box_lo[0] : (snap == 1 ? T.box_lo[1] : T.box_lo[2]));
+            if (snap == 0) out[0] = bd; else if (snap == 1) out[1] = bd; else out[2] = bd;
+        }
+#pragma unroll
+        for (int c = 3; c < 9; ++c) out[c] = c < NV ? (double)y[c % NV] : 0.0;
+        out[9] = L;
+        out[10] = __hiloint2double((int)((uint32_t)face | flags), (int)nsteps);
+        out[11] = lam;
+        double2 *r2 = reinterpret_cast<double2 *>(T.rec + (size_t)slot * REC_DOUBLES);
+#pragma unroll
+        for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
+    }
+
+    // Offset, in the current frame, of the face (axis, upper?) of the trace box.
+    __device__ __forceinline__ float face_offset(const Trace3Args &A, int axis, bool upper) const
+    {
+        const int cd = axis == 0 ? C[0] : (axis == 1 ? C[1] : C[2]);
+        const int cb = upper ? (axis == 0 ? A.ch[0] : (axis == 1 ? A.ch[1] : A.ch[2])) : (axis == 0 ? A.cl[0] : (axis == 1 ? A.cl[1] : A.cl[2]));
+        const float ob = upper ? (axis == 0 ? A.off_hi[0] : (axis == 1 ? A.off_hi[1] : A.off_hi[2]))
+                               : (axis == 0 ? A.off_lo[0] : (axis == 1 ? A.off_lo[1] : A.off_lo[2]));
+        const float hd = axis == 0 ? A.hf[0] : (axis == 1 ? A.hf[1] : A.hf[2]);
+        return fmaf((float)(cb - cd), hd, ob);
+    }
+
+    // Is the point at offsets e of the frame cell inside the closed trace box?  Cells strictly between the cells that
+    // hold the faces of the box need one unsigned compare per axis; the others compare the offset with the face's.
+    __device__ __forceinline__ bool inside3(const Trace3Args &A, const float e[3]) const
+    {
+        if ((unsigned)(C[0] - A.cl[0] - 1) < A.cw[0] && (unsigned)(C[1] - A.cl[1] - 1) < A.cw[1] && (unsigned)(C[2] - A.cl[2] - 1) < A.cw[2])
+            return true;
+        bool in = true;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const bool lo_ok = C[d] > A.cl[d] || (C[d] == A.cl[d] && e[d] >= A.off_lo[d]);
+            const bool hi_ok = C[d] < A.ch[d] || (C[d] == A.ch[d] && e[d] <= A.off_hi[d]);
+            in = in && lo_ok && hi_ok;
+        }
+        return in;
+    }
+
+    // One attempt = exactly four field evaluations for every lane, whatever its phase (the state machine of
+    // LineState2::advance, reading A4): phase 0 trial step; phase 1 first landing step of size hp (k1 and the trial end,
+    // as a displacement from y so that it survives a change of frame, go to the stash); phases 2..4 spend the first
+    // evaluation at the previous trial end for one Newton update of hp; phase 4 lands.
+    __device__ bool advance(const Trace3Args &A)
+    {
+#define st (A.stash + ((size_t)blockIdx.x * blockDim.x + threadIdx.x))
+#define TT ((size_t)gridDim.x * blockDim.x)
+        const TraceArgs &T = A.T;
+        float b[3], k[NV], bn, hs, h = 0.f;
+        float acc[NV], accL, ys[NV];
+        {
+            float p0[3] = { y[0], y[1], y[2] };
+            if (phase >= 2) { p0[0] += st[(S3_DXT + 0) * TT]; p0[1] += st[(S3_DXT + 1) * TT]; p0[2] += st[(S3_DXT + 2) * TT]; }
+            enter_cell(A, p0);
+            stage(p0, y, b, k);
+            bn = norm3f_fast(b);
+            if (phase == 0) {
+                if (!(bn >= A.null_eps)) { finish(A, 255, nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL, -1); return true; }
+                if ((long long)nsteps >= T.max_steps || lam >= T.max_length) { finish(A, 255, REC_CAP, -1); return true; }
+                h = A.h_step;
+                if (lam + (double)h > T.max_length) h = (float)(T.max_length - lam);
+                hs = h;
+            } else {
+                float hp = st[S3_HP * TT];
+                if (phase == 1) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) st[(S3_K1 + c) * TT] = b[c];
+#pragma unroll
+                    for (int c = 3; c < NV; ++c) st[(S3_K1 + c) * TT] = k[c];
+                    st[S3_BN * TT] = bn;
+                } else {
+                    const int af = __float_as_int(st[S3_AXIS_FACE * TT]);
+                    const int axis = af >> 8, fc = af & 255;
+                    const float hfull = st[S3_HFULL * TT];
+                    const float bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
+                    const float xd = axis == 0 ? p0[0] : (axis == 1 ? p0[1] : p0[2]);
+                    const float gg = back ? -bd : bd, r = xd - face_offset(A, axis, (fc & 1) != 0);
+                    if (gg != 0.f) {
+                        const float hn = hp - r / gg;
+                        if (hn == hn) hp = fminf(fmaxf(hn, 0.f), hfull);
+                    }
+                    st[S3_HP * TT] = hp;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) b[c] = st[(S3_K1 + c) * TT];
+#pragma unroll
+                    for (int c = 3; c < NV; ++c) k[c] = st[(S3_K1 + c) * TT];
+                    bn = st[S3_BN * TT];
+                }
+                hs = hp;
+            }
+        }
+        const float shs = back ? -hs : hs;
+        if (T.method == QSL_EULER) {
+#pragma unroll
+            for (int c = 0; c < NV; ++c) ys[c] = fmaf(shs, c < 3 ? b[c] : k[c], y[c]);
+            enter_cell(A, ys);
+            accL = hs * bn;
+        } else {
+            const float half = 0.5f * shs;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ys[c] = fmaf(half, b[c], y[c]);
+            enter_cell(A, ys);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fmaf(half, k[c], y[c]); }
+            accL = bn;
+            // ---- stage 2
+            stage(ys, ys, b, k);
+            {
+                float xn[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) xn[c] = fmaf(half, b[c], y[c]);
+                enter_cell(A, xn);
+                bn = norm3f_fast(b);
+#pragma unroll
+                for (int c = 0; c < NV; ++c) {
+                    const float kc = c < 3 ? b[c] : k[c];
+                    acc[c] = fmaf(2.f, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fmaf(half, kc, y[c]);
+                }
+                accL = fmaf(2.f, bn, accL);
+            }
+            // ---- stage 3
+            stage(ys, ys, b, k);
+            {
+                float xn[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) xn[c] = fmaf(shs, b[c], y[c]);
+                enter_cell(A, xn);
+                bn = norm3f_fast(b);
+#pragma unroll
+                for (int c = 0; c < NV; ++c) {
+                    const float kc = c < 3 ? b[c] : k[c];
+                    acc[c] = fmaf(2.f, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fmaf(shs, kc, y[c]);
+                }
+                accL = fmaf(2.f, bn, accL);
+            }
+            // ---- stage 4
+            stage(ys, ys, b, k);
+            {
+                const float fL = hs * (1.0f / 6.0f), f = back ? -fL : fL;
+                float xn[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) xn[c] = fmaf(f, b[c] + acc[c], y[c]);
+                enter_cell(A, xn);             // the trial end is where the next attempt starts if it is accepted
+                bn = norm3f_fast(b);
+#pragma unroll
+                for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fmaf(f, k[c] + acc[c], y[c]);
+                accL = fL * (bn + accL);
+            }
+        }
+        // ys = trial end (offsets in the current frame), accL = length of the trial step
+        if (phase == 0) {
+            if (inside3(A, ys)) {
+#pragma unroll
+                for (int c = 0; c < NV; ++c) y[c] = ys[c];
+                L += (double)accL; lam += (double)h; ++nsteps;
+                return false;
+            }
+            // first face crossed by the chord: smallest fraction, tie -> lowest axis, then low face (reading A4)
+            float phi = INFINITY; int ax = -1, fc = 255; float bd = 0.f;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const bool lo_v = C[d] < A.cl[d] || (C[d] == A.cl[d] && ys[d] < A.off_lo[d]);
+                const bool hi_v = C[d] > A.ch[d] || (C[d] == A.ch[d] && ys[d] > A.off_hi[d]);
+                if (lo_v || hi_v) {
+                    const float fo = face_offset(A, d, !lo_v);
+                    const float f = (fo - y[d]) / (ys[d] - y[d]);
+                    if (f < phi) { phi = f; ax = d; fc = 2 * d + (lo_v ? 0 : 1); bd = fo; }
+                }
+            }
+            if (ax < 0) { finish(A, 255, REC_STALL, -1); return true; }   // non-finite trial point
+            const float yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
+            if (yd == bd) {
+                // the line starts on the face it leaves through: the landing of O4 is one zero-length step
+                ++nsteps;
+                finish(A, fc, 0, ax);
+                return true;
+            }
+            st[S3_HP * TT] = phi * h; st[S3_HFULL * TT] = h;
+            st[S3_AXIS_FACE * TT] = __int_as_float((ax << 8) | fc);
+            phase = 1;
+            return false;
+        }
+        if (phase < 4) {
+            st[(S3_DXT + 0) * TT] = ys[0] - y[0]; st[(S3_DXT + 1) * TT] = ys[1] - y[1]; st[(S3_DXT + 2) * TT] = ys[2] - y[2];
+            ++phase;
+            return false;
+        }
+        // phase 4: final landing step
+        const int af = __float_as_int(st[S3_AXIS_FACE * TT]);
+#pragma unroll
+        for (int c = 0; c < NV; ++c) y[c] = ys[c];
+        L += (double)accL; lam += (double)st[S3_HP * TT]; ++nsteps;
+        finish(A, af & 255, 0, af >> 8);
+        return true;
+#undef st
+#undef TT
+    }
+};
+
+// O2 (PAPER.md:160 eq. 9, :163; reading A7) in fp64 from the packed fp32 node samples, one thread per seed in sorted
+// order: (a^, b^) = 6 doubles per seed for LineState3::init.  Done once per line, so it is not worth an fp32 variant.
+template <bool INTERP>
+__global__ void __launch_bounds__(128) seed_basis3_kernel(const TraceArgs A, double *__restrict__ basis)
+{
+    const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= A.n) return;
+    const uint32_t si = A.perm[pos];
+    const double x[3] = { A.seeds[3 * (size_t)si], A.seeds[3 * (size_t)si + 1], A.seeds[3 * (size_t)si + 2] };
+    double o[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
+    if (inside_box(A, x)) {
+        double b[3], J[9], m, hmin;
+        evaluate<float, false, INTERP, false, false>(A, x, b, J, m, hmin);
+        const double inv = 1.0 / norm3(b);
+        const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
+        int e = 0;
+        if (fabs(u[1]) < fabs(u[e])) e = 1;
+        if (fabs(u[2]) < fabs(u[e == 1 ? 1 : 0])) e = 2;
+        const double ue = e == 0 ? u[0] : (e == 1 ? u[1] : u[2]);
+        double av[3] = { -u[0] * ue, -u[1] * ue, -u[2] * ue };
+        if (e == 0) av[0] += 1.0; else if (e == 1) av[1] += 1.0; else av[2] += 1.0;
+        const double ia = 1.0 / norm3(av);
+        av[0] *= ia; av[1] *= ia; av[2] *= ia;
+        o[0] = av[0]; o[1] = av[1]; o[2] = av[2];
+        o[3] = u[1] * av[2] - u[2] * av[1];
+        o[4] = u[2] * av[0] - u[0] * av[2];
+        o[5] = u[0] * av[1] - u[1] * av[0];
+    }
+    double2 *w = reinterpret_cast<double2 *>(basis + 6 * (size_t)pos);
+    w[0] = make_double2(o[0], o[1]); w[1] = make_double2(o[2], o[3]); w[2] = make_double2(o[4], o[5]);
+}
+
+#ifndef QSL_T3_THREADS
+#define QSL_T3_THREADS 128
+#endif
+#ifndef QSL_T3_MIN_BLOCKS_LQ
+#define QSL_T3_MIN_BLOCKS_LQ 5
+#endif
+#ifndef QSL_T3_MIN_BLOCKS_L
+#define QSL_T3_MIN_BLOCKS_L 8
+#endif
+// Persistent grid, work items (one direction of one line) popped from a global counter with a warp-aggregated atomic; a
+// lane whose line ended refills at once (same queue as trace2_kernel).
+template <bool DEV, bool INTERP, bool REFILL>
+__global__ void __launch_bounds__(QSL_T3_THREADS, DEV ? QSL_T3_MIN_BLOCKS_LQ : QSL_T3_MIN_BLOCKS_L) trace3_kernel(const Trace3Args A)
+{
+    LineState3<DEV, INTERP> ls;
+    const long long n_items = 2 * A.T.n;
+    unsigned long long my_steps = 0;
+    if (!REFILL) {
+        const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        if (q < n_items) {
+            ls.nsteps = 0;
+            if (ls.init(A, q)) { while (!ls.advance(A)) {} }
+            my_steps = ls.nsteps;
+        }
+    } else {
+        const unsigned lane = threadIdx.x & 31u;
+        bool have = false, drained = false;
+        while (true) {
+            if (!have && !drained) {
+                const unsigned m = __activemask();
+                const int leader = __ffs(m) - 1;
+                unsigned long long base = 0;
+                if ((int)lane == leader) base = atomicAdd(A.T.queue, (unsigned long long)__popc(m));
+                base = __shfl_sync(m, base, leader);
+                const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
+                if (q >= n_items) drained = true;
+                else have = ls.init(A, q);
+            }
+            if (__all_sync(0xffffffffu, drained && !have)) break;
+            if (have) {
+                if (ls.advance(A)) { my_steps += ls.nsteps; have = false; }
+            }
+        }
+    }
+    if (A.T.total_steps) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) my_steps += __shfl_xor_sync(0xffffffffu, my_steps, o);
+        if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(A.T.total_steps, my_steps);
+    }
+}
+
+}  // namespace qsl
