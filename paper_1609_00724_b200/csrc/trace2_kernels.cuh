@@ -21,15 +21,15 @@ __device__ __forceinline__ double4 load_cell4(const double4 *p)
     return r;
 }
 
-// |v| for the length integrand (reading A3) and the stall test: hardware reciprocal-square-root seed and one coupled
-// Newton step (relative error ~1e-13, five orders below the parity gate on L) instead of the IEEE sqrt sequence with its
-// fix-up branch; arguments outside [2^-767, 2^769) (zero, subnormal, huge, NaN) take the exact path.
+// |v| for the length integrand (reading A3) and the stall test, branch-free: hardware reciprocal-square-root seed of
+// max(|v|^2, 2^-600) and one coupled Newton step (relative error ~1e-13, five orders below the parity gate on L) instead
+// of the IEEE sqrt sequence with its fix-up branch.  |v|^2 = 0 gives exactly 0, NaN and overflow propagate (the stall
+// test then ends the line); |v| < 2^-300 comes out too small by at most 2^-300, far below any stall threshold.
 __device__ __forceinline__ double norm3_fast(const double v[3])
 {
     const double n2 = fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0]));
-    if ((unsigned)(__double2hiint(n2) - 0x10000000) >= 0x60000000u) return sqrt(n2);
     double r;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(n2));
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(fmax(n2, 0x1p-600)));
     const double s = n2 * r, hr = 0.5 * r;
     const double e = fma(-s, hr, 0.5);                 // 0.5 (1 - n2 r^2)
     const double s1 = fma(s, e, s), h1 = fma(hr, e, hr);

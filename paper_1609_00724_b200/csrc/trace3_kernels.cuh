@@ -33,13 +33,13 @@ struct Trace3Args {
 
 enum { S3_K1 = 0, S3_BN = 9, S3_DXT = 10, S3_HP = 13, S3_HFULL = 14, S3_AXIS_FACE = 15, STASH3_FLOATS = 16 };
 
-// |v| in fp32: hardware reciprocal square root and one Newton step (relative error ~1e-7); zero, subnormal, huge and
-// NaN arguments take the IEEE path.
+// |v| in fp32, branch-free: hardware reciprocal square root of max(|v|^2, 2^-100) and one Newton step (relative error
+// ~1e-7).  |v|^2 = 0 gives exactly 0; NaN and overflow propagate (and then stop the line through the stall test);
+// |v| below 2^-50 comes out too small by up to 2^-50, far under any stall threshold.
 __device__ __forceinline__ float norm3f_fast(const float v[3])
 {
     const float n2 = fmaf(v[2], v[2], fmaf(v[1], v[1], v[0] * v[0]));
-    if ((unsigned)(__float_as_int(n2) - 0x10000000) >= 0x60000000u) return sqrtf(n2);
-    const float r = rsqrtf(n2);
+    const float r = rsqrtf(fmaxf(n2, 7.8886e-31f));
     const float s = n2 * r;
     return fmaf(fmaf(-s, s, n2), 0.5f * r, s);
 }
@@ -73,19 +73,16 @@ struct LineState3 {
     {
         const unsigned u0 = (unsigned)__float_as_int(p[0]), u1 = (unsigned)__float_as_int(p[1]), u2 = (unsigned)__float_as_int(p[2]);
         if (!(u0 < (unsigned)__float_as_int(A.hf[0]) && u1 < (unsigned)__float_as_int(A.hf[1]) && u2 < (unsigned)__float_as_int(A.hf[2]))) {
-            int s[3];
+            // one level of divergence: a lane that is only extrapolating beyond the edge of the grid (no neighbour to
+            // step to) reloads the cell it already has
 #pragma unroll
-            for (int d = 0; d < 3; ++d)
-                s[d] = p[d] < 0.f ? (C[d] > 0 ? -1 : 0) : (p[d] >= A.hf[d] ? (C[d] < A.cmax[d] ? 1 : 0) : 0);
-            if (s[0] | s[1] | s[2]) {
-#pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    C[d] += s[d];
-                    const float sh = (float)s[d] * A.hf[d];
-                    p[d] -= sh; y[d] -= sh;
-                }
-                load_cell(A);
+            for (int d = 0; d < 3; ++d) {
+                const bool dn = p[d] < 0.f && C[d] > 0, up = p[d] >= A.hf[d] && C[d] < A.cmax[d];
+                C[d] += up ? 1 : (dn ? -1 : 0);
+                const float sh = up ? A.hf[d] : (dn ? -A.hf[d] : 0.f);
+                p[d] -= sh; y[d] -= sh;
             }
+            load_cell(A);
         }
     }
 
