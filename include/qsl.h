@@ -55,6 +55,8 @@ enum { QSL_ARITH_F64 = 0, QSL_ARITH_F32 = 1 };           /* arithmetic of the in
 #define QSL_FLAG_NO_SORT    1u    /* do not Morton-order the seeds before tracing                                  */
 #define QSL_FLAG_NO_REFILL  2u    /* one work item per thread instead of the persistent work queue                 */
 #define QSL_FLAG_KERNEL_V1  4u    /* corner kernel: 8 AoS sample gathers per RK stage instead of the per-cell table  */
+#define QSL_FLAG_KERNEL_FRAME 8u  /* fp64 on a uniform grid: the cell-frame kernel (integer cell index + offset, the
+                                     design of the fp32 kernel) instead of the absolute-coordinate cell-table kernel  */
 
 /* ---- field (PAPER.md:54 input cubes; :93-107 eq. 3-4 interpolation; :178 normalise-then-interpolate) --------- */
 typedef struct qsl_field qsl_field;          /* opaque, library-owned */

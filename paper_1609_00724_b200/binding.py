@@ -22,7 +22,7 @@ QSL_ARITH_F64, QSL_ARITH_F32 = 0, 1
 QSL_LAYOUT_CELL_TABLE, QSL_LAYOUT_NODES_ONLY, QSL_LAYOUT_CELL_TABLE_F32, QSL_LAYOUT_CELL_TABLES_BOTH = 0, 1, 2, 3
 QSL_ST_SEED_OUTSIDE, QSL_ST_NULL_AT_SEED, QSL_ST_STALL_F, QSL_ST_STALL_B = 1, 2, 4, 8
 QSL_ST_CAP_F, QSL_ST_CAP_B, QSL_ST_OPEN = 16, 32, 64
-QSL_FLAG_NO_SORT, QSL_FLAG_NO_REFILL, QSL_FLAG_KERNEL_V1 = 1, 2, 4
+QSL_FLAG_NO_SORT, QSL_FLAG_NO_REFILL, QSL_FLAG_KERNEL_V1, QSL_FLAG_KERNEL_FRAME = 1, 2, 4, 8
 
 _dp = C.POINTER(C.c_double)
 

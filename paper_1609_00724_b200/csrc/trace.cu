@@ -10,6 +10,7 @@ cudaError_t launch_trace_f32(const TraceArgs &A, bool dev, bool refill, cudaStre
 cudaError_t launch_trace_f64(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 int launch_trace2(TraceArgs &A, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 int launch_trace3(const TraceArgs &T, const void *cells32, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
+int launch_trace3_f64(const TraceArgs &T, bool samples_f32, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 cudaError_t launch_epilogue_f32(const EpilogueArgs &E, cudaStream_t s);
 cudaError_t launch_epilogue_f64(const EpilogueArgs &E, cudaStream_t s);
 }  // namespace qsl
@@ -103,6 +104,9 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         if (e == cudaSuccess && p->arith == QSL_ARITH_F32) {
             const int ps = prof_slot(p->mode);
             rc = launch_trace3(A, f->d_cells32, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
+        } else if (e == cudaSuccess && v2 && !f->view.stretched && (p->flags & QSL_FLAG_KERNEL_FRAME)) {
+            const int ps = prof_slot(p->mode);
+            rc = launch_trace3_f64(A, f->sample_type == QSL_F32, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
         } else if (e == cudaSuccess && v2) {
             // the cell-table kernel allocates its own scratch and brackets its launch with the profiling events
             const int ps = prof_slot(p->mode);

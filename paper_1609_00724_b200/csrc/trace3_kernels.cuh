@@ -17,50 +17,84 @@
 
 namespace qsl {
 
+// Scalar-type traits of the kernel: T = float (QSL_ARITH_F32, 96 B table entries) or double (the fp64 table).
+template <typename T> struct Real3;
+template <> struct Real3<float> {
+    using V4 = float4;
+    static __device__ __forceinline__ float4 load(const float4 *p) { return __ldg(p); }
+    // bit pattern for the "0 <= p < h" test (one unsigned compare per axis): exact in fp32
+    static __device__ __forceinline__ unsigned bits(float v) { return (unsigned)__float_as_int(v); }
+    static __device__ __forceinline__ float rsqrt_seed(float n2) { return rsqrtf(fmaxf(n2, 7.8886e-31f)); }
+};
+template <> struct Real3<double> {
+    using V4 = double4;
+    static __device__ __forceinline__ double4 load(const double4 *p)
+    {
+        double4 r;   // one 256-bit LDG (sm_100)
+        asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+        return r;
+    }
+    // high word only: sufficient, not necessary (false for p within 2^-20 relative below h: a redundant reload)
+    static __device__ __forceinline__ unsigned bits(double v) { return (unsigned)__double2hiint(v); }
+    static __device__ __forceinline__ double rsqrt_seed(double n2)
+    {
+        double r;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(fmax(n2, 0x1p-600)));
+        return r;
+    }
+};
+
+template <typename T>
 struct Trace3Args {
-    TraceArgs T;
-    const float4 *cells32;       // 6 float4 per cell: monomial coefficients a[8 c + m] of the trilinear interpolant
-    float hf[3];                 // cell edges
-    float h_step;                // step_frac * min_d h_d
+    TraceArgs T0;                // the arguments of qsl_trace common to all kernels
+    const typename Real3<T>::V4 *cells;   // 6 V4 per cell: monomial coefficients a[8 c + m] of the trilinear interpolant
+    T hf[3];                     // cell edges
+    unsigned hbits[3];           // Real3<T>::bits(hf)
+    T h_step;                    // step_frac * min_d h_d
     int cmax[3];                 // n_d - 2: last cell index per axis
     int cell_sy, cell_sz;        // table strides in cells
     int cl[3], ch[3];            // cells containing box_lo / box_hi (box_hi on a node belongs to the cell below it)
     unsigned cw[3];              // max(ch - cl - 1, 0): number of cells strictly between them
-    float off_lo[3], off_hi[3];  // offsets of box_lo / box_hi from the origins of cells cl / ch
-    float null_eps;
-    float *stash;                // per-thread landing scratch, STASH3_FLOATS x n_threads
+    T off_lo[3], off_hi[3];      // offsets of box_lo / box_hi from the origins of cells cl / ch
+    T null_eps;
+    T *stash;                    // per-thread landing scratch, STASH3_SLOTS x n_threads
 };
 
-enum { S3_K1 = 0, S3_BN = 9, S3_DXT = 10, S3_HP = 13, S3_HFULL = 14, S3_AXIS_FACE = 15, STASH3_FLOATS = 16 };
+enum { S3_K1 = 0, S3_BN = 9, S3_DXT = 10, S3_HP = 13, S3_HFULL = 14, S3_AXIS_FACE = 15, STASH3_SLOTS = 16 };
 
-// |v| in fp32, branch-free: hardware reciprocal square root of max(|v|^2, 2^-100) and one Newton step (relative error
-// ~1e-7).  |v|^2 = 0 gives exactly 0; NaN and overflow propagate (and then stop the line through the stall test);
-// |v| below 2^-50 comes out too small by up to 2^-50, far under any stall threshold.
-__device__ __forceinline__ float norm3f_fast(const float v[3])
+// |v|, branch-free: hardware reciprocal square root of max(|v|^2, tiny) and one coupled Newton step (relative error
+// ~1e-7 in fp32, ~1e-13 in fp64).  |v|^2 = 0 gives exactly 0; NaN and overflow propagate (and then stop the line through
+// the stall test); |v| below 2^-50 (fp32) / 2^-300 (fp64) comes out too small, far under any stall threshold.
+template <typename T>
+__device__ __forceinline__ T norm3r_fast(const T v[3])
 {
-    const float n2 = fmaf(v[2], v[2], fmaf(v[1], v[1], v[0] * v[0]));
-    const float r = rsqrtf(fmaxf(n2, 7.8886e-31f));
-    const float s = n2 * r;
-    return fmaf(fmaf(-s, s, n2), 0.5f * r, s);
+    const T n2 = fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0]));
+    const T r = Real3<T>::rsqrt_seed(n2);
+    const T s = n2 * r, hr = T(0.5) * r;
+    if (sizeof(T) == 4) return fma(fma(-s, s, n2), hr, s);
+    const T e = fma(-s, hr, T(0.5));                   // 0.5 (1 - n2 r^2)
+    const T s1 = fma(s, e, s), h1 = fma(hr, e, hr);
+    return fma(fma(-s1, s1, n2), h1, s1);
 }
 
-template <bool DEV, bool INTERP>
+template <typename T, bool DEV, bool INTERP>
 struct LineState3 {
+    using Args = Trace3Args<T>;
     static constexpr int NV = DEV ? 9 : 3;
-    float a[24];             // cached cell: monomial coefficients
+    T a[24];             // cached cell: monomial coefficients
     int C[3];                // its index = the frame of every offset below
-    float y[NV];             // y[0..2]: offset of the line's point from the origin of cell C; delta1, delta2
+    T y[NV];             // y[0..2]: offset of the line's point from the origin of cell C; delta1, delta2
     double L, lam;
     uint32_t nsteps, slot;
     int phase;
     bool back;
 
-    __device__ __forceinline__ void load_cell(const Trace3Args &A)
+    __device__ __forceinline__ void load_cell(const Args &A)
     {
-        const float4 *__restrict__ p = A.cells32 + ((size_t)((unsigned)C[2] * (unsigned)A.cell_sz + (unsigned)C[1] * (unsigned)A.cell_sy + (unsigned)C[0])) * 6;
+        const typename Real3<T>::V4 *__restrict__ p = A.cells + ((size_t)((unsigned)C[2] * (unsigned)A.cell_sz + (unsigned)C[1] * (unsigned)A.cell_sy + (unsigned)C[0])) * 6;
 #pragma unroll
         for (int q = 0; q < 6; ++q) {
-            const float4 v = __ldg(p + q);
+            const typename Real3<T>::V4 v = Real3<T>::load(p + q);
             a[4 * q] = v.x; a[4 * q + 1] = v.y; a[4 * q + 2] = v.z; a[4 * q + 3] = v.w;
         }
     }
@@ -69,17 +103,16 @@ struct LineState3 {
     // the offset is not) by a neighbour step per axis, and moves the frame of p and of the line's own point with it.
     // Consecutive evaluation points are at most half a cell apart (|b| <= 1, h = step_frac cell), so one step suffices.
     // The "still inside" test is one unsigned compare per axis on the bit pattern: 0 <= p < h.
-    __device__ __forceinline__ void enter_cell(const Trace3Args &A, float p[3])
+    __device__ __forceinline__ void enter_cell(const Args &A, T p[3])
     {
-        const unsigned u0 = (unsigned)__float_as_int(p[0]), u1 = (unsigned)__float_as_int(p[1]), u2 = (unsigned)__float_as_int(p[2]);
-        if (!(u0 < (unsigned)__float_as_int(A.hf[0]) && u1 < (unsigned)__float_as_int(A.hf[1]) && u2 < (unsigned)__float_as_int(A.hf[2]))) {
+        if (!(Real3<T>::bits(p[0]) < A.hbits[0] && Real3<T>::bits(p[1]) < A.hbits[1] && Real3<T>::bits(p[2]) < A.hbits[2])) {
             // one level of divergence: a lane that is only extrapolating beyond the edge of the grid (no neighbour to
             // step to) reloads the cell it already has
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                const bool dn = p[d] < 0.f && C[d] > 0, up = p[d] >= A.hf[d] && C[d] < A.cmax[d];
+                const bool dn = p[d] < T(0.) && C[d] > 0, up = p[d] >= A.hf[d] && C[d] < A.cmax[d];
                 C[d] += up ? 1 : (dn ? -1 : 0);
-                const float sh = up ? A.hf[d] : (dn ? -A.hf[d] : 0.f);
+                const T sh = up ? A.hf[d] : (dn ? -A.hf[d] : T(0.));
                 p[d] -= sh; y[d] -= sh;
             }
             load_cell(A);
@@ -87,42 +120,43 @@ struct LineState3 {
     }
 
     // Field evaluation at offsets d inside the cached cell fused with the deviation products (as LineState2::stage).
-    __device__ __forceinline__ void stage(const float d[3], const float *ys, float b[3], float *k)
+    __device__ __forceinline__ void stage(const T d[3], const T *ys, T b[3], T *k)
     {
-        const float dx = d[0], dy = d[1], dz = d[2];
-        float v[3], g[9];
+        const T dx = d[0], dy = d[1], dz = d[2];
+        T v[3], g[9];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const float *q = a + 8 * c;
-            const float P = fmaf(q[7], dz, q[3]), Q = fmaf(q[5], dz, q[1]), R = fmaf(q[6], dz, q[2]), S = fmaf(q[4], dz, q[0]);
-            const float E = fmaf(P, dy, Q), F = fmaf(R, dy, S);
-            v[c] = fmaf(E, dx, F);
+            const T *q = a + 8 * c;
+            const T P = fma(q[7], dz, q[3]), Q = fma(q[5], dz, q[1]), R = fma(q[6], dz, q[2]), S = fma(q[4], dz, q[0]);
+            const T E = fma(P, dy, Q), F = fma(R, dy, S);
+            v[c] = fma(E, dx, F);
             if (DEV || INTERP) {
                 g[3 * c] = E;
-                g[3 * c + 1] = fmaf(P, dx, R);
-                g[3 * c + 2] = fmaf(fmaf(q[7], dy, q[5]), dx, fmaf(q[6], dy, q[4]));
+                g[3 * c + 1] = fma(P, dx, R);
+                g[3 * c + 2] = fma(fma(q[7], dy, q[5]), dx, fma(q[6], dy, q[4]));
             }
         }
         if (!INTERP) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) b[c] = v[c];
-        } else {
+        } else
+        {
             // reading A2: b = B/|B|, J = (G - u (u^T G))/|B|
-            const float nn = sqrtf(fmaf(v[2], v[2], fmaf(v[1], v[1], v[0] * v[0])));
-            if (nn < 1e-37f) {
+            const T nn = sqrt(fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0])));
+            if (nn < (sizeof(T) == 4 ? T(1e-37) : T(1e-300))) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) b[c] = 0.f;
+                for (int c = 0; c < 3; ++c) b[c] = T(0.);
 #pragma unroll
-                for (int q = 0; q < 9; ++q) g[q] = 0.f;
+                for (int q = 0; q < 9; ++q) g[q] = T(0.);
             } else {
-                const float inv = 1.0f / nn;
-                const float u[3] = { v[0] * inv, v[1] * inv, v[2] * inv };
+                const T inv = T(1.0) / nn;
+                const T u[3] = { v[0] * inv, v[1] * inv, v[2] * inv };
 #pragma unroll
                 for (int c = 0; c < 3; ++c) b[c] = u[c];
                 if (DEV) {
 #pragma unroll
                     for (int e = 0; e < 3; ++e) {
-                        const float uG = fmaf(u[2], g[6 + e], fmaf(u[1], g[3 + e], u[0] * g[e]));
+                        const T uG = fma(u[2], g[6 + e], fma(u[1], g[3 + e], u[0] * g[e]));
 #pragma unroll
                         for (int c = 0; c < 3; ++c) g[3 * c + e] = (g[3 * c + e] - u[c] * uG) * inv;
                     }
@@ -134,47 +168,47 @@ struct LineState3 {
             for (int w = 0; w < 2; ++w)
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
-                    k[(3 + 3 * w + c) % NV] = fmaf(g[3 * c + 2], ys[(5 + 3 * w) % NV], fmaf(g[3 * c + 1], ys[(4 + 3 * w) % NV], g[3 * c] * ys[(3 + 3 * w) % NV]));
+                    k[(3 + 3 * w + c) % NV] = fma(g[3 * c + 2], ys[(5 + 3 * w) % NV], fma(g[3 * c + 1], ys[(4 + 3 * w) % NV], g[3 * c] * ys[(3 + 3 * w) % NV]));
         }
     }
 
     // Starts work item q (false if it ended at once: seed outside the trace box).  The seed's cell is found once, in
     // fp64, exactly as O1 does (floor of (x - lo)/h, clamped); the basis a^, b^ of O2 comes from seed_basis3_kernel.
-    __device__ bool init(const Trace3Args &A, long long q)
+    __device__ bool init(const Args &A, long long q)
     {
-        const TraceArgs &T = A.T;
+        const TraceArgs &G = A.T0;
         long long pos; int dir;
-        if (T.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= T.n ? 1 : 0; pos = q - (long long)dir * T.n; }
-        slot = (uint32_t)((long long)dir * T.n + pos);
+        if (G.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= G.n ? 1 : 0; pos = q - (long long)dir * G.n; }
+        slot = (uint32_t)((long long)dir * G.n + pos);
         back = dir != 0;
-        const uint32_t si = T.perm[pos];
-        const double x[3] = { T.seeds[3 * (size_t)si], T.seeds[3 * (size_t)si + 1], T.seeds[3 * (size_t)si + 2] };
+        const uint32_t si = G.perm[pos];
+        const double x[3] = { G.seeds[3 * (size_t)si], G.seeds[3 * (size_t)si + 1], G.seeds[3 * (size_t)si + 2] };
         L = 0.0; lam = 0.0; nsteps = 0; phase = 0;
-        if (!inside_box(T, x)) {
+        if (!inside_box(G, x)) {
             double out[REC_DOUBLES];
 #pragma unroll
             for (int c = 0; c < REC_DOUBLES; ++c) out[c] = c < 3 ? x[c] : 0.0;
             out[10] = __hiloint2double((int)(255u | REC_SEED_OUTSIDE), 0);
-            double2 *r2 = reinterpret_cast<double2 *>(T.rec + (size_t)slot * REC_DOUBLES);
+            double2 *r2 = reinterpret_cast<double2 *>(G.rec + (size_t)slot * REC_DOUBLES);
 #pragma unroll
             for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
             return false;
         }
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            const double u = (x[d] - T.fv.lo[d]) * T.inv_h[d];
+            const double u = (x[d] - G.fv.lo[d]) * G.inv_h[d];
             int i = (int)floor(u);
             i = max(0, min(i, A.cmax[d]));
             C[d] = i;
-            y[d] = (float)(x[d] - fma((double)i, T.fv.h[d], T.fv.lo[d]));
+            y[d] = (T)(x[d] - fma((double)i, G.fv.h[d], G.fv.lo[d]));
         }
 #pragma unroll
-        for (int c = 3; c < NV; ++c) y[c] = 0.f;
+        for (int c = 3; c < NV; ++c) y[c] = T(0.);
         if (DEV) {
-            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(T.basis + 6 * (size_t)pos);
+            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(G.basis + 6 * (size_t)pos);
             const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
-            y[3 % NV] = (float)b0.x; y[4 % NV] = (float)b0.y; y[5 % NV] = (float)b1.x;
-            y[6 % NV] = (float)b1.y; y[7 % NV] = (float)b2.x; y[8 % NV] = (float)b2.y;
+            y[3 % NV] = (T)b0.x; y[4 % NV] = (T)b0.y; y[5 % NV] = (T)b1.x;
+            y[6 % NV] = (T)b1.y; y[7 % NV] = (T)b2.x; y[8 % NV] = (T)b2.y;
         }
         load_cell(A);
         return true;
@@ -182,15 +216,15 @@ struct LineState3 {
 
     // Writes the per-direction record in fp64: position = origin of the frame cell + offset; `snap` >= 0 puts the
     // coordinate of that axis exactly on the face it landed on.
-    __device__ void finish(const Trace3Args &A, int face, uint32_t flags, int snap)
+    __device__ void finish(const Args &A, int face, uint32_t flags, int snap)
     {
-        const TraceArgs &T = A.T;
+        const TraceArgs &G = A.T0;
         double out[REC_DOUBLES];
 #pragma unroll
-        for (int d = 0; d < 3; ++d) out[d] = fma((double)C[d], T.fv.h[d], T.fv.lo[d]) + (double)y[d];
+        for (int d = 0; d < 3; ++d) out[d] = fma((double)C[d], G.fv.h[d], G.fv.lo[d]) + (double)y[d];
         if (snap >= 0) {
-            const double bd = (face & 1) ? (snap == 0 ? T.box_hi[0] : (snap == 1 ? T.box_hi[1] : T.box_hi[2]))
-                                         : (snap == 0 ? T.box_lo[0] : (snap == 1 ? T.box_lo[1] : T.box_lo[2]));
+            const double bd = (face & 1) ? (snap == 0 ? G.box_hi[0] : (snap == 1 ? G.box_hi[1] : G.box_hi[2]))
+                                         : (snap == 0 ? G.box_lo[0] : (snap == 1 ? G.box_lo[1] : G.box_lo[2]));
             if (snap == 0) out[0] = bd; else if (snap == 1) out[1] = bd; else out[2] = bd;
         }
 #pragma unroll
@@ -198,25 +232,25 @@ struct LineState3 {
         out[9] = L;
         out[10] = __hiloint2double((int)((uint32_t)face | flags), (int)nsteps);
         out[11] = lam;
-        double2 *r2 = reinterpret_cast<double2 *>(T.rec + (size_t)slot * REC_DOUBLES);
+        double2 *r2 = reinterpret_cast<double2 *>(G.rec + (size_t)slot * REC_DOUBLES);
 #pragma unroll
         for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
     }
 
     // Offset, in the current frame, of the face (axis, upper?) of the trace box.
-    __device__ __forceinline__ float face_offset(const Trace3Args &A, int axis, bool upper) const
+    __device__ __forceinline__ T face_offset(const Args &A, int axis, bool upper) const
     {
         const int cd = axis == 0 ? C[0] : (axis == 1 ? C[1] : C[2]);
         const int cb = upper ? (axis == 0 ? A.ch[0] : (axis == 1 ? A.ch[1] : A.ch[2])) : (axis == 0 ? A.cl[0] : (axis == 1 ? A.cl[1] : A.cl[2]));
-        const float ob = upper ? (axis == 0 ? A.off_hi[0] : (axis == 1 ? A.off_hi[1] : A.off_hi[2]))
+        const T ob = upper ? (axis == 0 ? A.off_hi[0] : (axis == 1 ? A.off_hi[1] : A.off_hi[2]))
                                : (axis == 0 ? A.off_lo[0] : (axis == 1 ? A.off_lo[1] : A.off_lo[2]));
-        const float hd = axis == 0 ? A.hf[0] : (axis == 1 ? A.hf[1] : A.hf[2]);
-        return fmaf((float)(cb - cd), hd, ob);
+        const T hd = axis == 0 ? A.hf[0] : (axis == 1 ? A.hf[1] : A.hf[2]);
+        return fma((T)(cb - cd), hd, ob);
     }
 
     // Is the point at offsets e of the frame cell inside the closed trace box?  Cells strictly between the cells that
     // hold the faces of the box need one unsigned compare per axis; the others compare the offset with the face's.
-    __device__ __forceinline__ bool inside3(const Trace3Args &A, const float e[3]) const
+    __device__ __forceinline__ bool inside3(const Args &A, const T e[3]) const
     {
         if ((unsigned)(C[0] - A.cl[0] - 1) < A.cw[0] && (unsigned)(C[1] - A.cl[1] - 1) < A.cw[1] && (unsigned)(C[2] - A.cl[2] - 1) < A.cw[2])
             return true;
@@ -234,27 +268,27 @@ struct LineState3 {
     // LineState2::advance, reading A4): phase 0 trial step; phase 1 first landing step of size hp (k1 and the trial end,
     // as a displacement from y so that it survives a change of frame, go to the stash); phases 2..4 spend the first
     // evaluation at the previous trial end for one Newton update of hp; phase 4 lands.
-    __device__ bool advance(const Trace3Args &A)
+    __device__ bool advance(const Args &A)
     {
 #define st (A.stash + ((size_t)blockIdx.x * blockDim.x + threadIdx.x))
 #define TT ((size_t)gridDim.x * blockDim.x)
-        const TraceArgs &T = A.T;
-        float b[3], k[NV], bn, hs, h = 0.f;
-        float acc[NV], accL, ys[NV];
+        const TraceArgs &G = A.T0;
+        T b[3], k[NV], bn, hs, h = T(0.);
+        T acc[NV], accL, ys[NV];
         {
-            float p0[3] = { y[0], y[1], y[2] };
+            T p0[3] = { y[0], y[1], y[2] };
             if (phase >= 2) { p0[0] += st[(S3_DXT + 0) * TT]; p0[1] += st[(S3_DXT + 1) * TT]; p0[2] += st[(S3_DXT + 2) * TT]; }
             enter_cell(A, p0);
             stage(p0, y, b, k);
-            bn = norm3f_fast(b);
+            bn = norm3r_fast<T>(b);
             if (phase == 0) {
                 if (!(bn >= A.null_eps)) { finish(A, 255, nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL, -1); return true; }
-                if ((long long)nsteps >= T.max_steps || lam >= T.max_length) { finish(A, 255, REC_CAP, -1); return true; }
+                if ((long long)nsteps >= G.max_steps || lam >= G.max_length) { finish(A, 255, REC_CAP, -1); return true; }
                 h = A.h_step;
-                if (lam + (double)h > T.max_length) h = (float)(T.max_length - lam);
+                if (lam + (double)h > G.max_length) h = (T)(G.max_length - lam);
                 hs = h;
             } else {
-                float hp = st[S3_HP * TT];
+                T hp = st[S3_HP * TT];
                 if (phase == 1) {
 #pragma unroll
                     for (int c = 0; c < 3; ++c) st[(S3_K1 + c) * TT] = b[c];
@@ -262,15 +296,15 @@ struct LineState3 {
                     for (int c = 3; c < NV; ++c) st[(S3_K1 + c) * TT] = k[c];
                     st[S3_BN * TT] = bn;
                 } else {
-                    const int af = __float_as_int(st[S3_AXIS_FACE * TT]);
+                    const int af = (int)st[S3_AXIS_FACE * TT];
                     const int axis = af >> 8, fc = af & 255;
-                    const float hfull = st[S3_HFULL * TT];
-                    const float bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
-                    const float xd = axis == 0 ? p0[0] : (axis == 1 ? p0[1] : p0[2]);
-                    const float gg = back ? -bd : bd, r = xd - face_offset(A, axis, (fc & 1) != 0);
-                    if (gg != 0.f) {
-                        const float hn = hp - r / gg;
-                        if (hn == hn) hp = fminf(fmaxf(hn, 0.f), hfull);
+                    const T hfull = st[S3_HFULL * TT];
+                    const T bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
+                    const T xd = axis == 0 ? p0[0] : (axis == 1 ? p0[1] : p0[2]);
+                    const T gg = back ? -bd : bd, r = xd - face_offset(A, axis, (fc & 1) != 0);
+                    if (gg != T(0.)) {
+                        const T hn = hp - r / gg;
+                        if (hn == hn) hp = fmin(fmax(hn, T(0.)), hfull);
                     }
                     st[S3_HP * TT] = hp;
 #pragma unroll
@@ -282,61 +316,61 @@ struct LineState3 {
                 hs = hp;
             }
         }
-        const float shs = back ? -hs : hs;
-        if (T.method == QSL_EULER) {
+        const T shs = back ? -hs : hs;
+        if (G.method == QSL_EULER) {
 #pragma unroll
-            for (int c = 0; c < NV; ++c) ys[c] = fmaf(shs, c < 3 ? b[c] : k[c], y[c]);
+            for (int c = 0; c < NV; ++c) ys[c] = fma(shs, c < 3 ? b[c] : k[c], y[c]);
             enter_cell(A, ys);
             accL = hs * bn;
         } else {
-            const float half = 0.5f * shs;
+            const T half = T(0.5) * shs;
 #pragma unroll
-            for (int c = 0; c < 3; ++c) ys[c] = fmaf(half, b[c], y[c]);
+            for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
             enter_cell(A, ys);
 #pragma unroll
-            for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fmaf(half, k[c], y[c]); }
+            for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
             accL = bn;
             // ---- stage 2
             stage(ys, ys, b, k);
             {
-                float xn[3];
+                T xn[3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fmaf(half, b[c], y[c]);
+                for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
                 enter_cell(A, xn);
-                bn = norm3f_fast(b);
+                bn = norm3r_fast<T>(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) {
-                    const float kc = c < 3 ? b[c] : k[c];
-                    acc[c] = fmaf(2.f, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fmaf(half, kc, y[c]);
+                    const T kc = c < 3 ? b[c] : k[c];
+                    acc[c] = fma(T(2.), kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(half, kc, y[c]);
                 }
-                accL = fmaf(2.f, bn, accL);
+                accL = fma(T(2.), bn, accL);
             }
             // ---- stage 3
             stage(ys, ys, b, k);
             {
-                float xn[3];
+                T xn[3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fmaf(shs, b[c], y[c]);
+                for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
                 enter_cell(A, xn);
-                bn = norm3f_fast(b);
+                bn = norm3r_fast<T>(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) {
-                    const float kc = c < 3 ? b[c] : k[c];
-                    acc[c] = fmaf(2.f, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fmaf(shs, kc, y[c]);
+                    const T kc = c < 3 ? b[c] : k[c];
+                    acc[c] = fma(T(2.), kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(shs, kc, y[c]);
                 }
-                accL = fmaf(2.f, bn, accL);
+                accL = fma(T(2.), bn, accL);
             }
             // ---- stage 4
             stage(ys, ys, b, k);
             {
-                const float fL = hs * (1.0f / 6.0f), f = back ? -fL : fL;
-                float xn[3];
+                const T fL = hs * (T(1.0) / T(6.0)), f = back ? -fL : fL;
+                T xn[3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fmaf(f, b[c] + acc[c], y[c]);
+                for (int c = 0; c < 3; ++c) xn[c] = fma(f, b[c] + acc[c], y[c]);
                 enter_cell(A, xn);             // the trial end is where the next attempt starts if it is accepted
-                bn = norm3f_fast(b);
+                bn = norm3r_fast<T>(b);
 #pragma unroll
-                for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fmaf(f, k[c] + acc[c], y[c]);
+                for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, k[c] + acc[c], y[c]);
                 accL = fL * (bn + accL);
             }
         }
@@ -349,19 +383,19 @@ struct LineState3 {
                 return false;
             }
             // first face crossed by the chord: smallest fraction, tie -> lowest axis, then low face (reading A4)
-            float phi = INFINITY; int ax = -1, fc = 255; float bd = 0.f;
+            T phi = INFINITY; int ax = -1, fc = 255; T bd = T(0.);
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const bool lo_v = C[d] < A.cl[d] || (C[d] == A.cl[d] && ys[d] < A.off_lo[d]);
                 const bool hi_v = C[d] > A.ch[d] || (C[d] == A.ch[d] && ys[d] > A.off_hi[d]);
                 if (lo_v || hi_v) {
-                    const float fo = face_offset(A, d, !lo_v);
-                    const float f = (fo - y[d]) / (ys[d] - y[d]);
+                    const T fo = face_offset(A, d, !lo_v);
+                    const T f = (fo - y[d]) / (ys[d] - y[d]);
                     if (f < phi) { phi = f; ax = d; fc = 2 * d + (lo_v ? 0 : 1); bd = fo; }
                 }
             }
             if (ax < 0) { finish(A, 255, REC_STALL, -1); return true; }   // non-finite trial point
-            const float yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
+            const T yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
             if (yd == bd) {
                 // the line starts on the face it leaves through: the landing of O4 is one zero-length step
                 ++nsteps;
@@ -369,7 +403,7 @@ struct LineState3 {
                 return true;
             }
             st[S3_HP * TT] = phi * h; st[S3_HFULL * TT] = h;
-            st[S3_AXIS_FACE * TT] = __int_as_float((ax << 8) | fc);
+            st[S3_AXIS_FACE * TT] = (T)((ax << 8) | fc);
             phase = 1;
             return false;
         }
@@ -379,7 +413,7 @@ struct LineState3 {
             return false;
         }
         // phase 4: final landing step
-        const int af = __float_as_int(st[S3_AXIS_FACE * TT]);
+        const int af = (int)st[S3_AXIS_FACE * TT];
 #pragma unroll
         for (int c = 0; c < NV; ++c) y[c] = ys[c];
         L += (double)accL; lam += (double)st[S3_HP * TT]; ++nsteps;
@@ -390,9 +424,9 @@ struct LineState3 {
     }
 };
 
-// O2 (PAPER.md:160 eq. 9, :163; reading A7) in fp64 from the packed fp32 node samples, one thread per seed in sorted
-// order: (a^, b^) = 6 doubles per seed for LineState3::init.  Done once per line, so it is not worth an fp32 variant.
-template <bool INTERP>
+// O2 (PAPER.md:160 eq. 9, :163; reading A7) in fp64 from the packed node samples (S = their storage type), one thread per
+// seed in sorted order: (a^, b^) = 6 doubles per seed for LineState3::init.  Once per line: not worth an fp32 variant.
+template <typename S, bool INTERP>
 __global__ void __launch_bounds__(128) seed_basis3_kernel(const TraceArgs A, double *__restrict__ basis)
 {
     const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -402,7 +436,7 @@ __global__ void __launch_bounds__(128) seed_basis3_kernel(const TraceArgs A, dou
     double o[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
     if (inside_box(A, x)) {
         double b[3], J[9], m, hmin;
-        evaluate<float, false, INTERP, false, false>(A, x, b, J, m, hmin);
+        evaluate<S, false, INTERP, false, false>(A, x, b, J, m, hmin);
         const double inv = 1.0 / norm3(b);
         const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
         int e = 0;
@@ -431,13 +465,21 @@ __global__ void __launch_bounds__(128) seed_basis3_kernel(const TraceArgs A, dou
 #ifndef QSL_T3_MIN_BLOCKS_L
 #define QSL_T3_MIN_BLOCKS_L 8
 #endif
+#ifndef QSL_T3_MIN_BLOCKS_LQ64
+#define QSL_T3_MIN_BLOCKS_LQ64 3
+#endif
+#ifndef QSL_T3_MIN_BLOCKS_L64
+#define QSL_T3_MIN_BLOCKS_L64 4
+#endif
 // Persistent grid, work items (one direction of one line) popped from a global counter with a warp-aggregated atomic; a
 // lane whose line ended refills at once (same queue as trace2_kernel).
-template <bool DEV, bool INTERP, bool REFILL>
-__global__ void __launch_bounds__(QSL_T3_THREADS, DEV ? QSL_T3_MIN_BLOCKS_LQ : QSL_T3_MIN_BLOCKS_L) trace3_kernel(const Trace3Args A)
+template <typename T, bool DEV, bool INTERP, bool REFILL>
+__global__ void __launch_bounds__(QSL_T3_THREADS, sizeof(T) == 4 ? (DEV ? QSL_T3_MIN_BLOCKS_LQ : QSL_T3_MIN_BLOCKS_L)
+                                                                  : (DEV ? QSL_T3_MIN_BLOCKS_LQ64 : QSL_T3_MIN_BLOCKS_L64))
+    trace3_kernel(const Trace3Args<T> A)
 {
-    LineState3<DEV, INTERP> ls;
-    const long long n_items = 2 * A.T.n;
+    LineState3<T, DEV, INTERP> ls;
+    const long long n_items = 2 * A.T0.n;
     unsigned long long my_steps = 0;
     if (!REFILL) {
         const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -454,7 +496,7 @@ __global__ void __launch_bounds__(QSL_T3_THREADS, DEV ? QSL_T3_MIN_BLOCKS_LQ : Q
                 const unsigned m = __activemask();
                 const int leader = __ffs(m) - 1;
                 unsigned long long base = 0;
-                if ((int)lane == leader) base = atomicAdd(A.T.queue, (unsigned long long)__popc(m));
+                if ((int)lane == leader) base = atomicAdd(A.T0.queue, (unsigned long long)__popc(m));
                 base = __shfl_sync(m, base, leader);
                 const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
                 if (q >= n_items) drained = true;
@@ -466,10 +508,10 @@ __global__ void __launch_bounds__(QSL_T3_THREADS, DEV ? QSL_T3_MIN_BLOCKS_LQ : Q
             }
         }
     }
-    if (A.T.total_steps) {
+    if (A.T0.total_steps) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) my_steps += __shfl_xor_sync(0xffffffffu, my_steps, o);
-        if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(A.T.total_steps, my_steps);
+        if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(A.T0.total_steps, my_steps);
     }
 }
 

@@ -12,10 +12,10 @@ from tests.parity import compare_trace, cpu_field, gpu_field, run_both
 
 pytestmark = pytest.mark.gpu
 
-V1 = qsl.QSL_FLAG_KERNEL_V1
+V1, FRAME = qsl.QSL_FLAG_KERNEL_V1, qsl.QSL_FLAG_KERNEL_FRAME
 ALL_FLAGS = [0, qsl.QSL_FLAG_NO_REFILL, qsl.QSL_FLAG_NO_SORT, qsl.QSL_FLAG_NO_REFILL | qsl.QSL_FLAG_NO_SORT,
-             V1, V1 | qsl.QSL_FLAG_NO_REFILL, V1 | qsl.QSL_FLAG_NO_SORT]
-KERNELS = [0, V1]          # per-cell table kernel (default) and corner-gather kernel
+             V1, V1 | qsl.QSL_FLAG_NO_REFILL, V1 | qsl.QSL_FLAG_NO_SORT, FRAME, FRAME | qsl.QSL_FLAG_NO_REFILL]
+KERNELS = [0, V1, FRAME]   # per-cell table kernel (default), corner-gather kernel, cell-frame kernel (uniform grids)
 
 
 @pytest.mark.parametrize("sample_type", ["f32", "f64"])
