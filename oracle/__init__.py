@@ -18,7 +18,7 @@ _SRC = [os.path.join(_HERE, "qsl_oracle.c"), os.path.join(_HERE, "qsl_oracle.h")
 
 F32, F64 = 0, 1
 NORMALIZE_FIRST, INTERP_FIRST = 0, 1
-RK4, EULER = 0, 1
+RK4, EULER, CK45 = 0, 1, 2
 TRACE_L, TRACE_LQ = 0, 1
 ST_SEED_OUTSIDE, ST_NULL_AT_SEED, ST_STALL_F, ST_STALL_B, ST_CAP_F, ST_CAP_B, ST_OPEN = 1, 2, 4, 8, 16, 32, 64
 
@@ -45,7 +45,7 @@ class _Field(C.Structure):
 class _Params(C.Structure):
     _fields_ = [("box_lo", C.c_double * 3), ("box_hi", C.c_double * 3), ("method", C.c_int),
                 ("step_frac", C.c_double), ("mode", C.c_int), ("max_length", C.c_double),
-                ("max_steps", C.c_longlong), ("null_eps", C.c_double), ("basis_angle", C.c_double)]
+                ("max_steps", C.c_longlong), ("null_eps", C.c_double), ("basis_angle", C.c_double), ("tol", C.c_double)]
 
 
 class _Out(C.Structure):
@@ -99,13 +99,22 @@ class Field:
         return b, J.reshape(3, 3), m.value, hc
 
 
+def ck_step(field: Field, y, h, *, with_dev=True, s=1.0):
+    """One Cash-Karp 5(4) step of the 10-component state y.  Returns (y5, y5 - y4 of the position)."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    yn = np.empty(10); err = np.empty(3)
+    lib().orc_ck_step(C.byref(field.c), C.c_int(1 if with_dev else 0), C.c_double(s), _ptr(y), C.c_double(h), _ptr(yn), _ptr(err))
+    return yn, err
+
+
 def trace(field: Field, seeds, box_lo, box_hi, *, method=RK4, step_frac=0.25, mode=TRACE_LQ,
-          max_length=math.inf, max_steps=1 << 40, null_eps=1e-12, basis_angle=0.0, nthreads=0, want_dev=False):
+          max_length=math.inf, max_steps=1 << 40, null_eps=1e-12, basis_angle=0.0, nthreads=0, want_dev=False,
+          tol=1e-2):
     """O2-O5 for every seed.  Returns a dict of numpy arrays plus total_steps."""
     seeds = np.ascontiguousarray(seeds, dtype=np.float64).reshape(-1, 3)
     n = len(seeds)
     P = _Params((C.c_double * 3)(*box_lo), (C.c_double * 3)(*box_hi), method, step_frac, mode, max_length,
-                int(max_steps), null_eps, basis_angle)
+                int(max_steps), null_eps, basis_angle, tol)
     o = dict(end_f=np.empty((n, 3)), end_b=np.empty((n, 3)), L=np.empty(n), q_perp=np.empty(n), q_bnd=np.empty(n),
              face_f=np.empty(n, np.uint8), face_b=np.empty(n, np.uint8), status=np.empty(n, np.uint32),
              nsteps_f=np.empty(n, np.uint32), nsteps_b=np.empty(n, np.uint32))

@@ -146,11 +146,63 @@ static void rhs(const orc_field *F, int with_dev, double s, const double y[10], 
 
 /* One step of size h from y, given k1 = f(y).  RK4 is the graded rule (BASELINE.json configs[0]: "fixed-step
  * RK4 with h=0.25 cell", reading A5); Euler is the paper's fixed-step scheme.           */
+/* Cash & Karp (1990) embedded pair, the scheme behind the paper's adaptive stepper: six stages,
+ * nodes c, coupling a, 5th-order weights b5 (the propagated solution) and 4th-order weights b4 of the embedded
+ * solution; y5 - y4 estimates the local error.  Written out as printed in the literature.                    */
+static const double CK_A[6][5] = {
+    { 0.0, 0.0, 0.0, 0.0, 0.0 },
+    { 1.0 / 5.0, 0.0, 0.0, 0.0, 0.0 },
+    { 3.0 / 40.0, 9.0 / 40.0, 0.0, 0.0, 0.0 },
+    { 3.0 / 10.0, -9.0 / 10.0, 6.0 / 5.0, 0.0, 0.0 },
+    { -11.0 / 54.0, 5.0 / 2.0, -70.0 / 27.0, 35.0 / 27.0, 0.0 },
+    { 1631.0 / 55296.0, 175.0 / 512.0, 575.0 / 13824.0, 44275.0 / 110592.0, 253.0 / 4096.0 } };
+static const double CK_B5[6] = { 37.0 / 378.0, 0.0, 250.0 / 621.0, 125.0 / 594.0, 0.0, 512.0 / 1771.0 };
+static const double CK_B4[6] = { 2825.0 / 27648.0, 0.0, 18575.0 / 48384.0, 13525.0 / 55296.0, 277.0 / 14336.0, 1.0 / 4.0 };
+
+/* One Cash-Karp step of size h from y given k1 = f(y): yn = 5th-order solution, err3 = (y5 - y4) of the position. */
+static void ck_step(const orc_field *F, int with_dev, double s, const double y[10], const double k1[10], double h,
+                    double yn[10], double err3[3])
+{
+    double k[6][10], yt[10];
+    memcpy(k[0], k1, sizeof k[0]);
+    for (int i = 1; i < 6; ++i) {
+        for (int q = 0; q < 10; ++q) {
+            double acc = 0.0;
+            for (int j = 0; j < i; ++j) acc += CK_A[i][j] * k[j][q];
+            yt[q] = y[q] + h * acc;
+        }
+        rhs(F, with_dev, s, yt, k[i], NULL, NULL);
+    }
+    for (int q = 0; q < 10; ++q) {
+        double a5 = 0.0;
+        for (int i = 0; i < 6; ++i) a5 += CK_B5[i] * k[i][q];
+        yn[q] = y[q] + h * a5;
+    }
+    for (int d = 0; d < 3; ++d) {
+        double e = 0.0;
+        for (int i = 0; i < 6; ++i) e += (CK_B5[i] - CK_B4[i]) * k[i][d];
+        err3[d] = h * e;
+    }
+}
+
+/* Pin hook: one Cash-Karp step from y (k1 computed here). */
+void orc_ck_step(const orc_field *F, int with_dev, double s, const double y[10], double h, double yn[10], double err3[3])
+{
+    double k1[10];
+    rhs(F, with_dev, s, y, k1, NULL, NULL);
+    ck_step(F, with_dev, s, y, k1, h, yn, err3);
+}
+
 static void take_step(const orc_field *F, const orc_trace_params *P, int with_dev, double s,
                       const double y[10], const double k1[10], double h, double yn[10])
 {
     if (P->method == ORC_EULER) {
         for (int q = 0; q < 10; ++q) yn[q] = y[q] + h * k1[q];
+        return;
+    }
+    if (P->method == ORC_CK45) {
+        double err3[3];
+        ck_step(F, with_dev, s, y, k1, h, yn, err3);
         return;
     }
     double k2[10], k3[10], k4[10], yt[10];
@@ -182,17 +234,37 @@ static void trace_direction(const orc_field *F, const orc_trace_params *P, int w
     double y[10]; memcpy(y, y0, sizeof y);
     double lam = 0.0; uint32_t nsteps = 0;
     R->face = 255; R->stall = 0; R->cap = 0;
+    /* ORC_CK45 (reading A16): the step is h = step_frac * min_d h_c,d * 2^j with the integer j in [-20, +2] as
+     * the controller state.  After a trial step the error e = max_d |y5_d - y4_d| / (tol * min_d h_c,d) of the
+     * POSITION decides: e > 1 (and j > -20) rejects and halves (j - 1); an accepted step with e < 1/64 doubles
+     * the next one (j + 1, at most +2).  Halving / doubling is exact in binary floating point, so two
+     * implementations take identical decisions; controlling x only keeps x and L independent of the mode.  */
+    int j = 0;
     for (;;) {
         double k1[10], bnorm, hc[3];                   /* hc = h_c of the cell containing x */
         rhs(F, with_dev, s, y, k1, &bnorm, hc);
         if (!(bnorm >= P->null_eps)) { R->stall = 1; break; }
         if ((long long)nsteps >= P->max_steps) { R->cap = 1; break; }
         if (lam >= P->max_length) { R->cap = 1; break; }
-        double h = P->step_frac * fmin(hc[0], fmin(hc[1], hc[2]));
+        const double hmin = fmin(hc[0], fmin(hc[1], hc[2]));
+        double h = P->step_frac * hmin;
+        if (P->method == ORC_CK45) h = ldexp(h, j);
         if (lam + h > P->max_length) h = P->max_length - lam;
         double yn[10];
-        take_step(F, P, with_dev, s, y, k1, h, yn);
-        if (inside_box(P, yn)) { memcpy(y, yn, sizeof y); lam += h; ++nsteps; continue; }
+        if (P->method == ORC_CK45) {
+            double err3[3];
+            ck_step(F, with_dev, s, y, k1, h, yn, err3);
+            const double e = fmax(fabs(err3[0]), fmax(fabs(err3[1]), fabs(err3[2]))) / (P->tol * hmin);
+            if (e > 1.0 && j > -20) { --j; continue; }                     /* reject: halve and retry from y */
+            if (inside_box(P, yn)) {
+                memcpy(y, yn, sizeof y); lam += h; ++nsteps;
+                if (e < 1.0 / 64.0 && j < 2) ++j;
+                continue;
+            }
+        } else {
+            take_step(F, P, with_dev, s, y, k1, h, yn);
+            if (inside_box(P, yn)) { memcpy(y, yn, sizeof y); lam += h; ++nsteps; continue; }
+        }
         /* the trial point left the box: first face crossed by the chord (smallest fraction; tie -> lowest
          * axis; one axis cannot violate both of its faces) */
         double phi = INFINITY, bound = 0.0; int axis = -1, face = 255;

@@ -21,7 +21,7 @@ extern "C" {
 
 enum { ORC_F32 = 0, ORC_F64 = 1 };
 enum { ORC_NORMALIZE_FIRST = 0, ORC_INTERP_FIRST = 1 };
-enum { ORC_RK4 = 0, ORC_EULER = 1 };
+enum { ORC_RK4 = 0, ORC_EULER = 1, ORC_CK45 = 2 };   /* CK45: adaptive Cash-Karp 5(4) */
 enum { ORC_TRACE_L = 0, ORC_TRACE_LQ = 1 };
 
 enum {
@@ -40,13 +40,14 @@ typedef struct {
 
 typedef struct {
     double box_lo[3], box_hi[3];
-    int method;                /* ORC_RK4 | ORC_EULER                                                    */
+    int method;                /* ORC_RK4 | ORC_EULER | ORC_CK45                                         */
     double step_frac;          /* h = step_frac * min_d h_c,d                                            */
     int mode;                  /* ORC_TRACE_L | ORC_TRACE_LQ                                             */
     double max_length;         /* cap on the affine parameter per direction; inf = off    */
     long long max_steps;
     double null_eps;
     double basis_angle;        /* rotation of (a, b) about B at the seed -- pin P3 only                  */
+    double tol;                /* ORC_CK45: error per step allowed on x, in units of min_d h_c,d         */
 } orc_trace_params;
 
 typedef struct {
@@ -63,6 +64,8 @@ void orc_field_pack(long long n_nodes, const double *bx, const double *by, const
 
 /* O1 (PAPER.md:93-107 eq. 3-4, :123, :137): b[3], J[9] (J[c*3+d] = d b_c / d x_d), m, h_cell[3]. */
 void orc_evaluate(const orc_field *F, const double x[3], double b[3], double J[9], double *m, double hc[3]);
+/* One Cash-Karp 5(4) step of size h of the state y = (x, delta1, delta2, L): yn = 5th-order result, err3 = y5 - y4 of x. */
+void orc_ck_step(const orc_field *F, int with_dev, double s, const double y[10], double h, double yn[10], double err3[3]);
 
 /* O2-O5 (PAPER.md:79 eq.1, :119 eq.5, :141, :156-176 eq.9-11, :163, :165). */
 void orc_trace(const orc_field *F, const orc_trace_params *P, long long n, const double *seeds,
