@@ -36,7 +36,8 @@ int qsl_compiled_arch(void);
 /* ---- enums ------------------------------------------------------------------------------------------------ */
 enum { QSL_F32 = 0, QSL_F64 = 1 };                       /* storage type of the packed field samples             */
 enum { QSL_NORMALIZE_FIRST = 0, QSL_INTERP_FIRST = 1 };  /* PAPER.md:178 (fn. 9) = NORMALIZE_FIRST, the default   */
-enum { QSL_RK4 = 0, QSL_EULER = 1 };                     /* PAPER.md:141; RK4: BASELINE.json configs (reading A5) */
+enum { QSL_RK4 = 0, QSL_EULER = 1, QSL_CK45 = 2 };       /* PAPER.md:141; RK4: BASELINE.json configs (reading A5);
+                                                            CK45: adaptive Cash-Karp 5(4), PAPER.md:141, :143 (reading A16) */
 enum { QSL_TRACE_L = 0, QSL_TRACE_LQ = 1 };              /* L only (FLEDGE pass) | L and Q                        */
 enum { QSL_LAYOUT_CELL_TABLE = 0, QSL_LAYOUT_NODES_ONLY = 1,    /* what qsl_field_create keeps in HBM (see qsl_grid_desc) */
        QSL_LAYOUT_CELL_TABLE_F32 = 2, QSL_LAYOUT_CELL_TABLES_BOTH = 3 };
@@ -94,7 +95,7 @@ long long qsl_field_bytes(const qsl_field *f);
 /* ---- trace (PAPER.md:79 eq. 1; :119 eq. 5; :141 integrators; :156-176 eq. 9-11 Q; :163 boundaries; :165 cap) --- */
 typedef struct {
     double box_lo[3], box_hi[3]; /* trace box, inside the grid box; may be smaller (raised lower boundary) */
-    int method;                  /* QSL_RK4 | QSL_EULER                                                            */
+    int method;                  /* QSL_RK4 | QSL_EULER | QSL_CK45 (fp64 arithmetic on the fp64 cell table only)   */
     double step_frac;            /* h = step_frac * min_d h_c,d of the cell containing x; > 0   */
     int mode;                    /* QSL_TRACE_L | QSL_TRACE_LQ                                                      */
     int arith;                   /* QSL_ARITH_F64 | QSL_ARITH_F32                                                   */
@@ -102,6 +103,10 @@ typedef struct {
     long long max_steps;         /* cap on accepted steps per direction; >= 1                                       */
     double null_eps;             /* stall threshold on |b|                                                          */
     unsigned int flags;          /* QSL_FLAG_*                                                                      */
+    double tol;                  /* QSL_CK45 only (> 0): error allowed per step on the position, in units of the
+                                    smallest edge of the current cell (PAPER.md:143 uses 1e-2).  The step is
+                                    step_frac * min_d h_c,d * 2^j, j in [-20, +2]: a step whose error estimate
+                                    |x5 - x4|_max exceeds tol is halved and retried, one below tol/64 doubles the next */
 } qsl_trace_params;
 
 typedef struct {                 /* every member may be NULL (output not wanted); n = number of seeds               */

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libqsl.so")
 
 QSL_F32, QSL_F64 = 0, 1
 QSL_NORMALIZE_FIRST, QSL_INTERP_FIRST = 0, 1
-QSL_RK4, QSL_EULER = 0, 1
+QSL_RK4, QSL_EULER, QSL_CK45 = 0, 1, 2
 QSL_TRACE_L, QSL_TRACE_LQ = 0, 1
 QSL_ARITH_F64, QSL_ARITH_F32 = 0, 1
 QSL_LAYOUT_CELL_TABLE, QSL_LAYOUT_NODES_ONLY, QSL_LAYOUT_CELL_TABLE_F32, QSL_LAYOUT_CELL_TABLES_BOTH = 0, 1, 2, 3
@@ -40,7 +40,7 @@ class _GridDesc(C.Structure):
 class _TraceParams(C.Structure):
     _fields_ = [("box_lo", C.c_double * 3), ("box_hi", C.c_double * 3), ("method", C.c_int),
                 ("step_frac", C.c_double), ("mode", C.c_int), ("arith", C.c_int), ("max_length", C.c_double),
-                ("max_steps", C.c_longlong), ("null_eps", C.c_double), ("flags", C.c_uint)]
+                ("max_steps", C.c_longlong), ("null_eps", C.c_double), ("flags", C.c_uint), ("tol", C.c_double)]
 
 
 class _TraceOut(C.Structure):
@@ -180,10 +180,10 @@ DEFAULT_OUTPUTS = ("end_f", "end_b", "L", "q_perp", "q_bnd", "face_f", "face_b",
 
 
 def make_trace_params(box_lo, box_hi, *, method=QSL_RK4, step_frac=0.25, mode=QSL_TRACE_LQ, arith=QSL_ARITH_F64,
-                      max_length=math.inf, max_steps=1 << 30, null_eps=1e-12, flags=0) -> _TraceParams:
+                      max_length=math.inf, max_steps=1 << 30, null_eps=1e-12, flags=0, tol=1e-2) -> _TraceParams:
     return _TraceParams((C.c_double * 3)(*[float(v) for v in box_lo]), (C.c_double * 3)(*[float(v) for v in box_hi]),
                         int(method), float(step_frac), int(mode), int(arith), float(max_length), int(max_steps),
-                        float(null_eps), int(flags))
+                        float(null_eps), int(flags), float(tol))
 
 
 def qsl_trace(field: Field, seeds: torch.Tensor, params: _TraceParams, *, outputs=DEFAULT_OUTPUTS, out=None,

@@ -9,6 +9,7 @@ namespace qsl {
 cudaError_t launch_trace_f32(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 cudaError_t launch_trace_f64(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 int launch_trace2(TraceArgs &A, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
+int launch_trace_ck(TraceArgs &A, double tol, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 int launch_trace3(const TraceArgs &T, const void *cells32, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 int launch_trace3_f64(const TraceArgs &T, bool samples_f32, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 cudaError_t launch_epilogue_f32(const EpilogueArgs &E, cudaStream_t s);
@@ -60,7 +61,9 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
                          const qsl_trace_out *out, unsigned long long *total_steps, void *stream)
 {
     if (!f || !p || !out || n < 0 || (n > 0 && !seeds)) return QSL_EINVAL;
-    if (p->method != QSL_RK4 && p->method != QSL_EULER) return QSL_EINVAL;
+    if (p->method != QSL_RK4 && p->method != QSL_EULER && p->method != QSL_CK45) return QSL_EINVAL;
+    // the adaptive stepper runs in fp64 on the fp64 cell table only, with a positive tolerance
+    if (p->method == QSL_CK45 && (!f->view.cells || p->arith != QSL_ARITH_F64 || !(p->tol > 0.0))) return QSL_EINVAL;
     if (p->mode != QSL_TRACE_L && p->mode != QSL_TRACE_LQ) return QSL_EINVAL;
     if (p->arith != QSL_ARITH_F64 && p->arith != QSL_ARITH_F32) return QSL_EINVAL;
     // fp32 arithmetic (reading A6): needs the fp32 coefficient table (QSL_LAYOUT_CELL_TABLE_F32 / _BOTH), which
@@ -101,7 +104,10 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
         const bool dev = p->mode == QSL_TRACE_LQ;
         const bool v2 = f->view.cells != nullptr && !(p->flags & QSL_FLAG_KERNEL_V1);
-        if (e == cudaSuccess && p->arith == QSL_ARITH_F32) {
+        if (e == cudaSuccess && p->method == QSL_CK45) {
+            const int ps = prof_slot(p->mode);
+            rc = launch_trace_ck(A, p->tol, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
+        } else if (e == cudaSuccess && p->arith == QSL_ARITH_F32) {
             const int ps = prof_slot(p->mode);
             rc = launch_trace3(A, f->d_cells32, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
         } else if (e == cudaSuccess && v2 && !f->view.stretched && (p->flags & QSL_FLAG_KERNEL_FRAME)) {

@@ -1,0 +1,180 @@
+// Adaptive Cash-Karp 5(4) trace kernel (QSL_CK45).  PAPER.md:141: "an adaptive Runge-Kutta
+// Cash-Karp method (Cash & Karp 1990)"; tolerance 1e-2, used "for testing the convergence properties" of
+// the fixed-step scheme.  Reading A16 of DESIGN.md fixes the controller: h = step_frac * min_d h_c,d * 2^j with the
+// integer j in [-20, +2] as per-line state; after a trial step e = max_d |x5_d - x4_d| / (tol * min_d h_c,d); e > 1
+// (and j > -20) rejects and halves; an accepted step with e < 1/64 doubles the next one.  Only the position is
+// controlled, so x, L and the step counts do not depend on the trace mode.
+//
+// The field evaluation, the cached per-cell polynomial, the records and the landing rule (reading A4) are those of
+// the cell-table kernel (LineState2); an attempt is six evaluations (plus one at the previous trial end during the
+// four landing attempts of a line).  This is the convergence-check integrator, not the throughput path: the five stage
+// derivatives of the 9-component state are held per thread and the kernel runs at two CTAs per SM.
+#pragma once
+#include "trace2_kernels.cuh"
+
+namespace qsl {
+
+template <bool DEV, bool STRETCHED, bool INTERP>
+struct LineStateCK : LineState2<DEV, STRETCHED, INTERP> {
+    using Base = LineState2<DEV, STRETCHED, INTERP>;
+    static constexpr int NV = Base::NV;
+    int j;                     // controller state: h = h0 2^j
+    double hp, hfull, bound, xt[3];
+    int axis, face;
+
+    // unsigned derivative (b, J d1, J d2) and |b| at the state ys; the direction sign is folded into the step
+    __device__ __forceinline__ void eval(const TraceArgs &A, const double *ys, double *k, double &bn)
+    {
+        double d[3], b[3];
+        this->enter_cell(A, ys, d);
+        this->stage(d, ys, b, k);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) k[c] = b[c];
+        bn = norm3_fast(b);
+    }
+
+    __device__ bool advance_ck(const TraceArgs &A, double tol)
+    {
+        // Cash & Karp (1990): coupling coefficients, 5th-order weights, and (5th - 4th)-order weight differences
+        constexpr double a21 = 1.0 / 5.0;
+        constexpr double a31 = 3.0 / 40.0, a32 = 9.0 / 40.0;
+        constexpr double a41 = 3.0 / 10.0, a42 = -9.0 / 10.0, a43 = 6.0 / 5.0;
+        constexpr double a51 = -11.0 / 54.0, a52 = 5.0 / 2.0, a53 = -70.0 / 27.0, a54 = 35.0 / 27.0;
+        constexpr double a61 = 1631.0 / 55296.0, a62 = 175.0 / 512.0, a63 = 575.0 / 13824.0, a64 = 44275.0 / 110592.0,
+                         a65 = 253.0 / 4096.0;
+        constexpr double b1 = 37.0 / 378.0, b3 = 250.0 / 621.0, b4 = 125.0 / 594.0, b6 = 512.0 / 1771.0;
+        constexpr double e1 = b1 - 2825.0 / 27648.0, e3 = b3 - 18575.0 / 48384.0, e4 = b4 - 13525.0 / 55296.0,
+                         e5 = -277.0 / 14336.0, e6 = b6 - 1.0 / 4.0;
+        double k1[NV], k2[NV], k3[NV], k4[NV], k5[NV], k6[NV], ys[NV];
+        double n1, n2, n3, n4, n5, n6;
+        double h = 0.0, hs, hmin = 0.0;
+        if (this->phase >= 2) {
+            // one Newton update of the landing step from the field at the previous trial end (reading A4)
+            double kt[NV], nt, p[NV];
+#pragma unroll
+            for (int c = 0; c < NV; ++c) p[c] = c < 3 ? xt[c] : this->y[c];
+            eval(A, p, kt, nt);
+            const double bd = axis == 0 ? kt[0] : (axis == 1 ? kt[1] : kt[2]);
+            const double xd = axis == 0 ? xt[0] : (axis == 1 ? xt[1] : xt[2]);
+            const double gg = this->back ? -bd : bd, r = xd - bound;
+            if (gg != 0.0) {
+                const double hn = hp - r / gg;
+                if (hn == hn) hp = fmin(fmax(hn, 0.0), hfull);
+            }
+        }
+        eval(A, this->y, k1, n1);
+        if (this->phase == 0) {
+            if (!(n1 >= A.null_eps)) { this->finish(A, 255, this->nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL); return true; }
+            if ((long long)this->nsteps >= A.max_steps || this->lam >= A.max_length) { this->finish(A, 255, REC_CAP); return true; }
+            hmin = STRETCHED ? fmin(this->hc[0], fmin(this->hc[1], this->hc[2])) : fmin(A.fv.h[0], fmin(A.fv.h[1], A.fv.h[2]));
+            h = (A.step_frac * hmin) * __hiloint2double((1023 + j) << 20, 0);      // exact scaling by 2^j
+            if (this->lam + h > A.max_length) h = A.max_length - this->lam;
+            hs = h;
+        } else {
+            hs = hp;
+        }
+        const double sh = this->back ? -hs : hs;
+#define QSL_CK_STAGE(EXPR, KOUT, NOUT)                                                   \
+        {                                                                                \
+            _Pragma("unroll") for (int c = 0; c < NV; ++c) ys[c] = fma(sh, (EXPR), this->y[c]); \
+            eval(A, ys, KOUT, NOUT);                                                     \
+        }
+        QSL_CK_STAGE(a21 * k1[c], k2, n2)
+        QSL_CK_STAGE(fma(a32, k2[c], a31 * k1[c]), k3, n3)
+        QSL_CK_STAGE(fma(a43, k3[c], fma(a42, k2[c], a41 * k1[c])), k4, n4)
+        QSL_CK_STAGE(fma(a54, k4[c], fma(a53, k3[c], fma(a52, k2[c], a51 * k1[c]))), k5, n5)
+        QSL_CK_STAGE(fma(a65, k5[c], fma(a64, k4[c], fma(a63, k3[c], fma(a62, k2[c], a61 * k1[c])))), k6, n6)
+#undef QSL_CK_STAGE
+        // 5th-order result and the position error estimate
+#pragma unroll
+        for (int c = 0; c < NV; ++c) ys[c] = fma(sh, fma(b6, k6[c], fma(b4, k4[c], fma(b3, k3[c], b1 * k1[c]))), this->y[c]);
+        const double Ln = fma(hs, fma(b6, n6, fma(b4, n4, fma(b3, n3, b1 * n1))), this->L);
+        if (this->phase == 0) {
+            double emax = 0.0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double e = hs * fma(e6, k6[c], fma(e5, k5[c], fma(e4, k4[c], fma(e3, k3[c], e1 * k1[c]))));
+                emax = fmax(emax, fabs(e));
+            }
+            const double en = emax / (tol * hmin);
+            if (en > 1.0 && j > -20) { --j; return false; }                 // reject: halve, retry from y
+            if (inside_box(A, ys)) {
+#pragma unroll
+                for (int c = 0; c < NV; ++c) this->y[c] = ys[c];
+                this->L = Ln; this->lam += h; ++this->nsteps;
+                if (en < 1.0 / 64.0 && j < 2) ++j;
+                return false;
+            }
+            // first face crossed by the chord: smallest fraction, tie -> lowest axis (reading A4)
+            double phi = INFINITY; int ax = -1, fc = 255; double bd = 0.0;
+#pragma unroll
+            for (int dd = 0; dd < 3; ++dd) {
+                if (ys[dd] < A.box_lo[dd]) {
+                    const double f = (A.box_lo[dd] - this->y[dd]) / (ys[dd] - this->y[dd]);
+                    if (f < phi) { phi = f; ax = dd; fc = 2 * dd; bd = A.box_lo[dd]; }
+                } else if (ys[dd] > A.box_hi[dd]) {
+                    const double f = (A.box_hi[dd] - this->y[dd]) / (ys[dd] - this->y[dd]);
+                    if (f < phi) { phi = f; ax = dd; fc = 2 * dd + 1; bd = A.box_hi[dd]; }
+                }
+            }
+            if (ax < 0) { this->finish(A, 255, REC_STALL); return true; }   // non-finite trial point
+            hp = phi * h; hfull = h; bound = bd; axis = ax; face = fc;
+            this->phase = 1;
+            return false;
+        }
+        if (this->phase < 4) {
+            xt[0] = ys[0]; xt[1] = ys[1]; xt[2] = ys[2];
+            ++this->phase;
+            return false;
+        }
+        // phase 4: final landing step, snapped onto the face
+#pragma unroll
+        for (int c = 0; c < NV; ++c) this->y[c] = ys[c];
+        if (axis == 0) this->y[0] = bound; else if (axis == 1) this->y[1] = bound; else this->y[2] = bound;
+        this->L = Ln; this->lam += hp; ++this->nsteps;
+        this->finish(A, face, 0);
+        return true;
+    }
+};
+
+template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL>
+__global__ void __launch_bounds__(128, 2) trace_ck_kernel(const TraceArgs A, const double tol)
+{
+    LineStateCK<DEV, STRETCHED, INTERP> ls;
+    const long long n_items = 2 * A.n;
+    unsigned long long my_steps = 0;
+    if (!REFILL) {
+        const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        if (q < n_items) {
+            ls.j = 0;
+            if (ls.init(A, q)) { while (!ls.advance_ck(A, tol)) {} }
+            my_steps = ls.nsteps;
+        }
+    } else {
+        const unsigned lane = threadIdx.x & 31u;
+        bool have = false, drained = false;
+        while (true) {
+            if (!have && !drained) {
+                const unsigned m = __activemask();
+                const int leader = __ffs(m) - 1;
+                unsigned long long base = 0;
+                if ((int)lane == leader) base = atomicAdd(A.queue, (unsigned long long)__popc(m));
+                base = __shfl_sync(m, base, leader);
+                const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
+                if (q >= n_items) drained = true;
+                else { ls.j = 0; have = ls.init(A, q); }
+            }
+            if (__all_sync(0xffffffffu, drained && !have)) break;
+            if (have) {
+                if (ls.advance_ck(A, tol)) { my_steps += ls.nsteps; have = false; }
+            }
+        }
+    }
+    if (A.total_steps) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) my_steps += __shfl_xor_sync(0xffffffffu, my_steps, o);
+        if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(A.total_steps, my_steps);
+    }
+}
+
+}  // namespace qsl

@@ -25,12 +25,12 @@ def cpu_field(grid, B, sample_type, interp_mode):
 
 
 def run_both(grid, B, sample_type, seeds, box_lo, box_hi, *, interp_mode=0, mode=1, method=0, step_frac=0.25,
-             max_steps=1 << 30, max_length=math.inf, null_eps=1e-12, flags=0, want_dev=False):
+             max_steps=1 << 30, max_length=math.inf, null_eps=1e-12, flags=0, want_dev=False, tol=1e-2):
     st = "f32" if sample_type in ("f32", 0) else "f64"
     fg = gpu_field(grid, B, st, interp_mode)
     fc = cpu_field(grid, B, st, interp_mode)
     params = qsl.make_trace_params(box_lo, box_hi, method=method, step_frac=step_frac, mode=mode, max_length=max_length,
-                                   max_steps=max_steps, null_eps=null_eps, flags=flags)
+                                   max_steps=max_steps, null_eps=null_eps, flags=flags, tol=tol)
     outs = qsl.DEFAULT_OUTPUTS + (("dev_f", "dev_b") if want_dev else ())
     tot = torch.zeros(1, dtype=torch.int64, device="cuda")
     g = qsl.qsl_trace(fg, torch.from_numpy(np.ascontiguousarray(seeds)).cuda(), params, outputs=outs, total_steps=tot)
@@ -40,7 +40,7 @@ def run_both(grid, B, sample_type, seeds, box_lo, box_hi, *, interp_mode=0, mode
     for k in ("status", "nsteps_f", "nsteps_b"):
         g[k] = g[k].view(np.uint32)
     c = oracle.trace(fc, seeds, box_lo, box_hi, method=method, step_frac=step_frac, mode=mode, max_length=max_length,
-                     max_steps=max_steps, null_eps=null_eps, want_dev=want_dev)
+                     max_steps=max_steps, null_eps=null_eps, want_dev=want_dev, tol=tol)
     fg.destroy()
     return g, c
 
