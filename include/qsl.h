@@ -175,6 +175,43 @@ int qsl_refine(int ndim, int level, long long n, const unsigned int *coords, con
  * space-filling curve), exposed so that tests can check it on its own.                                              */
 int qsl_debug_sort_pairs(unsigned int *keys, unsigned int *vals, long long n, int key_bits, void *stream);
 
+/* ---- the paper's own refinement along a Hilbert curve (section 3.6; reading A17) -------- *
+ * A sample sits at the centre of a cell of the finest lattice n_d 2^R ("fine cell", integer coordinates c); its position
+ * is origin + sum_d (c_d + 0.5)/(n_d 2^R) e_d.  Its place along the curve is the 64-bit key of c on the Hilbert curve
+ * (Skilling 2004) of `bits` = qsl_hilbert_bits(lat, R) bits per axis; the shifted curve of PAPER.md:204 is the curve of
+ * bits + 1 bits through the cells c + shift.  All arrays are DEVICE pointers; coordinates are n*ndim uint32.            */
+/* Bits per axis of the cube bounding the finest lattice (>= 1), or QSL_EINVAL / QSL_ERANGE ((bits + 1) ndim > 63).       */
+int qsl_hilbert_bits(const qsl_lattice *lat, int R);
+/* Level-0 samples in dense order (c2 n1 + c1) n0 + c0: fine cell c0 2^R + 2^(R-1) and its centre (seeds: n*3 fp64).      */
+int qsl_hilbert_level0(const qsl_lattice *lat, int R, unsigned int *coords, double *seeds, void *stream);
+/* keys[i] = position along the curve of `bits` bits per axis of the cell coords[i] + shift; and the inverse.             */
+int qsl_hilbert_keys(int ndim, int bits, int shift, long long n, const unsigned int *coords, unsigned long long *keys,
+                     void *stream);
+int qsl_hilbert_cells(int ndim, int bits, int shift, long long n, const unsigned long long *keys, unsigned int *coords,
+                      void *stream);
+/* Sorts keys ascending in place (stable LSD radix sort on key_bits bits) and writes the permutation: the sorted keys[i] is
+ * the input keys[perm[i]].  qsl_gather: dst[i] = src[perm[i]] for elements of elem_bytes (a multiple of 4) bytes.          */
+int qsl_sort_keys64(long long n, unsigned long long *keys, unsigned int *perm, int key_bits, void *stream);
+int qsl_gather(long long n, const unsigned int *perm, int elem_bytes, const void *src, void *dst, void *stream);
+/* One refinement pass over n samples sorted by `keys` (the keys of the shifted curve if shift != 0):
+ * between successive samples i, i+1 with both L finite, |L[i+1] - L[i]| > thr and keys[i+1] - keys[i] >= 2 a new sample
+ * at key (keys[i] + keys[i+1]) >> 1 - "halfway along the Hilbert curve" - unless that cell (displaced back by shift) lies
+ * outside the lattice.  Writes, in curve order, left[j] = i, the fine cell and the position of every new sample, and the
+ * count to *n_new (HOST; synchronises the stream).  QSL_ERANGE if the count exceeds `capacity` (*n_new = needed).         */
+int qsl_hilbert_refine(const qsl_lattice *lat, int R, int shift, long long n, const unsigned long long *keys, const double *L,
+                       double thr, long long capacity, long long *left, unsigned int *new_coords, double *new_seeds,
+                       long long *n_new, void *stream);
+/* Merges a payload array of the old samples with that of the new ones, keeping the curve order: new sample j goes right
+ * after old sample left[j] (left ascending, as written by qsl_hilbert_refine).  out: n_old + n_new elements.               */
+int qsl_hilbert_merge(long long n_old, long long n_new, const long long *left, int elem_bytes, const void *old_vals,
+                      const void *new_vals, void *out, void *stream);
+/* Converter: samples sorted by their un-shifted keys -> dense map on the lattice n_d 2^r (r <= R), index
+ * (c2 d1 + c1) d0 + c0: the maximum of the finite Q inside a cell; a cell without sample takes 10^(log10 Q interpolated
+ * linearly in the key between the last sample with Q > 0 before the cell's key range and the first after it, at the middle
+ * of the range); one-sided at the ends of the curve; NaN if there is no such sample at all.                                 */
+int qsl_hilbert_convert(const qsl_lattice *lat, int R, int r, long long n, const unsigned long long *keys, const double *Q,
+                        double *out, void *stream);
+
 /* ---- measurement hooks (bench.py) ------------------------------------------------------------------ */
 /* qsl_profile_enable(1): every later qsl_trace records a CUDA event pair around its trace kernel (the dominant
  * kernel) on the caller's stream (up to 256 launches between two reads).  qsl_profile_trace_kernel_ms waits for the pairs

@@ -228,7 +228,7 @@ def convert(lat, R, r, keys, Q):
         p = bisect.bisect_left(uk, k0) - 1           # last usable sample before the range
         q = bisect.bisect_left(uk, k1)               # first usable sample after it
         if p >= 0 and q < len(uk):
-            t = (kc - uk[p]) / (uk[q] - uk[p])
+            t = float(kc - uk[p]) / float(uk[q] - uk[p])      # both differences rounded to fp64 first, then one division
             la, lb = math.log10(Q[usable[p]]), math.log10(Q[usable[q]])
             out[f] = 10.0 ** (la + t * (lb - la))
         elif p >= 0:

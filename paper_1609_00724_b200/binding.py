@@ -275,6 +275,118 @@ def qsl_refine(lattice, level: int, coords, S: torch.Tensor, tau: torch.Tensor, 
     return cc[: m.value], cs[: m.value], cb
 
 
+# ---- the paper's Hilbert-curve refinement (include/qsl.h) --------------------------------------------
+def _p(t):
+    return C.c_void_p(t.data_ptr()) if t is not None and t.numel() else None
+
+
+def qsl_hilbert_bits(lattice, R: int) -> int:
+    b = lib().qsl_hilbert_bits(C.byref(make_lattice(lattice)), C.c_int(R))
+    _check(min(b, 0), "qsl_hilbert_bits")
+    return int(b)
+
+
+def qsl_hilbert_level0(lattice, R: int, *, stream=None):
+    """(coords int32 (n, ndim), seeds float64 (n, 3)) of the level-0 samples in dense order."""
+    _require_cuda()
+    nd = int(lattice.ndim)
+    n = 1
+    for v in list(lattice.n)[:nd]:
+        n *= int(v)
+    coords = torch.empty((n, nd), dtype=torch.int32, device="cuda")
+    seeds = torch.empty((n, 3), dtype=torch.float64, device="cuda")
+    _check(lib().qsl_hilbert_level0(C.byref(make_lattice(lattice)), C.c_int(R), _p(coords), _p(seeds), _stream_ptr(stream)),
+           "qsl_hilbert_level0")
+    return coords, seeds
+
+
+def qsl_hilbert_keys(coords: torch.Tensor, bits: int, shift: int = 0, *, stream=None) -> torch.Tensor:
+    """coords: CUDA int32 (n, ndim).  Returns the keys as CUDA int64 (they are below 2^63)."""
+    _require_cuda()
+    n, nd = int(coords.shape[0]), int(coords.shape[1])
+    if coords.dtype != torch.int32 or not coords.is_cuda or not coords.is_contiguous():
+        raise QslError("coords must be a contiguous CUDA int32 (n, ndim) tensor")
+    keys = torch.empty(n, dtype=torch.int64, device="cuda")
+    _check(lib().qsl_hilbert_keys(C.c_int(nd), C.c_int(bits), C.c_int(shift), C.c_longlong(n), _p(coords), _p(keys),
+                                  _stream_ptr(stream)), "qsl_hilbert_keys")
+    return keys
+
+
+def qsl_hilbert_cells(keys: torch.Tensor, ndim: int, bits: int, shift: int = 0, *, stream=None) -> torch.Tensor:
+    _require_cuda()
+    n = int(keys.numel())
+    if keys.dtype != torch.int64 or not keys.is_cuda or not keys.is_contiguous():
+        raise QslError("keys must be a contiguous CUDA int64 tensor")
+    coords = torch.empty((n, ndim), dtype=torch.int32, device="cuda")
+    _check(lib().qsl_hilbert_cells(C.c_int(ndim), C.c_int(bits), C.c_int(shift), C.c_longlong(n), _p(keys), _p(coords),
+                                   _stream_ptr(stream)), "qsl_hilbert_cells")
+    return coords
+
+
+def qsl_sort_keys64(keys: torch.Tensor, key_bits: int = 64, *, stream=None) -> torch.Tensor:
+    """Sorts `keys` (CUDA int64, non-negative) in place; returns the permutation (CUDA int32)."""
+    _require_cuda()
+    n = int(keys.numel())
+    if keys.dtype != torch.int64 or not keys.is_cuda or not keys.is_contiguous():
+        raise QslError("keys must be a contiguous CUDA int64 tensor")
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    _check(lib().qsl_sort_keys64(C.c_longlong(n), _p(keys), _p(perm), C.c_int(key_bits), _stream_ptr(stream)), "qsl_sort_keys64")
+    return perm
+
+
+def qsl_gather(perm: torch.Tensor, src: torch.Tensor, *, stream=None) -> torch.Tensor:
+    """dst[i] = src[perm[i]] along the first axis (rows of a multiple of 4 bytes)."""
+    _require_cuda()
+    n = int(perm.numel())
+    if not src.is_cuda or not src.is_contiguous() or perm.dtype != torch.int32:
+        raise QslError("src must be a contiguous CUDA tensor, perm CUDA int32")
+    row = src.element_size() * (src.numel() // max(int(src.shape[0]), 1))
+    dst = torch.empty((n,) + tuple(src.shape[1:]), dtype=src.dtype, device="cuda")
+    _check(lib().qsl_gather(C.c_longlong(n), _p(perm), C.c_int(row), _p(src), _p(dst), _stream_ptr(stream)), "qsl_gather")
+    return dst
+
+
+def qsl_hilbert_refine(lattice, R: int, shift: int, keys: torch.Tensor, L: torch.Tensor, thr: float, *, capacity=None,
+                       stream=None):
+    """One refinement pass.  Returns (left int64 (m,), new_coords int32 (m, ndim), new_seeds float64 (m, 3))."""
+    _require_cuda()
+    n, nd = int(keys.numel()), int(lattice.ndim)
+    cap = int(capacity) if capacity is not None else max(n - 1, 0)
+    left = torch.empty(cap, dtype=torch.int64, device="cuda")
+    nc = torch.empty((cap, nd), dtype=torch.int32, device="cuda")
+    ns = torch.empty((cap, 3), dtype=torch.float64, device="cuda")
+    m = C.c_longlong(0)
+    _check(lib().qsl_hilbert_refine(C.byref(make_lattice(lattice)), C.c_int(R), C.c_int(shift), C.c_longlong(n), _p(keys),
+                                    _dev_f64(L, "L") if n else None, C.c_double(thr), C.c_longlong(cap), _p(left), _p(nc), _p(ns),
+                                    C.byref(m), _stream_ptr(stream)), "qsl_hilbert_refine")
+    return left[: m.value], nc[: m.value], ns[: m.value]
+
+
+def qsl_hilbert_merge(left: torch.Tensor, old: torch.Tensor, new: torch.Tensor, *, stream=None) -> torch.Tensor:
+    _require_cuda()
+    n_old, n_new = int(old.shape[0]), int(new.shape[0])
+    if old.dtype != new.dtype or old.shape[1:] != new.shape[1:] or not old.is_contiguous() or not new.is_contiguous():
+        raise QslError("old and new payloads must be contiguous tensors of the same dtype and row shape")
+    row = old.element_size()
+    for v in old.shape[1:]:
+        row *= int(v)
+    out = torch.empty((n_old + n_new,) + tuple(old.shape[1:]), dtype=old.dtype, device="cuda")
+    _check(lib().qsl_hilbert_merge(C.c_longlong(n_old), C.c_longlong(n_new), _p(left), C.c_int(row), _p(old), _p(new), _p(out),
+                                   _stream_ptr(stream)), "qsl_hilbert_merge")
+    return out
+
+
+def qsl_hilbert_convert(lattice, R: int, r: int, keys: torch.Tensor, Q: torch.Tensor, *, stream=None) -> torch.Tensor:
+    """Dense Q map on the lattice n_d 2^r, shape (d1, d0) or (d2, d1, d0)."""
+    _require_cuda()
+    nd = int(lattice.ndim)
+    dims = [int(v) << r for v in list(lattice.n)[:nd]]
+    out = torch.empty(tuple(dims[::-1]), dtype=torch.float64, device="cuda")
+    _check(lib().qsl_hilbert_convert(C.byref(make_lattice(lattice)), C.c_int(R), C.c_int(r), C.c_longlong(keys.numel()), _p(keys),
+                                     _p(Q), _p(out), _stream_ptr(stream)), "qsl_hilbert_convert")
+    return out
+
+
 # ---- measurement hooks (bench.py) ----------------------------------------------------------------------------------
 def qsl_profile_enable(on: bool = True):
     _require_cuda()

@@ -59,7 +59,8 @@ __global__ void __launch_bounds__(256) iota_kernel(long long n, uint32_t *perm)
 }
 
 // counts[digit * n_chunks + chunk] = number of keys of `chunk` whose current digit is `digit`
-__global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(long long n, const uint32_t *__restrict__ keys, int shift,
+template <typename K>
+__global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(long long n, const K *__restrict__ keys, int shift,
                                                                  long long n_chunks, uint32_t *__restrict__ counts)
 {
     __shared__ uint32_t h[SORT_WARPS][256];
@@ -69,16 +70,17 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(long long n, co
     const long long chunk = (long long)blockIdx.x * SORT_WARPS + w;
     if (chunk < n_chunks) {
         const long long lo = chunk * SORT_CHUNK, hi = min(lo + SORT_CHUNK, n);
-        for (long long i = lo + lane; i < hi; i += 32) atomicAdd(&h[w][(keys[i] >> shift) & 255u], 1u);
+        for (long long i = lo + lane; i < hi; i += 32) atomicAdd(&h[w][(uint32_t)(keys[i] >> shift) & 255u], 1u);
         __syncwarp();
         for (int b = lane; b < 256; b += 32) counts[(long long)b * n_chunks + chunk] = h[w][b];
     }
 }
 
-__global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(long long n, const uint32_t *__restrict__ keys,
+template <typename K>
+__global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(long long n, const K *__restrict__ keys,
                                                                     const uint32_t *__restrict__ vals, int shift, long long n_chunks,
                                                                     const unsigned long long *__restrict__ offsets,
-                                                                    uint32_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out)
+                                                                    K *__restrict__ keys_out, uint32_t *__restrict__ vals_out)
 {
     __shared__ unsigned long long base[SORT_WARPS][256];
     const unsigned lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
@@ -90,8 +92,9 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(long long n,
     for (long long i0 = lo; i0 < hi; i0 += 32) {
         const long long i = i0 + lane;
         const bool live = i < hi;
-        const uint32_t k = live ? keys[i] : 0u, v = live ? vals[i] : 0u;
-        const uint32_t digit = live ? ((k >> shift) & 255u) : 256u + lane;       // dead lanes match nobody
+        const K k = live ? keys[i] : (K)0;
+        const uint32_t v = live ? vals[i] : 0u;
+        const uint32_t digit = live ? ((uint32_t)(k >> shift) & 255u) : 256u + lane;   // dead lanes match nobody
         const unsigned peers = __match_any_sync(0xffffffffu, digit);
         const unsigned rank = __popc(peers & ((1u << lane) - 1u));
         unsigned long long dst = 0;
@@ -103,8 +106,9 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(long long n,
     }
 }
 
-int radix_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, long long n, int key_bits,
-                     cudaStream_t s)
+template <typename K>
+static int radix_sort_pairs_t(K *keys, uint32_t *vals, K *keys_tmp, uint32_t *vals_tmp, long long n, int key_bits,
+                              cudaStream_t s)
 {
     // sorts in place (an even number of passes ping-pongs back into keys / vals)
     int passes = (key_bits + 7) / 8;
@@ -119,23 +123,36 @@ int radix_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_
     cudaError_t e = cudaSuccess;
     if (rc == QSL_OK) {
         const unsigned blocks = (unsigned)((n_chunks + SORT_WARPS - 1) / SORT_WARPS);
-        uint32_t *ki = keys, *vi = vals, *ko = keys_tmp, *vo = vals_tmp;
+        K *ki = keys, *ko = keys_tmp;
+        uint32_t *vi = vals, *vo = vals_tmp;
         for (int p = 0; p < passes && e == cudaSuccess; ++p) {
             count_launch();
-            sort_hist_kernel<<<blocks, SORT_THREADS, 0, s>>>(n, ki, 8 * p, n_chunks, (uint32_t *)counts);
+            sort_hist_kernel<K><<<blocks, SORT_THREADS, 0, s>>>(n, ki, 8 * p, n_chunks, (uint32_t *)counts);
             e = exclusive_scan_u32(table, (const uint32_t *)counts, (unsigned long long *)offsets, (unsigned long long *)tiles,
                                    (unsigned long long *)total, s);
             if (e != cudaSuccess) break;
             count_launch();
-            sort_scatter_kernel<<<blocks, SORT_THREADS, 0, s>>>(n, ki, vi, 8 * p, n_chunks, (const unsigned long long *)offsets, ko, vo);
+            sort_scatter_kernel<K><<<blocks, SORT_THREADS, 0, s>>>(n, ki, vi, 8 * p, n_chunks, (const unsigned long long *)offsets, ko, vo);
             e = cudaGetLastError();
-            uint32_t *t = ki; ki = ko; ko = t;
-            t = vi; vi = vo; vo = t;
+            K *t = ki; ki = ko; ko = t;
+            uint32_t *u = vi; vi = vo; vo = u;
         }
         if (e != cudaSuccess) rc = record_cuda(e);
     }
     scratch_free(counts, s); scratch_free(offsets, s); scratch_free(tiles, s); scratch_free(total, s);
     return rc;
+}
+
+int radix_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, long long n, int key_bits,
+                     cudaStream_t s)
+{
+    return radix_sort_pairs_t<uint32_t>(keys, vals, keys_tmp, vals_tmp, n, key_bits, s);
+}
+
+int radix_sort_pairs64(unsigned long long *keys, uint32_t *vals, unsigned long long *keys_tmp, uint32_t *vals_tmp, long long n,
+                       int key_bits, cudaStream_t s)
+{
+    return radix_sort_pairs_t<unsigned long long>(keys, vals, keys_tmp, vals_tmp, n, key_bits, s);
 }
 
 int morton_order(const FieldView &fv, long long n, const double *seeds, uint32_t *perm, bool sort, cudaStream_t s)

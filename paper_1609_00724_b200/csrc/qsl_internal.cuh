@@ -42,6 +42,8 @@ struct FieldView {
 // Sort (key, value) pairs by 32-bit key, ascending, stable.  Hand-written LSD radix sort (order.cu).
 int radix_sort_pairs(uint32_t *keys, uint32_t *vals, uint32_t *keys_tmp, uint32_t *vals_tmp, long long n,
                      int key_bits, cudaStream_t s);
+int radix_sort_pairs64(unsigned long long *keys, uint32_t *vals, unsigned long long *keys_tmp, uint32_t *vals_tmp, long long n,
+                       int key_bits, cudaStream_t s);
 // perm (n) = seed indices ordered by the Morton code of the seed's field cell; identity if !sort.
 int morton_order(const FieldView &fv, long long n, const double *seeds, uint32_t *perm, bool sort, cudaStream_t s);
 

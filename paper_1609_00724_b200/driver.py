@@ -51,3 +51,47 @@ def adaptive_map(field, lattice, seeds0, params_L, params_LQ, n_levels: int, p: 
     res["steps_by_mode"] = acc
     res["total_steps"] = acc.sum(0, keepdim=True)
     return res
+
+
+def hilbert_map(lattice, R: int, thr: float, passes: int, shift: int, trace_fn, *, stream=None):
+    """The paper's own refinement loop (reading A17): orchestration only, every step is a
+    libqsl call.  Level-0 samples ordered along the Hilbert curve; per pass a refinement on the curve (a new sample halfway
+    along the curve wherever the field-line length of two successive samples differs by more than `thr`) and, if
+    `shift` != 0, the same on the curve shifted by `shift` fine cells, after which the samples go back to the original
+    order.  trace_fn(seeds CUDA float64 (m, 3)) -> (L, Q), CUDA float64 (m,) each - e.g. a closure over qsl_trace.
+
+    Returns dict(keys int64 (n,), coords int32 (n, ndim), L, Q, counts): the samples in curve order and the number of
+    samples after level 0 and after every (sub-)pass.  Feed keys and Q to qsl_hilbert_convert for the rectilinear map.
+    """
+    nd = int(lattice.ndim)
+    bits = B.qsl_hilbert_bits(lattice, R)
+    coords, seeds = B.qsl_hilbert_level0(lattice, R, stream=stream)
+    keys = B.qsl_hilbert_keys(coords, bits, 0, stream=stream)
+    perm = B.qsl_sort_keys64(keys, bits * nd, stream=stream)
+    coords = B.qsl_gather(perm, coords, stream=stream)
+    seeds = B.qsl_gather(perm, seeds, stream=stream)
+    L, Q = trace_fn(seeds)
+    counts = [int(keys.numel())]
+    for _ in range(passes):
+        for sh in ((0, shift) if shift else (0,)):
+            if sh:
+                ks = B.qsl_hilbert_keys(coords, bits + 1, sh, stream=stream)
+                perm = B.qsl_sort_keys64(ks, (bits + 1) * nd, stream=stream)
+                keys, coords, L, Q = (B.qsl_gather(perm, t, stream=stream) for t in (keys, coords, L, Q))
+            else:
+                ks = keys
+            left, nc, ns = B.qsl_hilbert_refine(lattice, R, sh, ks, L, thr, stream=stream)
+            if left.numel():
+                nL, nQ = trace_fn(ns.contiguous())
+                nk = B.qsl_hilbert_keys(nc.contiguous(), bits, 0, stream=stream)
+                keys = B.qsl_hilbert_merge(left, keys, nk, stream=stream)
+                coords = B.qsl_hilbert_merge(left, coords, nc.contiguous(), stream=stream)
+                L = B.qsl_hilbert_merge(left, L, nL.contiguous(), stream=stream)
+                Q = B.qsl_hilbert_merge(left, Q, nQ.contiguous(), stream=stream)
+            if sh:
+                kk = keys.clone()
+                perm = B.qsl_sort_keys64(kk, bits * nd, stream=stream)
+                coords, L, Q = (B.qsl_gather(perm, t, stream=stream) for t in (coords, L, Q))
+                keys = kk
+            counts.append(int(keys.numel()))
+    return dict(keys=keys, coords=coords, L=L, Q=Q, counts=counts)
