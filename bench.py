@@ -179,6 +179,10 @@ def workload_config(cfg, args, **extra):
          "trace_mode": "L+Q" if cfg["mode"] == 1 else "L", "refine_levels": int(cfg["levels"]),
          "step_rule": "RK4, h = 0.25 x smallest cell edge", "parallelism": "replicas x%d" % args.gpus,
          "l2": "flushed between timed steps (256 MiB write)"}
+    if int(cfg["levels"]) > 0:
+        c["refine"] = ("hilbert: length jump > %g between successive samples along the Hilbert curve, %d passes + shifted "
+                       "curve (shift %d)" % (args.hilbert_thr, int(lat.ndim) * int(cfg["levels"]), args.hilbert_shift)
+                       if getattr(args, "refine", "fledge") == "hilbert" else "fledge: FLEDGE > 95th percentile, 2x cells per level")
     c.update(extra)
     return c
 
@@ -205,6 +209,11 @@ def main():
     ap.add_argument("--arith", default="f64", choices=["f64", "f32"],
                     help="arithmetic of the integrator; f32 = QSL_ARITH_F32 throughput mode (fp32-sampled workloads only; "
                          "parity is gated in f64, DESIGN.md reading A6)")
+    ap.add_argument("--refine", default="fledge", choices=["fledge", "hilbert"],
+                    help="refinement scheme of cfg3 / cfg5: FLEDGE percentile + 2x cells (BASELINE.json configs), or the paper's "
+                         "own Hilbert-curve mid-point insertion on length jumps (PAPER.md:194-206; DESIGN.md reading A17)")
+    ap.add_argument("--hilbert-thr", type=float, default=0.05, help="field-line-length jump threshold of --refine hilbert")
+    ap.add_argument("--hilbert-shift", type=int, default=5, help="shift of the second curve in fine cells (0 = no shifted pass)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -259,8 +268,36 @@ def main():
             two = torch.zeros(2, dtype=torch.int64, device="cuda")
             two[mode:mode + 1] = tot
             return n, two
+        if hilbert:
+            r, acc = hilbert_step()
+            return r["counts"][-1], acc
         r = qsl.adaptive_map(field, lat, seeds, pL, pLQ, levels, cfg["p"])
         return n + sum(int(s.shape[0]) for s in r["seeds"][1:]), r["steps_by_mode"]
+
+    hilbert = args.refine == "hilbert" and levels > 0
+    hstate = {}
+
+    def hilbert_step():
+        """The paper's loop: level 0 L-only in curve order, then ndim x levels passes (each halves the key distance) on
+        the curve and on the shifted curve, new samples traced with Q; then the converter to the finest lattice."""
+        acc = torch.zeros(2, dtype=torch.int64, device="cuda")
+        calls = [0]
+
+        def tf(sd):
+            calls[0] += 1
+            if calls[0] == 1:
+                o = qsl.qsl_trace(field, sd, pL, outputs=("L",), total_steps=tot)
+                acc[0:1] += tot
+                return o["L"], torch.full_like(o["L"], float("nan"))
+            o = qsl.qsl_trace(field, sd, pLQ, outputs=("L", "q_perp"), total_steps=tot)
+            acc[1:2] += tot
+            return o["L"], o["q_perp"]
+
+        r = qsl.hilbert_map(lat, levels, args.hilbert_thr, int(lat.ndim) * levels, args.hilbert_shift, tf)
+        # the converter output at the finest lattice of cfg3 is 4.3 GB, of cfg5 69 GB: convert to level min(levels, 2)
+        hstate["map"] = qsl.qsl_hilbert_convert(lat, levels, min(levels, 2), r["keys"], r["Q"])
+        hstate["r"] = r
+        return r, acc
 
     host_out = {}
 
@@ -270,6 +307,10 @@ def main():
         if levels == 0:
             res = qsl.qsl_trace(field, d, pLQ if mode == 1 else pL, outputs=outs, out=out_bufs, total_steps=tot)
             results = [res[k] for k in outs]
+        elif hilbert:
+            # level-0 seeds are generated on the device by qsl_hilbert_level0: the host supplies the lattice only
+            r, _ = hilbert_step()
+            results = [r["keys"], r["L"], r["Q"], hstate["map"]]
         else:
             r = qsl.adaptive_map(field, lat, d, pL, pLQ, levels, cfg["p"])
             results = [r["L0"], r["S0"]]
