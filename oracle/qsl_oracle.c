@@ -77,10 +77,107 @@ static void locate_axis(const orc_field *F, int d, double x, int *i_out, double 
 /* PAPER.md:95 (eq. 3): B^(x) = sum_v B^{v+c} f_v(x - x_c; h_c); PAPER.md:101-107 (eq. 4): trilinear kernels
  * f_{abc} = w_a(x0/h0) w_b(x1/h1) w_c(x2/h2), w_0(t) = 1-t, w_1(t) = t.  PAPER.md:123, 137: the gradient acts
  * only on the kernels and is taken analytically: d w_0/dx = -1/h, d w_1/dx = +1/h.                         */
+static void finish_evaluate(const orc_field *F, const double val[4], double grad[4][3], double b[3], double J[9], double *m)
+{
+    if (F->interp_mode == ORC_NORMALIZE_FIRST) {
+        /* the interpolant of the pre-normalised samples, "not guaranteed to be a unit vector" (PAPER.md:178) */
+        for (int c = 0; c < 3; ++c) { b[c] = val[c]; for (int d = 0; d < 3; ++d) J[c * 3 + d] = grad[c][d]; }
+        *m = val[3];
+    } else {
+        /* reading A2: interpolate B, then normalise: b = B/|B|, J = (G - u (u^T G))/|B| */
+        const double n = sqrt((val[0] * val[0] + val[1] * val[1]) + val[2] * val[2]);
+        if (n < 1e-300) { for (int c = 0; c < 3; ++c) b[c] = 0.0; for (int q = 0; q < 9; ++q) J[q] = 0.0; *m = 0.0; }
+        else {
+            double u[3] = { val[0] / n, val[1] / n, val[2] / n };
+            for (int d = 0; d < 3; ++d) {
+                const double uG = (u[0] * grad[0][d] + u[1] * grad[1][d]) + u[2] * grad[2][d];
+                for (int c = 0; c < 3; ++c) J[c * 3 + d] = (grad[c][d] - u[c] * uG) / n;
+            }
+            for (int c = 0; c < 3; ++c) b[c] = u[c];
+            *m = n;
+        }
+    }
+}
+
+/* "The available interpolation schemes are trilinear, triquadratic (Dodgson 1997) and tricubic (Keys
+ * 1981) ... The interpolation kernels cover 8, 27, or 64 vertices neighboring that cell"; eq. (3): the kernels are
+ * functions of (x - x_c)/h_c of the cell containing x, whatever the spacing of the neighbouring cells.  Reading A18:
+ *  tricubic     Keys' cubic convolution (a = -1/2) on the nodes i-1 .. i+2 of each axis, t = (x - x_i)/h_i:
+ *               w = ((-t^3 + 2t^2 - t)/2, (3t^3 - 5t^2 + 2)/2, (-3t^3 + 4t^2 + t)/2, (t^3 - t^2)/2);
+ *               a node outside the grid takes Keys' boundary value f_-1 = 3 f_0 - 3 f_1 + f_2 (mirrored at the top);
+ *  triquadratic Dodgson's interpolating quadratic (r = 1) on the node j nearest to x (t >= 1/2 -> j = i + 1) and its
+ *               two neighbours, s = t - (j - i): w = (s^2 - s/2, 1 - 2 s^2, s^2 + s/2);
+ *               a node outside the grid takes the linear extrapolation f_-1 = 2 f_0 - f_1 (mirrored at the top).
+ * The gradient acts on the kernels only: d w/dx = w'(t)/h.  Returns the number of stencil nodes. */
+static int axis_stencil(int order, int n, int i, double t, double h, int idx[4], double w[4], double dw[4])
+{
+    if (order == ORC_TRICUBIC) {
+        const double t2 = t * t, t3 = t2 * t;
+        w[0] = 0.5 * ((-t3 + 2.0 * t2) - t);        dw[0] = 0.5 * ((-3.0 * t2 + 4.0 * t) - 1.0);
+        w[1] = 0.5 * ((3.0 * t3 - 5.0 * t2) + 2.0); dw[1] = 0.5 * (9.0 * t2 - 10.0 * t);
+        w[2] = 0.5 * ((-3.0 * t3 + 4.0 * t2) + t);  dw[2] = 0.5 * ((-9.0 * t2 + 8.0 * t) + 1.0);
+        w[3] = 0.5 * (t3 - t2);                     dw[3] = 0.5 * (3.0 * t2 - 2.0 * t);
+        for (int k = 0; k < 4; ++k) { idx[k] = i - 1 + k; dw[k] /= h; }
+        if (idx[0] < 0) {                            /* f_-1 = 3 f_0 - 3 f_1 + f_2 */
+            w[1] += 3.0 * w[0]; w[2] -= 3.0 * w[0]; w[3] += w[0]; w[0] = 0.0;
+            dw[1] += 3.0 * dw[0]; dw[2] -= 3.0 * dw[0]; dw[3] += dw[0]; dw[0] = 0.0;
+            idx[0] = 0;
+        }
+        if (idx[3] > n - 1) {                        /* f_n = 3 f_{n-1} - 3 f_{n-2} + f_{n-3} */
+            w[2] += 3.0 * w[3]; w[1] -= 3.0 * w[3]; w[0] += w[3]; w[3] = 0.0;
+            dw[2] += 3.0 * dw[3]; dw[1] -= 3.0 * dw[3]; dw[0] += dw[3]; dw[3] = 0.0;
+            idx[3] = n - 1;
+        }
+        return 4;
+    }
+    /* ORC_TRIQUADRATIC */
+    const int up = t >= 0.5 ? 1 : 0;
+    const int j = i + up;
+    const double s = t - (double)up;
+    w[0] = s * s - 0.5 * s;   dw[0] = (2.0 * s - 0.5) / h;
+    w[1] = 1.0 - 2.0 * s * s; dw[1] = (-4.0 * s) / h;
+    w[2] = s * s + 0.5 * s;   dw[2] = (2.0 * s + 0.5) / h;
+    for (int k = 0; k < 3; ++k) idx[k] = j - 1 + k;
+    if (idx[0] < 0) {                                /* f_-1 = 2 f_0 - f_1 */
+        w[1] += 2.0 * w[0]; w[2] -= w[0]; w[0] = 0.0;
+        dw[1] += 2.0 * dw[0]; dw[2] -= dw[0]; dw[0] = 0.0;
+        idx[0] = 0;
+    }
+    if (idx[2] > n - 1) {                            /* f_n = 2 f_{n-1} - f_{n-2} */
+        w[1] += 2.0 * w[2]; w[0] -= w[2]; w[2] = 0.0;
+        dw[1] += 2.0 * dw[2]; dw[0] -= dw[2]; dw[2] = 0.0;
+        idx[2] = n - 1;
+    }
+    return 3;
+}
+
 void orc_evaluate(const orc_field *F, const double x[3], double b[3], double J[9], double *m, double hc[3])
 {
     int i[3]; double t[3], h[3];
     for (int d = 0; d < 3; ++d) locate_axis(F, d, x[d], &i[d], &t[d], &h[d]);
+    if (F->order == ORC_TRIQUADRATIC || F->order == ORC_TRICUBIC) {
+        int idx[3][4], cnt[3]; double ww[3][4], dww[3][4];
+        const int nn[3] = { F->nx, F->ny, F->nz };
+        for (int d = 0; d < 3; ++d) cnt[d] = axis_stencil(F->order, nn[d], i[d], t[d], h[d], idx[d], ww[d], dww[d]);
+        double val[4] = { 0, 0, 0, 0 }, grad[4][3] = { { 0 } };
+        for (int c = 0; c < cnt[2]; ++c)
+            for (int bb = 0; bb < cnt[1]; ++bb)
+                for (int a = 0; a < cnt[0]; ++a) {
+                    const long long p = ((long long)idx[2][c] * F->ny + idx[1][bb]) * F->nx + idx[0][a];
+                    const double *s = F->packed + 4 * p;
+                    const double f = ww[0][a] * ww[1][bb] * ww[2][c];
+                    const double f0 = dww[0][a] * ww[1][bb] * ww[2][c];
+                    const double f1 = ww[0][a] * dww[1][bb] * ww[2][c];
+                    const double f2 = ww[0][a] * ww[1][bb] * dww[2][c];
+                    for (int q = 0; q < 4; ++q) {
+                        val[q] += s[q] * f;
+                        grad[q][0] += s[q] * f0; grad[q][1] += s[q] * f1; grad[q][2] += s[q] * f2;
+                    }
+                }
+        finish_evaluate(F, val, grad, b, J, m);
+        if (hc) { hc[0] = h[0]; hc[1] = h[1]; hc[2] = h[2]; }
+        return;
+    }
     double w[3][2], dw[3][2];
     for (int d = 0; d < 3; ++d) {
         w[d][0] = 1.0 - t[d]; w[d][1] = t[d];
@@ -101,24 +198,7 @@ void orc_evaluate(const orc_field *F, const double x[3], double b[3], double J[9
                     grad[q][0] += s[q] * f0; grad[q][1] += s[q] * f1; grad[q][2] += s[q] * f2;
                 }
             }
-    if (F->interp_mode == ORC_NORMALIZE_FIRST) {
-        /* the interpolant of the pre-normalised samples, "not guaranteed to be a unit vector" (PAPER.md:178) */
-        for (int c = 0; c < 3; ++c) { b[c] = val[c]; for (int d = 0; d < 3; ++d) J[c * 3 + d] = grad[c][d]; }
-        *m = val[3];
-    } else {
-        /* reading A2: interpolate B, then normalise: b = B/|B|, J = (G - u (u^T G))/|B| */
-        const double n = sqrt((val[0] * val[0] + val[1] * val[1]) + val[2] * val[2]);
-        if (n < 1e-300) { for (int c = 0; c < 3; ++c) b[c] = 0.0; for (int q = 0; q < 9; ++q) J[q] = 0.0; *m = 0.0; }
-        else {
-            double u[3] = { val[0] / n, val[1] / n, val[2] / n };
-            for (int d = 0; d < 3; ++d) {
-                const double uG = (u[0] * grad[0][d] + u[1] * grad[1][d]) + u[2] * grad[2][d];
-                for (int c = 0; c < 3; ++c) J[c * 3 + d] = (grad[c][d] - u[c] * uG) / n;
-            }
-            for (int c = 0; c < 3; ++c) b[c] = u[c];
-            *m = n;
-        }
-    }
+    finish_evaluate(F, val, grad, b, J, m);
     if (hc) { hc[0] = h[0]; hc[1] = h[1]; hc[2] = h[2]; }
 }
 
