@@ -41,6 +41,7 @@ enum { QSL_RK4 = 0, QSL_EULER = 1, QSL_CK45 = 2 };       /* PAPER.md:141; RK4: B
 enum { QSL_TRACE_L = 0, QSL_TRACE_LQ = 1 };              /* L only (FLEDGE pass) | L and Q                        */
 enum { QSL_LAYOUT_CELL_TABLE = 0, QSL_LAYOUT_NODES_ONLY = 1,    /* what qsl_field_create keeps in HBM (see qsl_grid_desc) */
        QSL_LAYOUT_CELL_TABLE_F32 = 2, QSL_LAYOUT_CELL_TABLES_BOTH = 3 };
+enum { QSL_TRILINEAR = 0, QSL_TRIQUADRATIC = 2, QSL_TRICUBIC = 3 };   /* interpolation scheme (reading A18) */
 enum { QSL_ARITH_F64 = 0, QSL_ARITH_F32 = 1 };           /* arithmetic of the integrator (F32 only with F32 samples) */
 
 /* status bits of qsl_trace_out.status */
@@ -78,6 +79,11 @@ typedef struct {
                                     the table of QSL_ARITH_F32; fp32 samples on a uniform grid only (else QSL_EINVAL);
                                     QSL_ARITH_F64 traces of such a field run the corner kernel.
                                     QSL_LAYOUT_CELL_TABLES_BOTH: the fp64 and the fp32 table                          */
+    int interp_order;            /* QSL_TRILINEAR (0, default; eq. 3-4) | QSL_TRIQUADRATIC (Dodgson 1997, 27
+                                    vertices) | QSL_TRICUBIC (Keys 1981, 64 vertices): PAPER.md:91-93, gradients taken
+                                    analytically on the kernels (:123, :137).  The higher orders need >= 3 / >= 4 nodes per
+                                    axis and QSL_NORMALIZE_FIRST (else QSL_EINVAL), keep the node samples only (layout is
+                                    ignored) and are traced by the gather kernel in fp64 with QSL_RK4 / QSL_EULER         */
 } qsl_grid_desc;
 
 /* Packs the three component cubes (DEVICE, fp64, nx*ny*nz each) into one AoS array of (b^x, b^y, b^z, |B|) samples

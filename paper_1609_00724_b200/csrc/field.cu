@@ -164,8 +164,14 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     if (d->sample_type != QSL_F32 && d->sample_type != QSL_F64) return QSL_EINVAL;
     if (d->interp_mode != QSL_NORMALIZE_FIRST && d->interp_mode != QSL_INTERP_FIRST) return QSL_EINVAL;
     if (d->layout < QSL_LAYOUT_CELL_TABLE || d->layout > QSL_LAYOUT_CELL_TABLES_BOTH) return QSL_EINVAL;
-    const bool want64 = d->layout == QSL_LAYOUT_CELL_TABLE || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH;
-    const bool want32 = d->layout == QSL_LAYOUT_CELL_TABLE_F32 || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH;
+    if (d->interp_order != QSL_TRILINEAR && d->interp_order != QSL_TRIQUADRATIC && d->interp_order != QSL_TRICUBIC) return QSL_EINVAL;
+    const bool ho = d->interp_order != QSL_TRILINEAR;     // higher-order kernels: node samples only, paper mode only
+    if (ho) {
+        const int need = d->interp_order == QSL_TRICUBIC ? 4 : 3;
+        if (d->nx < need || d->ny < need || d->nz < need || d->interp_mode != QSL_NORMALIZE_FIRST) return QSL_EINVAL;
+    }
+    const bool want64 = !ho && (d->layout == QSL_LAYOUT_CELL_TABLE || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH);
+    const bool want32 = !ho && (d->layout == QSL_LAYOUT_CELL_TABLE_F32 || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH);
     if (want32 && (d->sample_type != QSL_F32 || d->stretched)) return QSL_EINVAL;   // fp32 arithmetic: fp32 samples, uniform grid
     const long long n = (long long)d->nx * d->ny * d->nz;
     if (n >= (1ll << 31)) return QSL_ERANGE;   // node index is 32-bit inside the gather
@@ -200,6 +206,7 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     v.nx = d->nx; v.ny = d->ny; v.nz = d->nz;
     v.stretched = d->stretched ? 1 : 0;
     v.interp_mode = d->interp_mode;
+    v.order = ho ? d->interp_order : 1;
     for (int a = 0; a < 3; ++a) {
         // node coordinates: given (stretched) or lo + i*h (uniform), always resident for the locate of the stretched path
         double *tmp = new (std::nothrow) double[dims[a]];

@@ -34,6 +34,7 @@ struct FieldView {
     int nx, ny, nz;
     int stretched;
     int interp_mode;
+    int order;                // interpolation order: 1 trilinear, 2 triquadratic (Dodgson), 3 tricubic (Keys)
     double lo[3], hi[3];
     double h[3];              // uniform spacing (hi - lo)/(n - 1)
     const double *axis[3];    // device node coordinates (always present)

@@ -104,11 +104,146 @@ __device__ __forceinline__ void trilinear(double c000, double c100, double c010,
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Higher-order interpolation ("trilinear, triquadratic (Dodgson 1997) and tricubic
+// (Keys 1981) ... 8, 27, or 64 vertices"; eq. (3): kernels f_v(x - x_c; h_c) in the units of the cell containing x;
+// :123, :137: the gradient is taken analytically on the kernels).  Reading A18 of DESIGN.md:
+//   ORDER 3  Keys' cubic convolution (a = -1/2) on the nodes i-1 .. i+2 of each axis, t = (x - x_i)/h_i; a node outside
+//            the grid takes Keys' boundary value f_-1 = 3 f_0 - 3 f_1 + f_2 (mirrored at the upper end);
+//   ORDER 2  Dodgson's interpolating quadratic (r = 1) on the node nearest to x (t >= 1/2 -> i + 1) and its two
+//            neighbours, s = t - (j - i); outside the grid the linear extrapolation f_-1 = 2 f_0 - f_1.
+// Per axis: node indices (clamped; a folded node has weight 0), weights and d weight / dx.
+template <int ORDER>
+__device__ __forceinline__ void axis_stencil(int n, int i, double t, double inv_h, int idx[ORDER + 1], double w[ORDER + 1],
+                                             double dw[ORDER + 1])
+{
+    if (ORDER == 3) {
+        const double t2 = t * t, t3 = t2 * t;
+        w[0] = 0.5 * ((-t3 + 2.0 * t2) - t);        dw[0] = 0.5 * ((-3.0 * t2 + 4.0 * t) - 1.0);
+        w[1] = 0.5 * ((3.0 * t3 - 5.0 * t2) + 2.0); dw[1] = 0.5 * (9.0 * t2 - 10.0 * t);
+        w[2] = 0.5 * ((-3.0 * t3 + 4.0 * t2) + t);  dw[2] = 0.5 * ((-9.0 * t2 + 8.0 * t) + 1.0);
+        w[ORDER] = 0.5 * (t3 - t2);                 dw[ORDER] = 0.5 * (3.0 * t2 - 2.0 * t);
+#pragma unroll
+        for (int k = 0; k <= ORDER; ++k) { idx[k] = i - 1 + k; dw[k] *= inv_h; }
+        if (idx[0] < 0) {
+            w[1] += 3.0 * w[0]; w[2] -= 3.0 * w[0]; w[ORDER] += w[0]; w[0] = 0.0;
+            dw[1] += 3.0 * dw[0]; dw[2] -= 3.0 * dw[0]; dw[ORDER] += dw[0]; dw[0] = 0.0;
+            idx[0] = 0;
+        }
+        if (idx[ORDER] > n - 1) {
+            w[2] += 3.0 * w[ORDER]; w[1] -= 3.0 * w[ORDER]; w[0] += w[ORDER]; w[ORDER] = 0.0;
+            dw[2] += 3.0 * dw[ORDER]; dw[1] -= 3.0 * dw[ORDER]; dw[0] += dw[ORDER]; dw[ORDER] = 0.0;
+            idx[ORDER] = n - 1;
+        }
+    } else {
+        const int up = t >= 0.5 ? 1 : 0;
+        const int j = i + up;
+        const double s = t - (double)up;
+        w[0] = s * s - 0.5 * s;   dw[0] = (2.0 * s - 0.5) * inv_h;
+        w[1] = 1.0 - 2.0 * s * s; dw[1] = (-4.0 * s) * inv_h;
+        w[2] = s * s + 0.5 * s;   dw[2] = (2.0 * s + 0.5) * inv_h;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) idx[k] = j - 1 + k;
+        if (idx[0] < 0) {
+            w[1] += 2.0 * w[0]; w[2] -= w[0]; w[0] = 0.0;
+            dw[1] += 2.0 * dw[0]; dw[2] -= dw[0]; dw[0] = 0.0;
+            idx[0] = 0;
+        }
+        if (idx[2] > n - 1) {
+            w[1] += 2.0 * w[2]; w[0] -= w[2]; w[2] = 0.0;
+            dw[1] += 2.0 * dw[2]; dw[0] -= dw[2]; dw[2] = 0.0;
+            idx[2] = n - 1;
+        }
+    }
+}
+
+// Separable tensor-product sum over the (ORDER + 1)^3 stencil: x innermost (value and d/dx of every component), then y,
+// then z.  val[4] = (v0, v1, v2, |B| sample), g[c*3 + d] = d v_c / d x_d.
+template <typename S, bool STRETCHED, bool WITH_J, bool WITH_M, int ORDER>
+__device__ __forceinline__ void interpolate_ho(const TraceArgs &A, const double x[3], double val[4], double g[9], double &hmin)
+{
+    using S4 = typename Sample4<S>::type;
+    constexpr int NS = ORDER + 1;
+    int i, j, k; double tx, ty, tz, ihx, ihy, ihz, hx, hy, hz;
+    locate<STRETCHED>(A, 0, A.fv.nx, x[0], i, tx, ihx, hx);
+    locate<STRETCHED>(A, 1, A.fv.ny, x[1], j, ty, ihy, hy);
+    locate<STRETCHED>(A, 2, A.fv.nz, x[2], k, tz, ihz, hz);
+    hmin = fmin(hx, fmin(hy, hz));
+    int ix[NS], iy[NS], iz[NS];
+    double wx[NS], dwx[NS], wy[NS], dwy[NS], wz[NS], dwz[NS];
+    axis_stencil<ORDER>(A.fv.nx, i, tx, ihx, ix, wx, dwx);
+    axis_stencil<ORDER>(A.fv.ny, j, ty, ihy, iy, wy, dwy);
+    axis_stencil<ORDER>(A.fv.nz, k, tz, ihz, iz, wz, dwz);
+    constexpr int NC = WITH_M ? 4 : 3;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) val[q] = 0.0;
+#pragma unroll
+    for (int q = 0; q < 9; ++q) g[q] = 0.0;
+    const S4 *__restrict__ base = (const S4 *)A.fv.samples;
+#pragma unroll
+    for (int c = 0; c < NS; ++c) {
+        double vy[NC], gxy[3], gyy[3];          // sums over the (x, y) plane c: value, d/dx, d/dy
+#pragma unroll
+        for (int q = 0; q < NC; ++q) vy[q] = 0.0;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) { gxy[q] = 0.0; gyy[q] = 0.0; }
+#pragma unroll
+        for (int b = 0; b < NS; ++b) {
+            const S4 *__restrict__ row = base + ((size_t)iz[c] * A.fv.ny + iy[b]) * A.fv.nx;
+            double vx[NC], gx[3];
+#pragma unroll
+            for (int q = 0; q < NC; ++q) vx[q] = 0.0;
+#pragma unroll
+            for (int q = 0; q < 3; ++q) gx[q] = 0.0;
+#pragma unroll
+            for (int a = 0; a < NS; ++a) {
+                const S4 sm = load_sample(row + ix[a]);
+                const double sv[4] = { (double)sm.x, (double)sm.y, (double)sm.z, (double)sm.w };
+#pragma unroll
+                for (int q = 0; q < NC; ++q) vx[q] = fma(wx[a], sv[q], vx[q]);
+                if (WITH_J) {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) gx[q] = fma(dwx[a], sv[q], gx[q]);
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < NC; ++q) vy[q] = fma(wy[b], vx[q], vy[q]);
+            if (WITH_J) {
+#pragma unroll
+                for (int q = 0; q < 3; ++q) { gxy[q] = fma(wy[b], gx[q], gxy[q]); gyy[q] = fma(dwy[b], vx[q], gyy[q]); }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < NC; ++q) val[q] = fma(wz[c], vy[q], val[q]);
+        if (WITH_J) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                g[q * 3 + 0] = fma(wz[c], gxy[q], g[q * 3 + 0]);
+                g[q * 3 + 1] = fma(wz[c], gyy[q], g[q * 3 + 1]);
+                g[q * 3 + 2] = fma(dwz[c], vy[q], g[q * 3 + 2]);
+            }
+        }
+    }
+}
+
 // Evaluate(x) -> b[3], J[9] (J[c*3+d] = d b_c / d x_d), optionally m = |B| and the cell size (O1 of DESIGN.md).
-template <typename S, bool STRETCHED, bool INTERP, bool WITH_J, bool WITH_M>
+template <typename S, bool STRETCHED, bool INTERP, bool WITH_J, bool WITH_M, int ORDER = 1>
 __device__ __forceinline__ void evaluate(const TraceArgs &A, const double x[3], double b[3], double J[9], double &m, double &hmin)
 {
     using S4 = typename Sample4<S>::type;
+    if (ORDER != 1) {
+        // paper mode only (NORMALIZE_FIRST): the interpolant of the pre-normalised samples is used as it is
+        double val[4], gg[9];
+        interpolate_ho<S, STRETCHED, WITH_J, WITH_M, ORDER == 1 ? 2 : ORDER>(A, x, val, gg, hmin);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) b[c] = val[c];
+        if (WITH_J) {
+#pragma unroll
+            for (int q = 0; q < 9; ++q) J[q] = gg[q];
+        }
+        m = val[3];
+        return;
+    }
     int i, j, k; double tx, ty, tz, ihx, ihy, ihz, hx, hy, hz;
     locate<STRETCHED>(A, 0, A.fv.nx, x[0], i, tx, ihx, hx);
     locate<STRETCHED>(A, 1, A.fv.ny, x[1], j, ty, ihy, hy);
@@ -186,7 +321,7 @@ __device__ __forceinline__ bool inside_box(const TraceArgs &A, const double x[3]
 //                field at the trial end (evaluated as a "5th stage" through the same evaluate call site)
 //   phase 4      final step of size hp, snap onto the face, done
 // NV = 9 with deviation vectors (QSL_TRACE_LQ), 3 without (QSL_TRACE_L): x and L are bit-identical in both modes.
-template <typename S, bool DEV, bool STRETCHED, bool INTERP>
+template <typename S, bool DEV, bool STRETCHED, bool INTERP, int ORDER = 1>
 struct LineState {
     static constexpr int NV = DEV ? 9 : 3;
     double y[NV];        // x, delta1, delta2
@@ -210,7 +345,7 @@ struct LineState {
         for (int c = 0; c < NV; ++c) y[c] = c < 3 ? x[c] : 0.0;
         if (!inside_box(A, x)) { finish(A, REC_SEED_OUTSIDE); return false; }
         double b[3], J[9], m, hmin;
-        evaluate<S, STRETCHED, INTERP, false, false>(A, x, b, J, m, hmin);
+        evaluate<S, STRETCHED, INTERP, false, false, ORDER>(A, x, b, J, m, hmin);
         const double nb = norm3(b);
         if (!(nb >= A.null_eps)) { finish(A, REC_NULL_AT_SEED); return false; }
         if (DEV) {
@@ -260,7 +395,7 @@ struct LineState {
 #pragma unroll 1
         for (int st = 0;; ++st) {
             double b[3], J[9], m, hmin;
-            evaluate<S, STRETCHED, INTERP, DEV, false>(A, ys, b, J, m, hmin);
+            evaluate<S, STRETCHED, INTERP, DEV, false, ORDER>(A, ys, b, J, m, hmin);
             const double bn = norm3(b);
             if (st == 0 && phase == 0) {
                 // O4: stall / caps are tested on k1 before the step; h from the cell containing x
@@ -355,10 +490,10 @@ struct LineState {
 // Kernels.  REFILL = false: one work item per thread (grid covers 2n items).  REFILL = true: persistent warps, a lane
 // whose line ended pops the next item from a global counter (warp-aggregated atomic), so ragged line lengths do not
 // idle lanes (north_star, "persistent trace kernel with a global work queue that refills lanes as lines terminate").
-template <typename S, bool DEV, bool STRETCHED, bool INTERP, bool REFILL>
+template <typename S, bool DEV, bool STRETCHED, bool INTERP, bool REFILL, int ORDER = 1>
 __global__ void __launch_bounds__(128) trace_kernel(const TraceArgs A)
 {
-    LineState<S, DEV, STRETCHED, INTERP> ls;
+    LineState<S, DEV, STRETCHED, INTERP, ORDER> ls;
     const long long n_items = 2 * A.n;
     unsigned long long my_steps = 0;
     if (!REFILL) {
@@ -404,13 +539,13 @@ struct EpilogueArgs {
 
 struct EndProj { double a[3], b[3], m; };
 
-template <typename S, bool STRETCHED, bool INTERP>
+template <typename S, bool STRETCHED, bool INTERP, int ORDER = 1>
 __device__ void project_end(const TraceArgs &A, const double *r, int face, bool bnd, EndProj &E)
 {
     // delta_perp = delta - B^(B^ . delta) with B^ re-normalised at the end point.
     // Reading A1 (bnd): slide along the field onto the end face instead, and weight by the normal field component.
     double b[3], J[9], m, hmin;
-    evaluate<S, STRETCHED, INTERP, false, true>(A, r, b, J, m, hmin);
+    evaluate<S, STRETCHED, INTERP, false, true, ORDER>(A, r, b, J, m, hmin);
     const double inv = 1.0 / norm3(b);
     const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
     const double *d1 = r + 3, *d2 = r + 6;
@@ -437,7 +572,7 @@ __device__ __forceinline__ double q_eq11(const EndProj &F, const EndProj &B, dou
     return (F.m * B.m) / (m0 * m0) * ((aF2 * bB2 + aB2 * bF2) - 2.0 * (abB * abF));
 }
 
-template <typename S, bool STRETCHED, bool INTERP>
+template <typename S, bool STRETCHED, bool INTERP, int ORDER = 1>
 __global__ void __launch_bounds__(128) epilogue_kernel(const EpilogueArgs E)
 {
     const TraceArgs &A = E.T;
@@ -501,16 +636,16 @@ __global__ void __launch_bounds__(128) epilogue_kernel(const EpilogueArgs E)
         // B_0 = |B| at the seed
         const double x0[3] = { A.seeds[3 * si], A.seeds[3 * si + 1], A.seeds[3 * si + 2] };
         double b0[3], J[9], m0, hmin;
-        evaluate<S, STRETCHED, INTERP, false, true>(A, x0, b0, J, m0, hmin);
+        evaluate<S, STRETCHED, INTERP, false, true, ORDER>(A, x0, b0, J, m0, hmin);
         EndProj PF, PB;
         if (O.q_perp) {
-            project_end<S, STRETCHED, INTERP>(A, rf, ff, false, PF);
-            project_end<S, STRETCHED, INTERP>(A, rb, fb, false, PB);
+            project_end<S, STRETCHED, INTERP, ORDER>(A, rf, ff, false, PF);
+            project_end<S, STRETCHED, INTERP, ORDER>(A, rb, fb, false, PB);
             O.q_perp[si] = q_eq11(PF, PB, m0);
         }
         if (O.q_bnd) {
-            project_end<S, STRETCHED, INTERP>(A, rf, ff, true, PF);
-            project_end<S, STRETCHED, INTERP>(A, rb, fb, true, PB);
+            project_end<S, STRETCHED, INTERP, ORDER>(A, rf, ff, true, PF);
+            project_end<S, STRETCHED, INTERP, ORDER>(A, rb, fb, true, PB);
             O.q_bnd[si] = q_eq11(PF, PB, m0);
         }
     }

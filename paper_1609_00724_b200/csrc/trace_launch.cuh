@@ -37,9 +37,48 @@ static cudaError_t launch_epilogue_variant(const EpilogueArgs &E, cudaStream_t s
     return cudaGetLastError();
 }
 
+// Higher-order interpolation (ORDER 2 / 3; paper mode NORMALIZE_FIRST only): always the persistent work-queue launch.
+template <typename S, bool DEV, bool STRETCHED, int ORDER>
+static cudaError_t launch_trace_ho_variant(const TraceArgs &A, cudaStream_t s)
+{
+    const long long n_items = 2 * A.n;
+    const int threads = 128;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<S, DEV, STRETCHED, false, true, ORDER>, threads, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    long long blocks = (long long)sm_count() * per_sm;
+    const long long need = (n_items + threads - 1) / threads;
+    if (blocks > need) blocks = need;
+    count_launch();
+    trace_kernel<S, DEV, STRETCHED, false, true, ORDER><<<(unsigned)blocks, threads, 0, s>>>(A);
+    return cudaGetLastError();
+}
+
+template <typename S, int ORDER>
+static cudaError_t launch_trace_ho(const TraceArgs &A, bool dev, cudaStream_t s)
+{
+    const bool st = A.fv.stretched != 0;
+    if (dev) return st ? launch_trace_ho_variant<S, true, true, ORDER>(A, s) : launch_trace_ho_variant<S, true, false, ORDER>(A, s);
+    return st ? launch_trace_ho_variant<S, false, true, ORDER>(A, s) : launch_trace_ho_variant<S, false, false, ORDER>(A, s);
+}
+
+template <typename S, int ORDER>
+static cudaError_t launch_epilogue_ho(const EpilogueArgs &E, cudaStream_t s)
+{
+    const int threads = 128;
+    const long long blocks = (E.T.n + threads - 1) / threads;
+    count_launch();
+    if (E.T.fv.stretched) epilogue_kernel<S, true, false, ORDER><<<(unsigned)blocks, threads, 0, s>>>(E);
+    else epilogue_kernel<S, false, false, ORDER><<<(unsigned)blocks, threads, 0, s>>>(E);
+    return cudaGetLastError();
+}
+
 template <typename S>
 cudaError_t launch_trace(const TraceArgs &A, bool dev, bool refill, cudaStream_t s)
 {
+    if (A.fv.order == 2) return launch_trace_ho<S, 2>(A, dev, s);
+    if (A.fv.order == 3) return launch_trace_ho<S, 3>(A, dev, s);
     const bool st = A.fv.stretched != 0, in = A.fv.interp_mode == QSL_INTERP_FIRST;
 #define QSL_DISPATCH(D, ST, IN) \
     if (dev == D && st == ST && in == IN) return launch_trace_variant<S, D, ST, IN>(A, refill, s);
@@ -52,6 +91,8 @@ cudaError_t launch_trace(const TraceArgs &A, bool dev, bool refill, cudaStream_t
 template <typename S>
 cudaError_t launch_epilogue(const EpilogueArgs &E, cudaStream_t s)
 {
+    if (E.T.fv.order == 2) return launch_epilogue_ho<S, 2>(E, s);
+    if (E.T.fv.order == 3) return launch_epilogue_ho<S, 3>(E, s);
     const bool st = E.T.fv.stretched != 0, in = E.T.fv.interp_mode == QSL_INTERP_FIRST;
     if (!st && !in) return launch_epilogue_variant<S, false, false>(E, s);
     if (!st && in) return launch_epilogue_variant<S, false, true>(E, s);
