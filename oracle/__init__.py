@@ -20,6 +20,7 @@ F32, F64 = 0, 1
 NORMALIZE_FIRST, INTERP_FIRST = 0, 1
 RK4, EULER, CK45 = 0, 1, 2
 TRILINEAR, TRIQUADRATIC, TRICUBIC = 1, 2, 3
+CARTESIAN, SPHERICAL = 0, 1
 TRACE_L, TRACE_LQ = 0, 1
 ST_SEED_OUTSIDE, ST_NULL_AT_SEED, ST_STALL_F, ST_STALL_B, ST_CAP_F, ST_CAP_B, ST_OPEN = 1, 2, 4, 8, 16, 32, 64
 
@@ -40,7 +41,7 @@ _dp = C.POINTER(C.c_double)
 class _Field(C.Structure):
     _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("stretched", C.c_int),
                 ("lo", C.c_double * 3), ("hi", C.c_double * 3),
-                ("xs", _dp), ("ys", _dp), ("zs", _dp), ("interp_mode", C.c_int), ("packed", _dp), ("order", C.c_int)]
+                ("xs", _dp), ("ys", _dp), ("zs", _dp), ("interp_mode", C.c_int), ("packed", _dp), ("order", C.c_int), ("geometry", C.c_int)]
 
 
 class _Params(C.Structure):
@@ -76,7 +77,7 @@ def _ptr(a, ty=C.c_double):
 class Field:
     """O0: packed field the oracle traces through.  `B` = (bx, by, bz) fp64 cubes of shape (nz, ny, nx)."""
 
-    def __init__(self, grid, B, sample_type=F64, interp_mode=NORMALIZE_FIRST, order=TRILINEAR):
+    def __init__(self, grid, B, sample_type=F64, interp_mode=NORMALIZE_FIRST, order=TRILINEAR, geometry=CARTESIAN):
         self.grid = grid
         bx, by, bz = (np.ascontiguousarray(a, dtype=np.float64).reshape(-1) for a in B)
         n = grid.nx * grid.ny * grid.nz
@@ -89,8 +90,9 @@ class Field:
         self._zs = np.ascontiguousarray(grid.zs, dtype=np.float64)
         self.c = _Field(grid.nx, grid.ny, grid.nz, int(bool(grid.stretched)),
                         (C.c_double * 3)(*grid.lo), (C.c_double * 3)(*grid.hi),
-                        _ptr(self._xs), _ptr(self._ys), _ptr(self._zs), interp_mode, _ptr(self.packed), int(order))
+                        _ptr(self._xs), _ptr(self._ys), _ptr(self._zs), interp_mode, _ptr(self.packed), int(order), int(geometry))
         self.order = int(order)
+        self.geometry = int(geometry)
         self.sample_type = sample_type
         self.interp_mode = interp_mode
 

@@ -209,23 +209,34 @@ static double dot3(const double a[3], const double b[3]) { return (a[0] * b[0] +
 /* State y = (x[3], delta1[3], delta2[3], L).  f(y) = (s b, s J delta1, s J delta2, |b|):
  * PAPER.md:79 (eq. 1) d x/d lambda = B^(x); PAPER.md:119 (eq. 5) d delta/d lambda = (delta . grad) B^;
  * reading A3: L = integral of |b_interp| d lambda (arc length of the numerical curve) as a 10th component. */
+/* Spherical geometry (reading A19): y = (phi, theta, r, delta phi, delta theta, delta r, ..., L), angles in radians,
+ * theta = latitude.  PAPER.md:83-85 (eq. 2): r cos(theta) phi' = B^_phi, r theta' = B^_theta, r' = B^_r.
+ * PAPER.md:125-135 (eq. 6, 7): r cos(theta) (delta phi)' = (delta u . grad_u) B^_phi, r (delta theta)' = (delta u . grad_u)
+ * B^_theta, (delta r)' = (delta u . grad_u) B^_r with grad_u = (d/dphi, d/dtheta, d/dr) acting on the interpolation kernels
+ * only - as printed, i.e. without the derivatives of the metric factors (fn. 8).                     */
+static void metric(const orc_field *F, const double y[10], double mf[3])
+{
+    if (F->geometry == ORC_SPHERICAL) { mf[0] = 1.0 / (y[2] * cos(y[1])); mf[1] = 1.0 / y[2]; mf[2] = 1.0; }
+    else { mf[0] = mf[1] = mf[2] = 1.0; }
+}
+
 static void rhs(const orc_field *F, int with_dev, double s, const double y[10], double dy[10], double *bnorm,
                 double hc[3])
 {
-    double b[3], J[9], m;
+    double b[3], J[9], m, mf[3];
     orc_evaluate(F, y, b, J, &m, hc);
-    for (int c = 0; c < 3; ++c) dy[c] = s * b[c];
+    metric(F, y, mf);
+    for (int c = 0; c < 3; ++c) dy[c] = s * b[c] * mf[c];
     for (int v = 0; v < 2; ++v) {
         const double *dl = y + 3 + 3 * v;
         for (int c = 0; c < 3; ++c)
-            dy[3 + 3 * v + c] = with_dev ? s * ((J[c * 3 + 0] * dl[0] + J[c * 3 + 1] * dl[1]) + J[c * 3 + 2] * dl[2]) : 0.0;
+            dy[3 + 3 * v + c] = with_dev ? s * ((J[c * 3 + 0] * dl[0] + J[c * 3 + 1] * dl[1]) + J[c * 3 + 2] * dl[2]) * mf[c] : 0.0;
     }
     dy[9] = norm3(b);
     if (bnorm) *bnorm = dy[9];
+    if (hc && F->geometry == ORC_SPHERICAL) { hc[0] *= y[2] * cos(y[1]); hc[1] *= y[2]; }   /* physical cell edges */
 }
 
-/* One step of size h from y, given k1 = f(y).  RK4 is the graded rule (BASELINE.json configs[0]: "fixed-step
- * RK4 with h=0.25 cell", reading A5); Euler is the paper's fixed-step scheme.           */
 /* Cash & Karp (1990) embedded pair, the scheme behind the paper's adaptive stepper: six stages,
  * nodes c, coupling a, 5th-order weights b5 (the propagated solution) and 4th-order weights b4 of the embedded
  * solution; y5 - y4 estimates the local error.  Written out as printed in the literature.                    */
@@ -363,7 +374,8 @@ static void trace_direction(const orc_field *F, const orc_trace_params *P, int w
             double yt[10], bt[3], Jt[9], mt;
             take_step(F, P, with_dev, s, y, k1, hp, yt);
             orc_evaluate(F, yt, bt, Jt, &mt, NULL);
-            const double g = s * bt[axis];
+            double mft[3]; metric(F, yt, mft);
+            const double g = s * bt[axis] * mft[axis];
             const double r = yt[axis] - bound;
             if (g != 0.0) {
                 double hn = hp - r / g;
@@ -392,7 +404,11 @@ static void project_end(const orc_field *F, const dir_result *R, int bnd, end_pr
     orc_evaluate(F, R->y, bE, J, &mE, NULL);
     const double nb = norm3(bE);
     const double u[3] = { bE[0] / nb, bE[1] / nb, bE[2] / nb };
-    const double *d1 = R->y + 3, *d2 = R->y + 6;
+    double d1[3], d2[3];
+    {   /* PAPER.md:156 (eq. 8): delta x_phi = r cos(theta) delta phi, delta x_theta = r delta theta, delta x_r = delta r */
+        double mf[3]; metric(F, R->y, mf);
+        for (int c = 0; c < 3; ++c) { d1[c] = R->y[3 + c] / mf[c]; d2[c] = R->y[6 + c] / mf[c]; }
+    }
     if (bnd && R->face != 255) {
         const int ax = R->face / 2;                    /* n_E = unit vector of that axis */
         const double un = u[ax];
@@ -457,6 +473,11 @@ static void trace_one(const orc_field *F, const orc_trace_params *P, const doubl
         for (int c = 0; c < 3; ++c) { const double a0 = a[c], b1 = bp[c]; a[c] = cs * a0 + sn * b1; bp[c] = cs * b1 - sn * a0; }
     }
     const int with_dev = P->mode == ORC_TRACE_LQ;
+    {   /* the pair is orthonormal in the orthonormal basis; the state carries coordinate deviations (eq. 8 inverted) */
+        double y00[10] = { seed[0], seed[1], seed[2] }, mf[3];
+        metric(F, y00, mf);
+        for (int c = 0; c < 3; ++c) { a[c] *= mf[c]; bp[c] *= mf[c]; }
+    }
     double y0[10] = { seed[0], seed[1], seed[2], a[0], a[1], a[2], bp[0], bp[1], bp[2], 0.0 };
     if (!with_dev) for (int c = 3; c < 9; ++c) y0[c] = 0.0;
     dir_result RF, RB;

@@ -21,6 +21,7 @@ extern "C" {
 
 enum { ORC_F32 = 0, ORC_F64 = 1 };
 enum { ORC_NORMALIZE_FIRST = 0, ORC_INTERP_FIRST = 1 };
+enum { ORC_CARTESIAN = 0, ORC_SPHERICAL = 1 };
 enum { ORC_TRILINEAR = 1, ORC_TRIQUADRATIC = 2, ORC_TRICUBIC = 3 };
 enum { ORC_RK4 = 0, ORC_EULER = 1, ORC_CK45 = 2 };   /* CK45: adaptive Cash-Karp 5(4) */
 enum { ORC_TRACE_L = 0, ORC_TRACE_LQ = 1 };
@@ -38,6 +39,8 @@ typedef struct {
     int interp_mode;           /* ORC_NORMALIZE_FIRST (paper) | ORC_INTERP_FIRST          */
     const double *packed;      /* n*4 doubles (v0,v1,v2,m): output of orc_field_pack                    */
     int order;                 /* 0 / ORC_TRILINEAR | ORC_TRIQUADRATIC | ORC_TRICUBIC (reading A18) */
+    int geometry;              /* ORC_CARTESIAN (0) | ORC_SPHERICAL: axes = (longitude phi, latitude theta, radius r),
+                                  components in the orthonormal basis (phi^, theta^, r^)  */
 } orc_field;
 
 typedef struct {
