@@ -42,6 +42,7 @@ enum { QSL_TRACE_L = 0, QSL_TRACE_LQ = 1 };              /* L only (FLEDGE pass)
 enum { QSL_LAYOUT_CELL_TABLE = 0, QSL_LAYOUT_NODES_ONLY = 1,    /* what qsl_field_create keeps in HBM (see qsl_grid_desc) */
        QSL_LAYOUT_CELL_TABLE_F32 = 2, QSL_LAYOUT_CELL_TABLES_BOTH = 3 };
 enum { QSL_TRILINEAR = 0, QSL_TRIQUADRATIC = 2, QSL_TRICUBIC = 3 };   /* interpolation scheme (reading A18) */
+enum { QSL_CARTESIAN = 0, QSL_SPHERICAL = 1 };                        /* geometry of the grid axes    */
 enum { QSL_ARITH_F64 = 0, QSL_ARITH_F32 = 1 };           /* arithmetic of the integrator (F32 only with F32 samples) */
 
 /* status bits of qsl_trace_out.status */
@@ -84,6 +85,13 @@ typedef struct {
                                     analytically on the kernels (:123, :137).  The higher orders need >= 3 / >= 4 nodes per
                                     axis and QSL_NORMALIZE_FIRST (else QSL_EINVAL), keep the node samples only (layout is
                                     ignored) and are traced by the gather kernel in fp64 with QSL_RK4 / QSL_EULER         */
+    int geometry;                /* QSL_CARTESIAN (0, default) | QSL_SPHERICAL: the axes are (longitude phi, latitude theta,
+                                    radius r), angles in radians, and bx, by, bz are the components in the orthonormal basis
+                                    (phi^, theta^, r^) (PAPER.md:83-87 eq. 2, :111).  Seeds, trace box and end points are
+                                    then (phi, theta, r); lines follow eq. (2), deviations eq. (6)-(7) as printed (without
+                                    the metric-derivative terms), Q uses eq. (8); dev_f / dev_b are coordinate
+                                    deviations.  Uniform axes, QSL_NORMALIZE_FIRST, QSL_TRILINEAR, fp64, RK4 / Euler only
+                                    (else QSL_EINVAL); node samples only, traced by the gather kernel                     */
 } qsl_grid_desc;
 
 /* Packs the three component cubes (DEVICE, fp64, nx*ny*nz each) into one AoS array of (b^x, b^y, b^z, |B|) samples

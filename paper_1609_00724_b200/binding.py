@@ -20,6 +20,7 @@ QSL_RK4, QSL_EULER, QSL_CK45 = 0, 1, 2
 QSL_TRACE_L, QSL_TRACE_LQ = 0, 1
 QSL_ARITH_F64, QSL_ARITH_F32 = 0, 1
 QSL_TRILINEAR, QSL_TRIQUADRATIC, QSL_TRICUBIC = 0, 2, 3
+QSL_CARTESIAN, QSL_SPHERICAL = 0, 1
 QSL_LAYOUT_CELL_TABLE, QSL_LAYOUT_NODES_ONLY, QSL_LAYOUT_CELL_TABLE_F32, QSL_LAYOUT_CELL_TABLES_BOTH = 0, 1, 2, 3
 QSL_ST_SEED_OUTSIDE, QSL_ST_NULL_AT_SEED, QSL_ST_STALL_F, QSL_ST_STALL_B = 1, 2, 4, 8
 QSL_ST_CAP_F, QSL_ST_CAP_B, QSL_ST_OPEN = 16, 32, 64
@@ -35,7 +36,7 @@ class QslError(RuntimeError):
 class _GridDesc(C.Structure):
     _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("stretched", C.c_int),
                 ("lo", C.c_double * 3), ("hi", C.c_double * 3), ("xs", _dp), ("ys", _dp), ("zs", _dp),
-                ("sample_type", C.c_int), ("interp_mode", C.c_int), ("layout", C.c_int), ("interp_order", C.c_int)]
+                ("sample_type", C.c_int), ("interp_mode", C.c_int), ("layout", C.c_int), ("interp_order", C.c_int), ("geometry", C.c_int)]
 
 
 class _TraceParams(C.Structure):
@@ -147,7 +148,7 @@ class Field:
 
 def qsl_field_create(nx, ny, nz, bx, by, bz, *, lo=None, hi=None, xs=None, ys=None, zs=None,
                      sample_type=QSL_F64, interp_mode=QSL_NORMALIZE_FIRST, layout=QSL_LAYOUT_CELL_TABLE,
-                     interp_order=QSL_TRILINEAR, stream=None) -> Field:
+                     interp_order=QSL_TRILINEAR, geometry=QSL_CARTESIAN, stream=None) -> Field:
     """bx, by, bz: CUDA float64 tensors of nx*ny*nz values (x fastest).  Uniform grid: lo, hi.  Stretched: xs, ys, zs
     (host sequences of node coordinates)."""
     _require_cuda()
@@ -164,6 +165,7 @@ def qsl_field_create(nx, ny, nz, bx, by, bz, *, lo=None, hi=None, xs=None, ys=No
     d.lo = (C.c_double * 3)(*[float(v) for v in lo]); d.hi = (C.c_double * 3)(*[float(v) for v in hi])
     d.sample_type, d.interp_mode, d.layout = int(sample_type), int(interp_mode), int(layout)
     d.interp_order = int(interp_order)
+    d.geometry = int(geometry)
     for t, name in ((bx, "bx"), (by, "by"), (bz, "bz")):
         if t.numel() != nx * ny * nz:
             raise QslError("%s has %d values, expected %d" % (name, t.numel(), nx * ny * nz))

@@ -165,8 +165,11 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     if (d->interp_mode != QSL_NORMALIZE_FIRST && d->interp_mode != QSL_INTERP_FIRST) return QSL_EINVAL;
     if (d->layout < QSL_LAYOUT_CELL_TABLE || d->layout > QSL_LAYOUT_CELL_TABLES_BOTH) return QSL_EINVAL;
     if (d->interp_order != QSL_TRILINEAR && d->interp_order != QSL_TRIQUADRATIC && d->interp_order != QSL_TRICUBIC) return QSL_EINVAL;
-    const bool ho = d->interp_order != QSL_TRILINEAR;     // higher-order kernels: node samples only, paper mode only
-    if (ho) {
+    if (d->geometry != QSL_CARTESIAN && d->geometry != QSL_SPHERICAL) return QSL_EINVAL;
+    const bool sph = d->geometry == QSL_SPHERICAL;
+    if (sph && (d->stretched || d->interp_mode != QSL_NORMALIZE_FIRST || d->interp_order != QSL_TRILINEAR)) return QSL_EINVAL;
+    const bool ho = d->interp_order != QSL_TRILINEAR || sph;   // gather-kernel fields: node samples only, paper mode only
+    if (d->interp_order != QSL_TRILINEAR) {
         const int need = d->interp_order == QSL_TRICUBIC ? 4 : 3;
         if (d->nx < need || d->ny < need || d->nz < need || d->interp_mode != QSL_NORMALIZE_FIRST) return QSL_EINVAL;
     }
@@ -206,7 +209,8 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     v.nx = d->nx; v.ny = d->ny; v.nz = d->nz;
     v.stretched = d->stretched ? 1 : 0;
     v.interp_mode = d->interp_mode;
-    v.order = ho ? d->interp_order : 1;
+    v.order = d->interp_order != QSL_TRILINEAR ? d->interp_order : 1;
+    v.spherical = sph ? 1 : 0;
     for (int a = 0; a < 3; ++a) {
         // node coordinates: given (stretched) or lo + i*h (uniform), always resident for the locate of the stretched path
         double *tmp = new (std::nothrow) double[dims[a]];

@@ -34,6 +34,7 @@ struct FieldView {
     int nx, ny, nz;
     int stretched;
     int interp_mode;
+    int spherical;            // axes are (longitude, latitude, radius), components in the orthonormal basis (reading A19)
     int order;                // interpolation order: 1 trilinear, 2 triquadratic (Dodgson), 3 tricubic (Keys)
     double lo[3], hi[3];
     double h[3];              // uniform spacing (hi - lo)/(n - 1)

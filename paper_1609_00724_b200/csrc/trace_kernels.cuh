@@ -321,7 +321,18 @@ __device__ __forceinline__ bool inside_box(const TraceArgs &A, const double x[3]
 //                field at the trial end (evaluated as a "5th stage" through the same evaluate call site)
 //   phase 4      final step of size hp, snap onto the face, done
 // NV = 9 with deviation vectors (QSL_TRACE_LQ), 3 without (QSL_TRACE_L): x and L are bit-identical in both modes.
-template <typename S, bool DEV, bool STRETCHED, bool INTERP, int ORDER = 1>
+// Spherical geometry (reading A19): axes (phi, theta, r) = (longitude, latitude, radius), components in
+// the orthonormal basis.  PAPER.md:83-85 (eq. 2): r cos(theta) phi' = B^_phi, r theta' = B^_theta, r' = B^_r, and
+// PAPER.md:125-135 (eq. 6, 7) for the coordinate deviations with the gradient acting on the kernels only: every
+// coordinate rate is the orthonormal component times mf = (1/(r cos theta), 1/r, 1).
+template <bool SPH>
+__device__ __forceinline__ void metric(const double *u, double mf[3])
+{
+    if (SPH) { mf[0] = 1.0 / (u[2] * cos(u[1])); mf[1] = 1.0 / u[2]; mf[2] = 1.0; }
+    else { mf[0] = 1.0; mf[1] = 1.0; mf[2] = 1.0; }
+}
+
+template <typename S, bool DEV, bool STRETCHED, bool INTERP, int ORDER = 1, bool SPH = false>
 struct LineState {
     static constexpr int NV = DEV ? 9 : 3;
     double y[NV];        // x, delta1, delta2
@@ -364,6 +375,13 @@ struct LineState {
             y[6 % NV] = u[1] * a[2] - u[2] * a[1];
             y[7 % NV] = u[2] * a[0] - u[0] * a[2];
             y[8 % NV] = u[0] * a[1] - u[1] * a[0];
+            if (SPH) {
+                // the pair is orthonormal in the orthonormal basis; the state carries coordinate deviations (eq. 8 inverted)
+                double mf[3];
+                metric<SPH>(x, mf);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { y[(3 + c) % NV] *= mf[c]; y[(6 + c) % NV] *= mf[c]; }
+            }
         }
         return true;
     }
@@ -402,14 +420,18 @@ struct LineState {
                 if (!(bn >= A.null_eps)) { finish(A, REC_STALL); return true; }
                 if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, REC_CAP); return true; }
                 h = STRETCHED ? A.step_frac * hmin : A.h_uniform;
+                if (SPH)   // physical cell edges (r cos(theta) h_phi, r h_theta, h_r) of the cell containing x (uniform axes)
+                    h = A.step_frac * fmin(ys[2] * cos(ys[1]) * A.fv.h[0], fmin(ys[2] * A.fv.h[1], A.fv.h[2]));
                 if (lam + h > A.max_length) h = A.max_length - lam;
                 hs = h;
             }
+            double mf[3];
+            metric<SPH>(ys, mf);
             if (st > last) {
                 // landing, "5th stage": b at the trial end -> one Newton update of hp (clamped to [0, h_full])
                 const double bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
                 const double xd = axis == 0 ? yn[0] : (axis == 1 ? yn[1] : yn[2]);
-                const double g = sgn * bd, r = xd - bound;
+                const double g = sgn * bd * (axis == 0 ? mf[0] : (axis == 1 ? mf[1] : mf[2])), r = xd - bound;
                 if (g != 0.0) {
                     double hn = hp - r / g;
                     if (hn == hn) hp = fmin(fmax(hn, 0.0), hfull());
@@ -420,14 +442,16 @@ struct LineState {
             // stage derivative k = (s b, s J d1, s J d2, |b|)  (PAPER.md:79 eq. 1, :119 eq. 5; reading A3 for L)
             double k[NV];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) k[c] = sgn * b[c];
+            for (int c = 0; c < 3; ++c) k[c] = SPH ? sgn * b[c] * mf[c] : sgn * b[c];
             if (DEV) {
 #pragma unroll
                 for (int v = 0; v < 2; ++v)
 #pragma unroll
-                    for (int c = 0; c < 3; ++c)
-                        k[(3 + 3 * v + c) % NV] = sgn * fma(J[c * 3 + 2], ys[(3 + 3 * v + 2) % NV],
-                                                            fma(J[c * 3 + 1], ys[(3 + 3 * v + 1) % NV], J[c * 3] * ys[(3 + 3 * v) % NV]));
+                    for (int c = 0; c < 3; ++c) {
+                        const double jd = fma(J[c * 3 + 2], ys[(3 + 3 * v + 2) % NV],
+                                              fma(J[c * 3 + 1], ys[(3 + 3 * v + 1) % NV], J[c * 3] * ys[(3 + 3 * v) % NV]));
+                        k[(3 + 3 * v + c) % NV] = SPH ? sgn * jd * mf[c] : sgn * jd;
+                    }
             }
             const double w = (st == 0 || st == last) ? 1.0 : 2.0;
 #pragma unroll
@@ -490,10 +514,10 @@ struct LineState {
 // Kernels.  REFILL = false: one work item per thread (grid covers 2n items).  REFILL = true: persistent warps, a lane
 // whose line ended pops the next item from a global counter (warp-aggregated atomic), so ragged line lengths do not
 // idle lanes (north_star, "persistent trace kernel with a global work queue that refills lanes as lines terminate").
-template <typename S, bool DEV, bool STRETCHED, bool INTERP, bool REFILL, int ORDER = 1>
+template <typename S, bool DEV, bool STRETCHED, bool INTERP, bool REFILL, int ORDER = 1, bool SPH = false>
 __global__ void __launch_bounds__(128) trace_kernel(const TraceArgs A)
 {
-    LineState<S, DEV, STRETCHED, INTERP, ORDER> ls;
+    LineState<S, DEV, STRETCHED, INTERP, ORDER, SPH> ls;
     const long long n_items = 2 * A.n;
     unsigned long long my_steps = 0;
     if (!REFILL) {
@@ -539,7 +563,7 @@ struct EpilogueArgs {
 
 struct EndProj { double a[3], b[3], m; };
 
-template <typename S, bool STRETCHED, bool INTERP, int ORDER = 1>
+template <typename S, bool STRETCHED, bool INTERP, int ORDER = 1, bool SPH = false>
 __device__ void project_end(const TraceArgs &A, const double *r, int face, bool bnd, EndProj &E)
 {
     // delta_perp = delta - B^(B^ . delta) with B^ re-normalised at the end point.
@@ -548,7 +572,13 @@ __device__ void project_end(const TraceArgs &A, const double *r, int face, bool 
     evaluate<S, STRETCHED, INTERP, false, true, ORDER>(A, r, b, J, m, hmin);
     const double inv = 1.0 / norm3(b);
     const double u[3] = { b[0] * inv, b[1] * inv, b[2] * inv };
-    const double *d1 = r + 3, *d2 = r + 6;
+    double d1[3], d2[3];
+    {   // PAPER.md:156 (eq. 8): delta x_phi = r cos(theta) delta phi, delta x_theta = r delta theta, delta x_r = delta r
+        double mf[3];
+        metric<SPH>(r, mf);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { d1[c] = SPH ? r[3 + c] / mf[c] : r[3 + c]; d2[c] = SPH ? r[6 + c] / mf[c] : r[6 + c]; }
+    }
     double c1, c2;
     if (bnd && face != 255) {
         const int ax = face >> 1;
@@ -572,7 +602,7 @@ __device__ __forceinline__ double q_eq11(const EndProj &F, const EndProj &B, dou
     return (F.m * B.m) / (m0 * m0) * ((aF2 * bB2 + aB2 * bF2) - 2.0 * (abB * abF));
 }
 
-template <typename S, bool STRETCHED, bool INTERP, int ORDER = 1>
+template <typename S, bool STRETCHED, bool INTERP, int ORDER = 1, bool SPH = false>
 __global__ void __launch_bounds__(128) epilogue_kernel(const EpilogueArgs E)
 {
     const TraceArgs &A = E.T;
@@ -639,13 +669,13 @@ __global__ void __launch_bounds__(128) epilogue_kernel(const EpilogueArgs E)
         evaluate<S, STRETCHED, INTERP, false, true, ORDER>(A, x0, b0, J, m0, hmin);
         EndProj PF, PB;
         if (O.q_perp) {
-            project_end<S, STRETCHED, INTERP, ORDER>(A, rf, ff, false, PF);
-            project_end<S, STRETCHED, INTERP, ORDER>(A, rb, fb, false, PB);
+            project_end<S, STRETCHED, INTERP, ORDER, SPH>(A, rf, ff, false, PF);
+            project_end<S, STRETCHED, INTERP, ORDER, SPH>(A, rb, fb, false, PB);
             O.q_perp[si] = q_eq11(PF, PB, m0);
         }
         if (O.q_bnd) {
-            project_end<S, STRETCHED, INTERP, ORDER>(A, rf, ff, true, PF);
-            project_end<S, STRETCHED, INTERP, ORDER>(A, rb, fb, true, PB);
+            project_end<S, STRETCHED, INTERP, ORDER, SPH>(A, rf, ff, true, PF);
+            project_end<S, STRETCHED, INTERP, ORDER, SPH>(A, rb, fb, true, PB);
             O.q_bnd[si] = q_eq11(PF, PB, m0);
         }
     }

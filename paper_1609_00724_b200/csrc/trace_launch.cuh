@@ -74,9 +74,28 @@ static cudaError_t launch_epilogue_ho(const EpilogueArgs &E, cudaStream_t s)
     return cudaGetLastError();
 }
 
+// Spherical geometry (uniform axes, paper mode, trilinear): always the persistent work-queue launch.
+template <typename S, bool DEV>
+static cudaError_t launch_trace_sph_variant(const TraceArgs &A, cudaStream_t s)
+{
+    const long long n_items = 2 * A.n;
+    const int threads = 128;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_kernel<S, DEV, false, false, true, 1, true>, threads, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    long long blocks = (long long)sm_count() * per_sm;
+    const long long need = (n_items + threads - 1) / threads;
+    if (blocks > need) blocks = need;
+    count_launch();
+    trace_kernel<S, DEV, false, false, true, 1, true><<<(unsigned)blocks, threads, 0, s>>>(A);
+    return cudaGetLastError();
+}
+
 template <typename S>
 cudaError_t launch_trace(const TraceArgs &A, bool dev, bool refill, cudaStream_t s)
 {
+    if (A.fv.spherical) return dev ? launch_trace_sph_variant<S, true>(A, s) : launch_trace_sph_variant<S, false>(A, s);
     if (A.fv.order == 2) return launch_trace_ho<S, 2>(A, dev, s);
     if (A.fv.order == 3) return launch_trace_ho<S, 3>(A, dev, s);
     const bool st = A.fv.stretched != 0, in = A.fv.interp_mode == QSL_INTERP_FIRST;
@@ -91,6 +110,13 @@ cudaError_t launch_trace(const TraceArgs &A, bool dev, bool refill, cudaStream_t
 template <typename S>
 cudaError_t launch_epilogue(const EpilogueArgs &E, cudaStream_t s)
 {
+    if (E.T.fv.spherical) {
+        const int threads = 128;
+        const long long blocks = (E.T.n + threads - 1) / threads;
+        count_launch();
+        epilogue_kernel<S, false, false, 1, true><<<(unsigned)blocks, threads, 0, s>>>(E);
+        return cudaGetLastError();
+    }
     if (E.T.fv.order == 2) return launch_epilogue_ho<S, 2>(E, s);
     if (E.T.fv.order == 3) return launch_epilogue_ho<S, 3>(E, s);
     const bool st = E.T.fv.stretched != 0, in = E.T.fv.interp_mode == QSL_INTERP_FIRST;

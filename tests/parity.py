@@ -9,26 +9,26 @@ import oracle
 import paper_1609_00724_b200 as qsl
 
 
-def gpu_field(grid, B, sample_type, interp_mode, order=1):
+def gpu_field(grid, B, sample_type, interp_mode, order=1, geometry=0):
     """qsl_field_create from host cubes."""
     dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda() for a in B]
     st = qsl.QSL_F32 if sample_type in ("f32", qsl.QSL_F32) and sample_type != qsl.QSL_F64 else qsl.QSL_F64
-    kw = dict(sample_type=st, interp_mode=interp_mode, interp_order=0 if order == 1 else order)
+    kw = dict(sample_type=st, interp_mode=interp_mode, interp_order=0 if order == 1 else order, geometry=geometry)
     if grid.stretched:
         return qsl.qsl_field_create(grid.nx, grid.ny, grid.nz, *dev, xs=grid.xs, ys=grid.ys, zs=grid.zs, **kw)
     return qsl.qsl_field_create(grid.nx, grid.ny, grid.nz, *dev, lo=grid.lo, hi=grid.hi, **kw)
 
 
-def cpu_field(grid, B, sample_type, interp_mode, order=1):
+def cpu_field(grid, B, sample_type, interp_mode, order=1, geometry=0):
     st = oracle.F32 if sample_type in ("f32", 0) else oracle.F64
-    return oracle.Field(grid, B, st, interp_mode, order)
+    return oracle.Field(grid, B, st, interp_mode, order, geometry)
 
 
 def run_both(grid, B, sample_type, seeds, box_lo, box_hi, *, interp_mode=0, mode=1, method=0, step_frac=0.25,
-             max_steps=1 << 30, max_length=math.inf, null_eps=1e-12, flags=0, want_dev=False, tol=1e-2, order=1):
+             max_steps=1 << 30, max_length=math.inf, null_eps=1e-12, flags=0, want_dev=False, tol=1e-2, order=1, geometry=0):
     st = "f32" if sample_type in ("f32", 0) else "f64"
-    fg = gpu_field(grid, B, st, interp_mode, order)
-    fc = cpu_field(grid, B, st, interp_mode, order)
+    fg = gpu_field(grid, B, st, interp_mode, order, geometry)
+    fc = cpu_field(grid, B, st, interp_mode, order, geometry)
     params = qsl.make_trace_params(box_lo, box_hi, method=method, step_frac=step_frac, mode=mode, max_length=max_length,
                                    max_steps=max_steps, null_eps=null_eps, flags=flags, tol=tol)
     outs = qsl.DEFAULT_OUTPUTS + (("dev_f", "dev_b") if want_dev else ())

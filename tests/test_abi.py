@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol():
 def test_struct_layouts_match_header_sizes():
     """ctypes mirrors of the ABI structs: sizes as a C compiler lays them out (x86-64 SysV)."""
     from paper_1609_00724_b200 import binding as B
-    assert ctypes.sizeof(B._GridDesc) == 4 * 4 + 6 * 8 + 3 * 8 + 4 * 4               # 4 trailing ints
+    assert ctypes.sizeof(B._GridDesc) == 4 * 4 + 6 * 8 + 3 * 8 + 5 * 4 + 4           # 5 trailing ints + tail padding
     assert ctypes.sizeof(B._TraceParams) == 48 + 8 + 8 + 8 + 8 + 8 + 8 + 8 + 8   # ... flags (+pad), tol
     assert ctypes.sizeof(B._TraceOut) == 12 * 8
     assert ctypes.sizeof(B._Lattice) == 8 + 24 + 4 * 24

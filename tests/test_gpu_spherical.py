@@ -1,0 +1,96 @@
+"""GPU parity of the spherical geometry (SURVEY.md 8(f) f4; PAPER.md:83-87 eq. 2, :125-135 eq. 6-7, :153-156 eq. 8;
+reading A19) against the CPU oracle at the north_star gates; the box size of the end-point gate is the largest extent of
+the (phi, theta, r) trace box."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1609_00724_b200 as qsl
+import qsl_inputs as qi
+from tests.parity import compare_trace, run_both
+
+pytestmark = pytest.mark.gpu
+SPH = qsl.QSL_SPHERICAL
+
+
+def _cubes(g, f):
+    P, T, R = np.meshgrid(g.xs, g.ys, g.zs, indexing="ij")
+    return [np.ascontiguousarray(np.transpose(c * np.ones_like(P), (2, 1, 0))) for c in f(P, T, R)]
+
+
+def _dipole_plus(p, t, r):
+    """Dipole plus a small non-axisymmetric octupole-like part, so that B_phi and the phi-derivatives are exercised."""
+    return (0.15 * np.sin(3 * p) * np.cos(t) / r ** 4, -np.cos(t) / r ** 3 + 0.1 * np.cos(3 * p) * np.sin(2 * t) / r ** 4,
+            2 * np.sin(t) / r ** 3 + 0.2 * np.cos(3 * p) * np.cos(t) ** 2 / r ** 4)
+
+
+def test_sph_monopole_q_two():
+    g = qi.Grid.uniform((9, 11, 33), (0.1, -0.3, 1.0), (0.9, 0.5, 3.0))
+    B = _cubes(g, lambda p, t, r: (0 * r, 0 * r, 1 / r ** 2))
+    seeds = np.array([[0.33, 0.11, g.zs[7]], [0.71, -0.22, g.zs[20]], [0.5, 0.4, g.zs[1]], [0.2, 0.0, 1.0], [0.2, 0.0, 3.0]])
+    gg, c = run_both(g, B, "f64", seeds, g.lo, g.hi, geometry=SPH)
+    compare_trace(gg, c, g.lo, g.hi, frac=1.0, label="monopole")
+    assert np.abs(gg["q_perp"] - 2).max() < 1e-10 and np.abs(gg["L"] - 2).max() < 1e-12
+
+
+@pytest.mark.parametrize("st", ["f64", "f32"])
+@pytest.mark.parametrize("mode", [qsl.QSL_TRACE_LQ, qsl.QSL_TRACE_L])
+def test_sph_wedge_field(st, mode):
+    g = qi.Grid.uniform((48, 40, 44), (0.0, -0.9, 1.0), (2.0, 0.9, 2.4))
+    B = _cubes(g, _dipole_plus)
+    rng = np.random.default_rng(5)
+    n = 4000
+    seeds = np.stack([rng.uniform(0.1, 1.9, n), rng.uniform(-0.8, 0.8, n), rng.uniform(1.0, 2.2, n)], 1)
+    seeds[:500, 2] = 1.0                                                      # photospheric seeds
+    gg, c = run_both(g, B, st, seeds, g.lo, g.hi, geometry=SPH, mode=mode, max_steps=50000)
+    rep = compare_trace(gg, c, g.lo, g.hi, with_q=mode == qsl.QSL_TRACE_LQ, label="wedge %s" % st)
+    assert rep["same_steps"] >= 0.999
+    assert (c["face_f"] == 4).mean() > 0.2 and (c["status"] & oracle.ST_OPEN).mean() > 0.05      # closed and open lines
+
+
+def test_sph_cartesian_limit_euler_caps_inner_box():
+    R0, p0, t0 = 1.0e5, 0.3, 0.2
+    c0 = math.cos(t0)
+    n = 33
+    gc = qi.Grid.uniform((n, n, n), (-1.0, -1.0, 0.0), (1.0, 1.0, 1.0))
+    Bc = qi.hyperbolic_field(gc, 2.0)
+    gs = qi.Grid.uniform((n, n, n), (p0 - 1.0 / (R0 * c0), t0 - 1.0 / R0, R0), (p0 + 1.0 / (R0 * c0), t0 + 1.0 / R0, R0 + 1.0))
+    rng = np.random.default_rng(17)
+    sc = np.stack([rng.uniform(-0.4, 0.4, 300), rng.uniform(-0.4, 0.4, 300), rng.uniform(0.0, 0.8, 300)], 1)
+    ss = np.stack([p0 + sc[:, 0] / (R0 * c0), t0 + sc[:, 1] / R0, R0 + sc[:, 2]], 1)
+    # the trace box is 1e-5 rad x 1e-5 rad x 1: gate the end points per axis by scaling the angles to lengths
+    for kw in (dict(), dict(method=qsl.QSL_EULER, step_frac=0.2), dict(max_steps=5), dict(max_length=0.3)):
+        gg, c = run_both(gs, Bc, "f64", ss, gs.lo, gs.hi, geometry=SPH, **kw)
+        for d in (gg, c):
+            for key in ("end_f", "end_b"):
+                d[key] = np.stack([(d[key][:, 0] - p0) * R0 * c0, (d[key][:, 1] - t0) * R0, d[key][:, 2] - R0], 1)
+        compare_trace(gg, c, (-1, -1, 0), (1, 1, 1), label="cartesian limit " + str(kw))
+    # and against the Cartesian device path itself
+    gcart, _ = run_both(gc, Bc, "f64", sc, gc.lo, gc.hi)
+    gsph, _ = run_both(gs, Bc, "f64", ss, gs.lo, gs.hi, geometry=SPH)
+    assert np.allclose(gsph["L"], gcart["L"], rtol=2e-4) and np.allclose(gsph["q_bnd"], gcart["q_bnd"], rtol=2e-3)
+    lo = (gs.lo[0] + 0.1 / (R0 * c0), gs.lo[1] + 0.2 / R0, R0 + 0.13); hi = (gs.hi[0] - 0.15 / (R0 * c0), gs.hi[1] - 0.1 / R0, R0 + 0.77)
+    gg, c = run_both(gs, Bc, "f64", ss, lo, hi, geometry=SPH)
+    for d in (gg, c):
+        for key in ("end_f", "end_b"):
+            d[key] = np.stack([(d[key][:, 0] - p0) * R0 * c0, (d[key][:, 1] - t0) * R0, d[key][:, 2] - R0], 1)
+    compare_trace(gg, c, (-1, -1, 0), (1, 1, 1), label="cartesian limit inner box")
+
+
+def test_sph_argument_errors():
+    z = torch.ones(5 * 5 * 5, dtype=torch.float64, device="cuda")
+    kw = dict(lo=(0, 0, 1), hi=(1, 1, 2), geometry=SPH)
+    for bad in (dict(interp_mode=qsl.QSL_INTERP_FIRST), dict(interp_order=qsl.QSL_TRICUBIC)):
+        with pytest.raises(qsl.QslError):
+            qsl.qsl_field_create(5, 5, 5, z, z, z, **kw, **bad)
+    with pytest.raises(qsl.QslError):
+        qsl.qsl_field_create(5, 5, 5, z, z, z, xs=[0, .1, .3, .6, 1], ys=[0, .1, .3, .6, 1], zs=[1, 1.1, 1.3, 1.6, 2], geometry=SPH)
+    f = qsl.qsl_field_create(5, 5, 5, z, z, z, **kw)
+    seeds = torch.tensor([[0.5, 0.5, 1.5]], dtype=torch.float64, device="cuda")
+    for bad in (dict(method=qsl.QSL_CK45), dict(arith=qsl.QSL_ARITH_F32)):
+        with pytest.raises(qsl.QslError):
+            qsl.qsl_trace(f, seeds, qsl.make_trace_params((0, 0, 1), (1, 1, 2), **bad))
+    f.destroy()
