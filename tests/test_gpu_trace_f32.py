@@ -151,3 +151,36 @@ def test_f32_requires_its_table():
     torch.cuda.synchronize()
     assert float((a["L"] - b["L"]).abs().max()) < 1e-4
     f.destroy()
+
+
+def test_f32_cfg4_full_size_sampled():
+    """BASELINE.json configs[3] at full size in the configuration `bench.py --arith f32` times: 256^3 seeds through the
+    fp32-sampled 256^3 field in fp32 arithmetic; a sample of the lines against the fp64 oracle (reading-A6 gates, and the
+    much tighter medians the cell-frame formulation actually reaches), every line through size-independent properties."""
+    from tests.test_gpu_full_size import _pick, _sample
+    cfg = qi.make_config("cfg4")
+    grid = cfg["grid"]
+    dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda() for a in cfg["B"]]
+    fg = qsl.qsl_field_create(grid.nx, grid.ny, grid.nz, *dev, lo=grid.lo, hi=grid.hi, sample_type=qsl.QSL_F32,
+                              layout=qsl.QSL_LAYOUT_CELL_TABLE_F32)
+    del dev
+    p = qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], arith=qsl.QSL_ARITH_F32, step_frac=cfg["step_frac"],
+                              max_steps=cfg["max_steps"], null_eps=cfg["null_eps"])
+    tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    g = qsl.qsl_trace(fg, torch.from_numpy(cfg["seeds"]).cuda(), p, total_steps=tot)
+    torch.cuda.synchronize()
+    lo = torch.tensor(cfg["box_lo"], dtype=torch.float64, device="cuda"); hi = torch.tensor(cfg["box_hi"], dtype=torch.float64, device="cuda")
+    assert int(tot.item()) == int(g["nsteps_f"].to(torch.int64).sum() + g["nsteps_b"].to(torch.int64).sum())
+    for end, face in ((g["end_f"], g["face_f"]), (g["end_b"], g["face_b"])):
+        landed = face != 255
+        ax = (face.to(torch.int64) >> 1).clamp(max=2)
+        bound = torch.where((face & 1).bool(), hi[ax], lo[ax])
+        assert bool((end.gather(1, ax[:, None])[:, 0][landed] == bound[landed]).all())     # snapped exactly onto the face
+        assert bool(((end >= lo - 1e-5) & (end <= hi + 1e-5)).all())
+    idx = _sample(len(cfg["seeds"]), 2039)
+    fc = cpu_field(grid, cfg["B"], "f32", 0)
+    c = oracle.trace(fc, cfg["seeds"][idx], cfg["box_lo"], cfg["box_hi"], step_frac=cfg["step_frac"], max_steps=cfg["max_steps"],
+                     null_eps=cfg["null_eps"])
+    rep = compare_f32(_pick(g, idx), c, cfg["box_lo"], cfg["box_hi"], label="f32 cfg4 full")
+    assert rep["n"] > 12000 and rep["end_med"] < 1e-7 and rep["L_med"] < 1e-6 and rep["q_perp_dlog_med"] < 1e-5, rep
+    fg.destroy()
