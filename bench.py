@@ -214,6 +214,8 @@ def main():
                          "own Hilbert-curve mid-point insertion on length jumps (PAPER.md:194-206; DESIGN.md reading A17)")
     ap.add_argument("--hilbert-thr", type=float, default=0.05, help="field-line-length jump threshold of --refine hilbert")
     ap.add_argument("--hilbert-shift", type=int, default=5, help="shift of the second curve in fine cells (0 = no shifted pass)")
+    ap.add_argument("--e2e-chunks", type=int, default=0,
+                    help="pieces the end-to-end path pipelines over two streams; 0 = one piece per 4 M lines (at most 8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -300,14 +302,16 @@ def main():
         return r, acc
 
     host_out = {}
+    host_res = {}
 
     def step_e2e():
         """The same through HOST buffers: pinned seeds -> device, hot path, results -> pinned host."""
-        d = seeds_host.cuda(non_blocking=True)
         if levels == 0:
-            res = qsl.qsl_trace(field, d, pLQ if mode == 1 else pL, outputs=outs, out=out_bufs, total_steps=tot)
-            results = [res[k] for k in outs]
-        elif hilbert:
+            # pinned seeds -> device, trace, results -> pinned host, pipelined in pieces over two streams (driver.trace_host)
+            qsl.trace_host(field, seeds_host, pLQ if mode == 1 else pL, outputs=outs, chunks=args.e2e_chunks or None, host_out=host_res)
+            return seeds_host.numel() * 8, sum(t.numel() * t.element_size() for t in host_res.values())
+        d = seeds_host.cuda(non_blocking=True)
+        if hilbert:
             # level-0 seeds are generated on the device by qsl_hilbert_level0: the host supplies the lattice only
             r, _ = hilbert_step()
             results = [r["keys"], r["L"], r["Q"], hstate["map"]]
@@ -416,6 +420,18 @@ def main():
                                   % ("FP32" if f32 else "FP64", PIPE_SLOTS_PER_STEP["LQ"], PIPE_SLOTS_PER_STEP["L"],
                                      "FFMA" if f32 else "DFMA"),
                     "true_flops_achieved_tflops": flops / (k_ms * 1e-3) / 1e12}
+        # the other candidate bound of SURVEY.md 8(d): divergent gathers of table entries through L1/L2.  Algorithmic
+        # traffic: a line enters a new cell every ~2.5 steps at h = 0.25 cell and then reads one table entry (192 B fp64,
+        # 96 B fp32); peak = 32-byte divergent gathers over an L2-resident (64 MiB) footprint, measured here.
+        try:
+            g_peak = qsl.qsl_peak_gather(32, 64 << 20) * 32.0 / 1e9
+            g_ach = (rk_steps / 2.5) * (96.0 if f32 else 192.0) / (k_ms * 1e-3) / 1e9
+            roofline["other_bounds"] = [{"bound": "l2_gather", "achieved": g_ach, "peak": g_peak, "unit": "GB/s",
+                                         "frac": g_ach / g_peak,
+                                         "convention": "one table entry per cell entered, a cell every 2.5 RK4 steps; peak = "
+                                                       "qsl_peak_gather(32 B, 64 MiB footprint)"}]
+        except Exception as exc:                                   # the roofline of the binding unit stands on its own
+            roofline["other_bounds"] = [{"bound": "l2_gather", "error": str(exc)}]
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

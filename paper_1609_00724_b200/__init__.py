@@ -10,4 +10,4 @@ from .binding import (  # noqa: F401
     qsl_peak_gather, qsl_hilbert_bits, qsl_hilbert_level0, qsl_hilbert_keys, qsl_hilbert_cells, qsl_sort_keys64, qsl_gather,
     qsl_hilbert_refine, qsl_hilbert_merge, qsl_hilbert_convert,
 )
-from .driver import adaptive_map, hilbert_map  # noqa: F401,E402
+from .driver import adaptive_map, hilbert_map, trace_host  # noqa: F401,E402
