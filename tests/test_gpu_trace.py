@@ -157,3 +157,22 @@ def test_nodes_only_layout_uses_corner_kernel_and_matches():
     for k in a:
         assert torch.equal(a[k], b[k]) or (torch.isnan(a[k]) == torch.isnan(b[k])).all() and torch.equal(
             torch.nan_to_num(a[k]), torch.nan_to_num(b[k])), k
+
+
+@pytest.mark.parametrize("chunks", [1, 3, None])
+def test_trace_host_pipelined_equals_one_call(chunks):
+    """driver.trace_host (pinned host buffers, pieces alternating between two streams) returns exactly what one qsl_trace
+    call returns: lines are independent, so cutting the seed set changes nothing."""
+    cfg = qi.make_config("cfg1", scale=0.5)
+    fg = gpu_field(cfg["grid"], cfg["B"], "f64", 0)
+    p = qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], max_steps=cfg["max_steps"])
+    outs = ("end_f", "end_b", "L", "q_perp", "q_bnd", "face_f", "face_b", "status", "nsteps_f")
+    seeds_host = torch.from_numpy(np.ascontiguousarray(cfg["seeds"])).pin_memory()
+    h = qsl.trace_host(fg, seeds_host, p, outputs=outs, chunks=chunks)
+    torch.cuda.synchronize()
+    g = qsl.qsl_trace(fg, seeds_host.cuda(), p, outputs=outs)
+    torch.cuda.synchronize()
+    for k in outs:
+        assert h[k].is_pinned() and torch.equal(h[k], g[k].cpu()), k
+    assert qsl.trace_host(fg, seeds_host[:0], p, outputs=("L",)) == {}
+    fg.destroy()
