@@ -1,7 +1,7 @@
 /* qsl.h -- C ABI of libqsl: B200-native (sm_100a) field-line tracing, squashing factor Q, field-line length L,
  * FLEDGE edge maps and adaptive seed refinement, after Tassev & Savcheva, "QSL Squasher" (arXiv:1609.00724).
  * Citations are "PAPER.md:<line>" of the paper text plus the section / equation they fall in; readings of silent
- * or ambiguous passages (A1..A14) are listed in DESIGN.md.
+ * or ambiguous passages (A1..A19) are listed in DESIGN.md.
  *
  * Conventions
  *  - Every function returns int: 0 = QSL_OK, < 0 = error (see qsl_strerror).  Nothing throws or aborts across the ABI.
@@ -9,7 +9,8 @@
  *    the library neither frees nor retains it.  The one exception is qsl_field_create, which copies its input into a
  *    library-owned packed buffer released by qsl_field_destroy.
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are asynchronous on that
- *    stream except where a count is returned to the host (qsl_refine's n_children), which synchronises the stream.
+ *    stream except where a count is returned to the host (qsl_refine's n_children, qsl_hilbert_refine's n_new), which
+ *    synchronises the stream.
  *    Scratch memory is taken from the stream-ordered CUDA memory pool of the current device.
  *  - Per-line problems are not errors: they are bits of the per-seed `status` output.
  *  - There is no CPU fallback: without a CUDA device every compute entry point returns QSL_ECUDA.
