@@ -296,8 +296,8 @@ def main():
             return o["L"], o["q_perp"]
 
         r = qsl.hilbert_map(lat, levels, args.hilbert_thr, int(lat.ndim) * levels, args.hilbert_shift, tf)
-        # the converter output at the finest lattice of cfg3 is 4.3 GB, of cfg5 69 GB: convert to level min(levels, 2)
-        hstate["map"] = qsl.qsl_hilbert_convert(lat, levels, min(levels, 2), r["keys"], r["Q"])
+        # the converter output at the finest lattice of cfg3 is 4.3 GB, of cfg5 275 GB: convert to level 2 (2-D) / 0 (3-D)
+        hstate["map"] = qsl.qsl_hilbert_convert(lat, levels, min(levels, 2) if int(lat.ndim) == 2 else 0, r["keys"], r["Q"])
         hstate["r"] = r
         return r, acc
 
