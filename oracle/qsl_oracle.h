@@ -8,6 +8,11 @@
  * Parity pins (tests/test_oracle_pins.py): P1 uniform field Q = 2; P2 hyperbolic closed forms; P3 invariances;
  * P4 finite-difference Jacobian (Pariat & Demoulin style); P5 bounds; P6 RK4 order;
  * P8 scipy.ndimage.sobel; P9 numpy order statistic; P10 brute-force refinement; P12 mode consistency.
+ * Rows f1-f4: tests/test_oracle_ck45.py (Cash-Karp: single-step orders 5 / 4 against the exact flow, deviation =
+ * derivative of the step map, closed forms, controller invariants), tests/test_oracle_interp.py (Dodgson / Keys kernels:
+ * interpolation, linear / quadratic reproduction, C1 / C0, gradient = derivative, convergence orders),
+ * tests/test_oracle_spherical.py (monopole Q = 2, dipole line geometry, Cartesian limit), and for oracle/hilbert.py
+ * tests/test_oracle_hilbert.py (curve properties, purpose of each pass, merge and converter by brute force).
  * On configs 2-5 no closed form exists: there the oracle itself is the reference ("parity pinned on the
  * analytic cases P1-P6, unpinned in absolute terms on configs 2-5").
  */
