@@ -92,7 +92,8 @@ typedef struct {
                                     then (phi, theta, r); lines follow eq. (2), deviations eq. (6)-(7) as printed (without
                                     the metric-derivative terms), Q uses eq. (8); dev_f / dev_b are coordinate
                                     deviations.  Uniform axes, QSL_NORMALIZE_FIRST, QSL_TRILINEAR, fp64, RK4 / Euler only
-                                    (else QSL_EINVAL); node samples only, traced by the gather kernel                     */
+                                    (else QSL_EINVAL); the cell-table kernel (fp64 table layouts) and the gather kernel
+                                    (QSL_LAYOUT_NODES_ONLY / QSL_FLAG_KERNEL_V1) both carry the geometry                  */
 } qsl_grid_desc;
 
 /* Packs the three component cubes (DEVICE, fp64, nx*ny*nz each) into one AoS array of (b^x, b^y, b^z, |B|) samples

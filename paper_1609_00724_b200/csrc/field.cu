@@ -168,14 +168,14 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     if (d->geometry != QSL_CARTESIAN && d->geometry != QSL_SPHERICAL) return QSL_EINVAL;
     const bool sph = d->geometry == QSL_SPHERICAL;
     if (sph && (d->stretched || d->interp_mode != QSL_NORMALIZE_FIRST || d->interp_order != QSL_TRILINEAR)) return QSL_EINVAL;
-    const bool ho = d->interp_order != QSL_TRILINEAR || sph;   // gather-kernel fields: node samples only, paper mode only
+    const bool ho = d->interp_order != QSL_TRILINEAR;           // gather-kernel fields: node samples only, paper mode only
     if (d->interp_order != QSL_TRILINEAR) {
         const int need = d->interp_order == QSL_TRICUBIC ? 4 : 3;
         if (d->nx < need || d->ny < need || d->nz < need || d->interp_mode != QSL_NORMALIZE_FIRST) return QSL_EINVAL;
     }
     const bool want64 = !ho && (d->layout == QSL_LAYOUT_CELL_TABLE || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH);
     const bool want32 = !ho && (d->layout == QSL_LAYOUT_CELL_TABLE_F32 || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH);
-    if (want32 && (d->sample_type != QSL_F32 || d->stretched)) return QSL_EINVAL;   // fp32 arithmetic: fp32 samples, uniform grid
+    if (want32 && (d->sample_type != QSL_F32 || d->stretched || sph)) return QSL_EINVAL;   // fp32 arithmetic: fp32 samples, uniform Cartesian grid
     const long long n = (long long)d->nx * d->ny * d->nz;
     if (n >= (1ll << 31)) return QSL_ERANGE;   // node index is 32-bit inside the gather
     const int dims[3] = { d->nx, d->ny, d->nz };

@@ -63,7 +63,8 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
     if (!f || !p || !out || n < 0 || (n > 0 && !seeds)) return QSL_EINVAL;
     if (p->method != QSL_RK4 && p->method != QSL_EULER && p->method != QSL_CK45) return QSL_EINVAL;
     // the adaptive stepper runs in fp64 on the fp64 cell table only, with a positive tolerance
-    if (p->method == QSL_CK45 && (!f->view.cells || p->arith != QSL_ARITH_F64 || !(p->tol > 0.0))) return QSL_EINVAL;
+    if (p->method == QSL_CK45 && (!f->view.cells || f->view.spherical || p->arith != QSL_ARITH_F64 || !(p->tol > 0.0)))
+        return QSL_EINVAL;
     if (p->mode != QSL_TRACE_L && p->mode != QSL_TRACE_LQ) return QSL_EINVAL;
     if (p->arith != QSL_ARITH_F64 && p->arith != QSL_ARITH_F32) return QSL_EINVAL;
     // fp32 arithmetic (reading A6): needs the fp32 coefficient table (QSL_LAYOUT_CELL_TABLE_F32 / _BOTH), which
@@ -110,7 +111,7 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         } else if (e == cudaSuccess && p->arith == QSL_ARITH_F32) {
             const int ps = prof_slot(p->mode);
             rc = launch_trace3(A, f->d_cells32, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
-        } else if (e == cudaSuccess && v2 && !f->view.stretched && (p->flags & QSL_FLAG_KERNEL_FRAME)) {
+        } else if (e == cudaSuccess && v2 && !f->view.stretched && !f->view.spherical && (p->flags & QSL_FLAG_KERNEL_FRAME)) {
             const int ps = prof_slot(p->mode);
             rc = launch_trace3_f64(A, f->sample_type == QSL_F32, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
         } else if (e == cudaSuccess && v2) {

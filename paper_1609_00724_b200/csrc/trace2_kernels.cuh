@@ -40,7 +40,9 @@ __device__ __forceinline__ double norm3_fast(const double v[3])
 // it must not occupy registers during the thousands of plain steps.  Layout [slot * n_threads + thread].
 enum { ST_K1 = 0, ST_BN = 9, ST_XT = 10, ST_HP = 13, ST_BOUND = 14, ST_HFULL = 15, ST_AXIS_FACE = 16, STASH_DOUBLES = 17 };
 
-template <bool DEV, bool STRETCHED, bool INTERP>
+// SPH: spherical geometry (reading A19): the coordinate rates are the orthonormal components times the metric factors
+// (1/(r cos theta), 1/r, 1) of the evaluation point; |b| for L and the stall test is taken before the scaling.
+template <bool DEV, bool STRETCHED, bool INTERP, bool SPH = false>
 struct LineState2 {
     static constexpr int NV = DEV ? 9 : 3;
     // cached cell: monomial coefficients a[8 c + m], origin (edges only on stretched grids)
@@ -160,6 +162,22 @@ struct LineState2 {
         }
     }
 
+    // b -> coordinate rates (and |b| of the unscaled vector), k -> coordinate deviation rates, at the point pt
+    __device__ __forceinline__ double to_rates(const double *pt, double b[3], double *k)
+    {
+        const double bn = norm3_fast(b);
+        if (SPH) {
+            double mf[3];
+            metric<SPH>(pt, mf);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                b[c] *= mf[c];
+                if (DEV) { k[(3 + c) % NV] *= mf[c]; k[(6 + c) % NV] *= mf[c]; }
+            }
+        }
+        return bn;
+    }
+
     // Starts work item q.  Returns false if the item ended at once (seed outside the trace box).  The orthonormal pair
     // a^, b^ of O2 comes from seed_basis_kernel (one thread per seed, all lanes busy) instead of being built here by
     // the one or two lanes of a warp that happen to be refilling; a null at the seed is caught by the first attempt.
@@ -181,6 +199,12 @@ struct LineState2 {
             const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(A.basis + 6 * (size_t)pos);
             const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
             y[3 % NV] = b0.x; y[4 % NV] = b0.y; y[5 % NV] = b1.x; y[6 % NV] = b1.y; y[7 % NV] = b2.x; y[8 % NV] = b2.y;
+            if (SPH) {   // orthonormal pair -> coordinate deviations (eq. 8 inverted)
+                double mf[3];
+                metric<SPH>(x, mf);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { y[(3 + c) % NV] *= mf[c]; y[(6 + c) % NV] *= mf[c]; }
+            }
         }
         return true;
     }
@@ -222,12 +246,14 @@ struct LineState2 {
             if (phase >= 2) { p0[0] = st[(ST_XT + 0) * T]; p0[1] = st[(ST_XT + 1) * T]; p0[2] = st[(ST_XT + 2) * T]; }
             enter_cell(A, p0, d);
             stage(d, y, b, k);
-            bn = norm3_fast(b);
+            bn = SPH ? to_rates(p0, b, k) : norm3_fast(b);
             if (phase == 0) {
                 // O4: stall / caps are tested on k1 before the step; h from the cell containing x
                 if (!(bn >= A.null_eps)) { finish(A, 255, nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL); return true; }
                 if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, 255, REC_CAP); return true; }
                 h = STRETCHED ? A.step_frac * fmin(hc[0], fmin(hc[1], hc[2])) : A.h_uniform;
+                if (SPH)   // physical cell edges (r cos(theta) h_phi, r h_theta, h_r) at the start of the step
+                    h = A.step_frac * fmin(y[2] * cos(y[1]) * A.fv.h[0], fmin(y[2] * A.fv.h[1], A.fv.h[2]));
                 if (lam + h > A.max_length) h = A.max_length - lam;
                 hs = h;
             } else {
@@ -267,6 +293,7 @@ struct LineState2 {
         } else {
             // RK4 (reading A5): k2 = f(y + h/2 k1), k3 = f(y + h/2 k2), k4 = f(y + h k3), y+ = y + h/6 (k1 + 2 k2 + 2 k3 + k4)
             const double half = 0.5 * shs;
+            double bnS = 0.0;          // |b| of the unscaled field vector (spherical geometry only)
 #pragma unroll
             for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
             enter_cell(A, ys, d);
@@ -275,12 +302,13 @@ struct LineState2 {
             accL = bn;
             // ---- stage 2
             stage(d, ys, b, k);
+            if (SPH) bnS = to_rates(ys, b, k);
             {
                 double xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
                 enter_cell(A, xn, d);
-                bn = norm3_fast(b);
+                bn = SPH ? bnS : norm3_fast(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) {
                     const double kc = c < 3 ? b[c] : k[c];
@@ -290,12 +318,13 @@ struct LineState2 {
             }
             // ---- stage 3
             stage(d, ys, b, k);
+            if (SPH) bnS = to_rates(ys, b, k);
             {
                 double xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
                 enter_cell(A, xn, d);
-                bn = norm3_fast(b);
+                bn = SPH ? bnS : norm3_fast(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) {
                     const double kc = c < 3 ? b[c] : k[c];
@@ -305,6 +334,7 @@ struct LineState2 {
             }
             // ---- stage 4
             stage(d, ys, b, k);
+            if (SPH) bnS = to_rates(ys, b, k);
             {
                 const double fL = hs * (1.0 / 6.0), f = back ? -fL : fL;
                 double xn[3];
@@ -312,7 +342,7 @@ struct LineState2 {
                 for (int c = 0; c < 3; ++c) xn[c] = fma(f, fma(1.0, b[c], acc[c]), y[c]);
                 // the trial end is where the next attempt starts if it is accepted: enter its cell now
                 enter_cell(A, xn, d);
-                bn = norm3_fast(b);
+                bn = SPH ? bnS : norm3_fast(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, fma(1.0, k[c], acc[c]), y[c]);
                 accL = fma(fL, fma(1.0, bn, accL), L);
@@ -419,10 +449,10 @@ __global__ void __launch_bounds__(128) seed_basis_kernel(const TraceArgs A, doub
 #ifndef QSL_T2_MIN_BLOCKS_L
 #define QSL_T2_MIN_BLOCKS_L 4
 #endif
-template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL>
+template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL, bool SPH = false>
 __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : QSL_T2_MIN_BLOCKS_L) trace2_kernel(const TraceArgs A)
 {
-    LineState2<DEV, STRETCHED, INTERP> ls;
+    LineState2<DEV, STRETCHED, INTERP, SPH> ls;
     const long long n_items = 2 * A.n;
     unsigned long long my_steps = 0;
     if (!REFILL) {

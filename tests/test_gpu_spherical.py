@@ -27,25 +27,30 @@ def _dipole_plus(p, t, r):
             2 * np.sin(t) / r ** 3 + 0.2 * np.cos(3 * p) * np.cos(t) ** 2 / r ** 4)
 
 
-def test_sph_monopole_q_two():
+KERNELS = [0, qsl.QSL_FLAG_KERNEL_V1]      # cell-table kernel (default) and gather kernel: both carry the geometry
+
+
+@pytest.mark.parametrize("flags", KERNELS)
+def test_sph_monopole_q_two(flags):
     g = qi.Grid.uniform((9, 11, 33), (0.1, -0.3, 1.0), (0.9, 0.5, 3.0))
     B = _cubes(g, lambda p, t, r: (0 * r, 0 * r, 1 / r ** 2))
     seeds = np.array([[0.33, 0.11, g.zs[7]], [0.71, -0.22, g.zs[20]], [0.5, 0.4, g.zs[1]], [0.2, 0.0, 1.0], [0.2, 0.0, 3.0]])
-    gg, c = run_both(g, B, "f64", seeds, g.lo, g.hi, geometry=SPH)
+    gg, c = run_both(g, B, "f64", seeds, g.lo, g.hi, geometry=SPH, flags=flags)
     compare_trace(gg, c, g.lo, g.hi, frac=1.0, label="monopole")
     assert np.abs(gg["q_perp"] - 2).max() < 1e-10 and np.abs(gg["L"] - 2).max() < 1e-12
 
 
+@pytest.mark.parametrize("flags", KERNELS)
 @pytest.mark.parametrize("st", ["f64", "f32"])
 @pytest.mark.parametrize("mode", [qsl.QSL_TRACE_LQ, qsl.QSL_TRACE_L])
-def test_sph_wedge_field(st, mode):
+def test_sph_wedge_field(st, mode, flags):
     g = qi.Grid.uniform((48, 40, 44), (0.0, -0.9, 1.0), (2.0, 0.9, 2.4))
     B = _cubes(g, _dipole_plus)
     rng = np.random.default_rng(5)
     n = 4000
     seeds = np.stack([rng.uniform(0.1, 1.9, n), rng.uniform(-0.8, 0.8, n), rng.uniform(1.0, 2.2, n)], 1)
     seeds[:500, 2] = 1.0                                                      # photospheric seeds
-    gg, c = run_both(g, B, st, seeds, g.lo, g.hi, geometry=SPH, mode=mode, max_steps=50000)
+    gg, c = run_both(g, B, st, seeds, g.lo, g.hi, geometry=SPH, mode=mode, max_steps=50000, flags=flags)
     rep = compare_trace(gg, c, g.lo, g.hi, with_q=mode == qsl.QSL_TRACE_LQ, label="wedge %s" % st)
     assert rep["same_steps"] >= 0.999
     assert (c["face_f"] == 4).mean() > 0.2 and (c["status"] & oracle.ST_OPEN).mean() > 0.05      # closed and open lines
@@ -62,7 +67,8 @@ def test_sph_cartesian_limit_euler_caps_inner_box():
     sc = np.stack([rng.uniform(-0.4, 0.4, 300), rng.uniform(-0.4, 0.4, 300), rng.uniform(0.0, 0.8, 300)], 1)
     ss = np.stack([p0 + sc[:, 0] / (R0 * c0), t0 + sc[:, 1] / R0, R0 + sc[:, 2]], 1)
     # the trace box is 1e-5 rad x 1e-5 rad x 1: gate the end points per axis by scaling the angles to lengths
-    for kw in (dict(), dict(method=qsl.QSL_EULER, step_frac=0.2), dict(max_steps=5), dict(max_length=0.3)):
+    for kw in (dict(), dict(flags=qsl.QSL_FLAG_KERNEL_V1), dict(method=qsl.QSL_EULER, step_frac=0.2), dict(max_steps=5),
+               dict(max_length=0.3), dict(max_length=0.3, flags=qsl.QSL_FLAG_KERNEL_V1)):
         gg, c = run_both(gs, Bc, "f64", ss, gs.lo, gs.hi, geometry=SPH, **kw)
         for d in (gg, c):
             for key in ("end_f", "end_b"):
@@ -93,4 +99,9 @@ def test_sph_argument_errors():
     for bad in (dict(method=qsl.QSL_CK45), dict(arith=qsl.QSL_ARITH_F32)):
         with pytest.raises(qsl.QslError):
             qsl.qsl_trace(f, seeds, qsl.make_trace_params((0, 0, 1), (1, 1, 2), **bad))
+    # the cell-frame kernel does not carry the geometry: the flag is ignored, the result is the spherical one
+    a = qsl.qsl_trace(f, seeds, qsl.make_trace_params((0, 0, 1), (1, 1, 2), flags=qsl.QSL_FLAG_KERNEL_FRAME))
+    b = qsl.qsl_trace(f, seeds, qsl.make_trace_params((0, 0, 1), (1, 1, 2)))
+    torch.cuda.synchronize()
+    assert torch.equal(a["L"], b["L"])
     f.destroy()
