@@ -101,53 +101,73 @@ static void finish_evaluate(const orc_field *F, const double val[4], double grad
 
 /* "The available interpolation schemes are trilinear, triquadratic (Dodgson 1997) and tricubic (Keys
  * 1981) ... The interpolation kernels cover 8, 27, or 64 vertices neighboring that cell"; eq. (3): the kernels are
- * functions of (x - x_c)/h_c of the cell containing x, whatever the spacing of the neighbouring cells.  Reading A18:
- *  tricubic     Keys' cubic convolution (a = -1/2) on the nodes i-1 .. i+2 of each axis, t = (x - x_i)/h_i:
- *               w = ((-t^3 + 2t^2 - t)/2, (3t^3 - 5t^2 + 2)/2, (-3t^3 + 4t^2 + t)/2, (t^3 - t^2)/2);
- *               a node outside the grid takes Keys' boundary value f_-1 = 3 f_0 - 3 f_1 + f_2 (mirrored at the top);
- *  triquadratic Dodgson's interpolating quadratic (r = 1) on the node j nearest to x (t >= 1/2 -> j = i + 1) and its
- *               two neighbours, s = t - (j - i): w = (s^2 - s/2, 1 - 2 s^2, s^2 + s/2);
- *               a node outside the grid takes the linear extrapolation f_-1 = 2 f_0 - f_1 (mirrored at the top).
- * The gradient acts on the kernels only: d w/dx = w'(t)/h.  Returns the number of stencil nodes. */
-static int axis_stencil(int order, int n, int i, double t, double h, int idx[4], double w[4], double dw[4])
+ * functions of (x - x_c)/h_c of the cell containing x, whatever the spacing of the neighbouring cells.  Reading A18,
+ * written out as its plain definition: per axis the interpolant is  sum_nodes f(node) K(s_node),  s_node = signed
+ * distance from the node to x in units of the cell containing x, K the published one-dimensional kernel:
+ *  tricubic     Keys' cubic convolution kernel with a = -1/2:
+ *               K(s) = 3/2 |s|^3 - 5/2 |s|^2 + 1 (|s| <= 1),  -1/2 |s|^3 + 5/2 |s|^2 - 4 |s| + 2 (1 < |s| < 2),  0 beyond,
+ *               on the nodes i-1 .. i+2 (s = t+1, t, t-1, t-2 with t = (x - x_i)/h_i);
+ *  triquadratic Dodgson's interpolating quadratic kernel (r = 1):
+ *               K(s) = 1 - 2 s^2 (|s| <= 1/2),  s^2 - 5/2 |s| + 3/2 (1/2 < |s| <= 3/2),  0 beyond,
+ *               on the node j nearest to x (t >= 1/2 -> j = i + 1) and its two neighbours.
+ * The gradient acts on the kernels only: d/dx K((x - x_node)/h) = K'(s)/h. */
+static double keys_kernel(double s, double *dk)
+{
+    const double a = fabs(s), sg = s < 0.0 ? -1.0 : 1.0;
+    if (a <= 1.0) { *dk = sg * (4.5 * a * a - 5.0 * a); return (1.5 * a * a * a - 2.5 * a * a) + 1.0; }
+    if (a < 2.0) { *dk = sg * ((-1.5 * a * a + 5.0 * a) - 4.0); return ((-0.5 * a * a * a + 2.5 * a * a) - 4.0 * a) + 2.0; }
+    *dk = 0.0; return 0.0;
+}
+
+/* The kernel is C0 with a kink at |s| = 1/2: which piece applies there is decided by the choice of the nearest node (the
+ * tie rule t >= 1/2 -> j = i + 1 of A18), so the caller says whether the node is that centre node. */
+static double dodgson_kernel(double s, int centre, double *dk)
+{
+    const double a = fabs(s), sg = s < 0.0 ? -1.0 : 1.0;
+    if (centre) { *dk = -4.0 * s; return 1.0 - 2.0 * s * s; }
+    if (a <= 1.5) { *dk = sg * (2.0 * a - 2.5); return (a * a - 2.5 * a) + 1.5; }
+    *dk = 0.0; return 0.0;
+}
+
+/* Reading A18, boundary rule: a stencil node outside the grid takes the extrapolated VALUE
+ *   tricubic (Keys 1981, his boundary condition):  f_-1 = 3 f_0 - 3 f_1 + f_2,  f_n = 3 f_{n-1} - 3 f_{n-2} + f_{n-3};
+ *   triquadratic (linear extrapolation):           f_-1 = 2 f_0 - f_1,          f_n = 2 f_{n-1} - f_{n-2},
+ * applied axis by axis (x, then y, then z) to the packed samples (b^_x, b^_y, b^_z, |B|). */
+static void sample_ext(const orc_field *F, int ix, int iy, int iz, double out[4])
+{
+    const int nn[3] = { F->nx, F->ny, F->nz };
+    int id[3] = { ix, iy, iz };
+    for (int d = 0; d < 3; ++d) {
+        if (id[d] >= 0 && id[d] <= nn[d] - 1) continue;
+        const int e = id[d] < 0 ? 0 : nn[d] - 1, st = id[d] < 0 ? 1 : -1;      /* edge node and the inward direction */
+        double f0[4], f1[4], f2[4];
+        int q[3] = { id[0], id[1], id[2] };
+        q[d] = e;          sample_ext(F, q[0], q[1], q[2], f0);
+        q[d] = e + st;     sample_ext(F, q[0], q[1], q[2], f1);
+        if (F->order == ORC_TRICUBIC) {
+            q[d] = e + 2 * st; sample_ext(F, q[0], q[1], q[2], f2);
+            for (int c = 0; c < 4; ++c) out[c] = (3.0 * f0[c] - 3.0 * f1[c]) + f2[c];
+        } else {
+            for (int c = 0; c < 4; ++c) out[c] = 2.0 * f0[c] - f1[c];
+        }
+        return;
+    }
+    const double *sp = F->packed + 4 * (((long long)iz * F->ny + iy) * F->nx + ix);
+    for (int c = 0; c < 4; ++c) out[c] = sp[c];
+}
+
+/* Stencil of one axis: first node index (may be -1, last may be n: sample_ext supplies the value), kernel weights and
+ * their x-derivatives.  Returns the number of stencil nodes. */
+static int axis_stencil(int order, int i, double t, double h, int *first, double w[4], double dw[4])
 {
     if (order == ORC_TRICUBIC) {
-        const double t2 = t * t, t3 = t2 * t;
-        w[0] = 0.5 * ((-t3 + 2.0 * t2) - t);        dw[0] = 0.5 * ((-3.0 * t2 + 4.0 * t) - 1.0);
-        w[1] = 0.5 * ((3.0 * t3 - 5.0 * t2) + 2.0); dw[1] = 0.5 * (9.0 * t2 - 10.0 * t);
-        w[2] = 0.5 * ((-3.0 * t3 + 4.0 * t2) + t);  dw[2] = 0.5 * ((-9.0 * t2 + 8.0 * t) + 1.0);
-        w[3] = 0.5 * (t3 - t2);                     dw[3] = 0.5 * (3.0 * t2 - 2.0 * t);
-        for (int k = 0; k < 4; ++k) { idx[k] = i - 1 + k; dw[k] /= h; }
-        if (idx[0] < 0) {                            /* f_-1 = 3 f_0 - 3 f_1 + f_2 */
-            w[1] += 3.0 * w[0]; w[2] -= 3.0 * w[0]; w[3] += w[0]; w[0] = 0.0;
-            dw[1] += 3.0 * dw[0]; dw[2] -= 3.0 * dw[0]; dw[3] += dw[0]; dw[0] = 0.0;
-            idx[0] = 0;
-        }
-        if (idx[3] > n - 1) {                        /* f_n = 3 f_{n-1} - 3 f_{n-2} + f_{n-3} */
-            w[2] += 3.0 * w[3]; w[1] -= 3.0 * w[3]; w[0] += w[3]; w[3] = 0.0;
-            dw[2] += 3.0 * dw[3]; dw[1] -= 3.0 * dw[3]; dw[0] += dw[3]; dw[3] = 0.0;
-            idx[3] = n - 1;
-        }
+        *first = i - 1;
+        for (int k = 0; k < 4; ++k) { w[k] = keys_kernel(t - (double)(k - 1), &dw[k]); dw[k] /= h; }
         return 4;
     }
-    /* ORC_TRIQUADRATIC */
-    const int up = t >= 0.5 ? 1 : 0;
-    const int j = i + up;
-    const double s = t - (double)up;
-    w[0] = s * s - 0.5 * s;   dw[0] = (2.0 * s - 0.5) / h;
-    w[1] = 1.0 - 2.0 * s * s; dw[1] = (-4.0 * s) / h;
-    w[2] = s * s + 0.5 * s;   dw[2] = (2.0 * s + 0.5) / h;
-    for (int k = 0; k < 3; ++k) idx[k] = j - 1 + k;
-    if (idx[0] < 0) {                                /* f_-1 = 2 f_0 - f_1 */
-        w[1] += 2.0 * w[0]; w[2] -= w[0]; w[0] = 0.0;
-        dw[1] += 2.0 * dw[0]; dw[2] -= dw[0]; dw[0] = 0.0;
-        idx[0] = 0;
-    }
-    if (idx[2] > n - 1) {                            /* f_n = 2 f_{n-1} - f_{n-2} */
-        w[1] += 2.0 * w[2]; w[0] -= w[2]; w[2] = 0.0;
-        dw[1] += 2.0 * dw[2]; dw[0] -= dw[2]; dw[2] = 0.0;
-        idx[2] = n - 1;
-    }
+    const int j = t >= 0.5 ? i + 1 : i;              /* nearest node */
+    *first = j - 1;
+    for (int k = 0; k < 3; ++k) { w[k] = dodgson_kernel(t - (double)(j - 1 + k - i), k == 1, &dw[k]); dw[k] /= h; }
     return 3;
 }
 
@@ -156,22 +176,21 @@ void orc_evaluate(const orc_field *F, const double x[3], double b[3], double J[9
     int i[3]; double t[3], h[3];
     for (int d = 0; d < 3; ++d) locate_axis(F, d, x[d], &i[d], &t[d], &h[d]);
     if (F->order == ORC_TRIQUADRATIC || F->order == ORC_TRICUBIC) {
-        int idx[3][4], cnt[3]; double ww[3][4], dww[3][4];
-        const int nn[3] = { F->nx, F->ny, F->nz };
-        for (int d = 0; d < 3; ++d) cnt[d] = axis_stencil(F->order, nn[d], i[d], t[d], h[d], idx[d], ww[d], dww[d]);
+        int first[3], cnt[3]; double ww[3][4], dww[3][4];
+        for (int d = 0; d < 3; ++d) cnt[d] = axis_stencil(F->order, i[d], t[d], h[d], &first[d], ww[d], dww[d]);
         double val[4] = { 0, 0, 0, 0 }, grad[4][3] = { { 0 } };
         for (int c = 0; c < cnt[2]; ++c)
             for (int bb = 0; bb < cnt[1]; ++bb)
                 for (int a = 0; a < cnt[0]; ++a) {
-                    const long long p = ((long long)idx[2][c] * F->ny + idx[1][bb]) * F->nx + idx[0][a];
-                    const double *s = F->packed + 4 * p;
+                    double sv[4];
+                    sample_ext(F, first[0] + a, first[1] + bb, first[2] + c, sv);
                     const double f = ww[0][a] * ww[1][bb] * ww[2][c];
                     const double f0 = dww[0][a] * ww[1][bb] * ww[2][c];
                     const double f1 = ww[0][a] * dww[1][bb] * ww[2][c];
                     const double f2 = ww[0][a] * ww[1][bb] * dww[2][c];
                     for (int q = 0; q < 4; ++q) {
-                        val[q] += s[q] * f;
-                        grad[q][0] += s[q] * f0; grad[q][1] += s[q] * f1; grad[q][2] += s[q] * f2;
+                        val[q] += sv[q] * f;
+                        grad[q][0] += sv[q] * f0; grad[q][1] += sv[q] * f1; grad[q][2] += sv[q] * f2;
                     }
                 }
         finish_evaluate(F, val, grad, b, J, m);

@@ -6,6 +6,7 @@ There is no CPU fallback: if the shared library is missing or no CUDA device is 
 from __future__ import annotations
 
 import ctypes as C
+import functools
 import math
 import os
 
@@ -90,6 +91,19 @@ def _stream_ptr(stream=None):
     return C.c_void_p(s.cuda_stream)
 
 
+def _on_stream(fn):
+    """Runs a binding call with its `stream=` argument as torch's current stream, so that the tensors the call allocates
+    (outputs, scratch) belong to that stream in the caching allocator and every torch-side operation next to the libqsl
+    launch is ordered with it."""
+    @functools.wraps(fn)
+    def wrapped(*args, stream=None, **kw):
+        if stream is None or stream == torch.cuda.current_stream():
+            return fn(*args, stream=stream, **kw)
+        with torch.cuda.stream(stream):
+            return fn(*args, stream=stream, **kw)
+    return wrapped
+
+
 def _dev_f64(t, name):
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
         raise QslError("%s must be a contiguous CUDA float64 tensor" % name)
@@ -130,8 +144,9 @@ class Field:
 
     def export(self, stream=None) -> torch.Tensor:
         dt = torch.float32 if self.sample_type == QSL_F32 else torch.float64
-        out = torch.empty((self.nz, self.ny, self.nx, 4), dtype=dt, device="cuda")
-        _check(lib().qsl_field_export(self.handle, C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "qsl_field_export")
+        with torch.cuda.stream(stream if stream is not None else torch.cuda.current_stream()):
+            out = torch.empty((self.nz, self.ny, self.nx, 4), dtype=dt, device="cuda")
+            _check(lib().qsl_field_export(self.handle, C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "qsl_field_export")
         return out
 
     def destroy(self):
@@ -146,6 +161,7 @@ class Field:
             pass
 
 
+@_on_stream
 def qsl_field_create(nx, ny, nz, bx, by, bz, *, lo=None, hi=None, xs=None, ys=None, zs=None,
                      sample_type=QSL_F64, interp_mode=QSL_NORMALIZE_FIRST, layout=QSL_LAYOUT_CELL_TABLE,
                      interp_order=QSL_TRILINEAR, geometry=QSL_CARTESIAN, stream=None) -> Field:
@@ -190,6 +206,7 @@ def make_trace_params(box_lo, box_hi, *, method=QSL_RK4, step_frac=0.25, mode=QS
                         float(null_eps), int(flags), float(tol))
 
 
+@_on_stream
 def qsl_trace(field: Field, seeds: torch.Tensor, params: _TraceParams, *, outputs=DEFAULT_OUTPUTS, out=None,
               total_steps: torch.Tensor | None = None, stream=None) -> dict:
     """Traces `seeds` (CUDA float64 (n,3)).  Returns a dict of CUDA tensors for the requested `outputs`
@@ -212,6 +229,7 @@ def qsl_trace(field: Field, seeds: torch.Tensor, params: _TraceParams, *, output
     return res
 
 
+@_on_stream
 def qsl_fledge_dense(L: torch.Tensor, ndim: int, *, out=None, stream=None) -> torch.Tensor:
     """L: CUDA float64 map of shape (d1, d0) or (d2, d1, d0) (axis 0 fastest).  Returns S of the same shape."""
     _require_cuda()
@@ -224,6 +242,7 @@ def qsl_fledge_dense(L: torch.Tensor, ndim: int, *, out=None, stream=None) -> to
     return S
 
 
+@_on_stream
 def qsl_fledge_sparse(lattice, level: int, L0: torch.Tensor, coords: list, Ls: list, child_base: list, *, stream=None):
     """Sparse FLEDGE at `level` >= 1.  coords[l], Ls[l] (l = 1..level) and child_base[l] (l = 0..level-1) are CUDA
     tensors as produced by qsl_refine / qsl_trace; index 0 of coords / Ls is ignored."""
@@ -246,6 +265,7 @@ def qsl_fledge_sparse(lattice, level: int, L0: torch.Tensor, coords: list, Ls: l
     return S
 
 
+@_on_stream
 def qsl_select(S: torch.Tensor, p: float, *, out=None, stream=None) -> torch.Tensor:
     """Nearest-rank order statistic of the finite values of S; returns a CUDA float64[1] tensor (no host sync)."""
     _require_cuda()
@@ -255,6 +275,7 @@ def qsl_select(S: torch.Tensor, p: float, *, out=None, stream=None) -> torch.Ten
     return tau
 
 
+@_on_stream
 def qsl_refine(lattice, level: int, coords, S: torch.Tensor, tau: torch.Tensor, *, capacity=None, stream=None):
     """Refines the cells with S > tau.  coords: CUDA int32 (n, ndim) or None for the dense level-0 lattice.
     Returns (child_coords int32 (m, ndim), child_seeds float64 (m, 3), child_base int64 (n,))."""
@@ -290,6 +311,7 @@ def qsl_hilbert_bits(lattice, R: int) -> int:
     return int(b)
 
 
+@_on_stream
 def qsl_hilbert_level0(lattice, R: int, *, stream=None):
     """(coords int32 (n, ndim), seeds float64 (n, 3)) of the level-0 samples in dense order."""
     _require_cuda()
@@ -304,6 +326,7 @@ def qsl_hilbert_level0(lattice, R: int, *, stream=None):
     return coords, seeds
 
 
+@_on_stream
 def qsl_hilbert_keys(coords: torch.Tensor, bits: int, shift: int = 0, *, stream=None) -> torch.Tensor:
     """coords: CUDA int32 (n, ndim).  Returns the keys as CUDA int64 (they are below 2^63)."""
     _require_cuda()
@@ -316,6 +339,7 @@ def qsl_hilbert_keys(coords: torch.Tensor, bits: int, shift: int = 0, *, stream=
     return keys
 
 
+@_on_stream
 def qsl_hilbert_cells(keys: torch.Tensor, ndim: int, bits: int, shift: int = 0, *, stream=None) -> torch.Tensor:
     _require_cuda()
     n = int(keys.numel())
@@ -327,6 +351,7 @@ def qsl_hilbert_cells(keys: torch.Tensor, ndim: int, bits: int, shift: int = 0, 
     return coords
 
 
+@_on_stream
 def qsl_sort_keys64(keys: torch.Tensor, key_bits: int = 64, *, stream=None) -> torch.Tensor:
     """Sorts `keys` (CUDA int64, non-negative) in place; returns the permutation (CUDA int32)."""
     _require_cuda()
@@ -338,6 +363,7 @@ def qsl_sort_keys64(keys: torch.Tensor, key_bits: int = 64, *, stream=None) -> t
     return perm
 
 
+@_on_stream
 def qsl_gather(perm: torch.Tensor, src: torch.Tensor, *, stream=None) -> torch.Tensor:
     """dst[i] = src[perm[i]] along the first axis (rows of a multiple of 4 bytes)."""
     _require_cuda()
@@ -350,6 +376,7 @@ def qsl_gather(perm: torch.Tensor, src: torch.Tensor, *, stream=None) -> torch.T
     return dst
 
 
+@_on_stream
 def qsl_hilbert_refine(lattice, R: int, shift: int, keys: torch.Tensor, L: torch.Tensor, thr: float, *, capacity=None,
                        stream=None):
     """One refinement pass.  Returns (left int64 (m,), new_coords int32 (m, ndim), new_seeds float64 (m, 3))."""
@@ -366,6 +393,7 @@ def qsl_hilbert_refine(lattice, R: int, shift: int, keys: torch.Tensor, L: torch
     return left[: m.value], nc[: m.value], ns[: m.value]
 
 
+@_on_stream
 def qsl_hilbert_merge(left: torch.Tensor, old: torch.Tensor, new: torch.Tensor, *, stream=None) -> torch.Tensor:
     _require_cuda()
     n_old, n_new = int(old.shape[0]), int(new.shape[0])
@@ -380,6 +408,7 @@ def qsl_hilbert_merge(left: torch.Tensor, old: torch.Tensor, new: torch.Tensor, 
     return out
 
 
+@_on_stream
 def qsl_hilbert_convert(lattice, R: int, r: int, keys: torch.Tensor, Q: torch.Tensor, *, stream=None) -> torch.Tensor:
     """Dense Q map on the lattice n_d 2^r, shape (d1, d0) or (d2, d1, d0)."""
     _require_cuda()

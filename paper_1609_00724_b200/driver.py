@@ -12,11 +12,18 @@ import torch
 from . import binding as B
 
 
+@B._on_stream
 def adaptive_map(field, lattice, seeds0, params_L, params_LQ, n_levels: int, p: float, *, stream=None,
-                 outputs=("L", "q_perp", "q_bnd", "status"), max_children=None):
+                 outputs=("L", "q_perp", "q_bnd", "status"), max_children=None, on_level=None, keep=None):
     """Runs level 0 (dense, `params_L`) and `n_levels` refinement levels (`params_LQ`).
 
     seeds0: CUDA float64 (n0*n1*n2, 3) level-0 seeds in dense index order.
+    `stream`: every libqsl launch AND every torch-side operation of the loop (allocations, the step-counter sums) run
+    on it (it is made torch's current stream for the duration of the call).
+    `on_level(level, coords, seeds, out)` is called after the trace of every refined level (1..n_levels) with that
+    level's device tensors (e.g. to copy a level to the host or to disk while the next one is traced); `keep`, a subset of
+    `outputs`, names what stays in the returned dict afterwards (default: everything; "L" is always kept, the sparse
+    FLEDGE of the next level reads it) - 3-D maps with hundreds of millions of refined samples need this.
     Returns a dict: L0 (dense map), S0, tau (CUDA float64[1]) and per-level lists coords / seeds / out (trace outputs) /
     S / child_base, plus `total_steps` (CUDA int64[1], summed over all levels) and `steps_by_mode` (CUDA int64[2]: RK
     steps of the L-only level-0 pass and of the L+Q passes over the refined seeds).
@@ -42,6 +49,10 @@ def adaptive_map(field, lattice, seeds0, params_L, params_LQ, n_levels: int, p: 
             break
         o = B.qsl_trace(field, cs, params_LQ, outputs=outputs, total_steps=steps, stream=stream)
         acc[1:2] += steps
+        if on_level is not None:
+            on_level(level + 1, cc, cs, o)
+        if keep is not None:
+            o = {k: v for k, v in o.items() if k == "L" or k in keep}
         res["out"].append(o)
         Ls.append(o["L"])
         if level + 1 < n_levels:
@@ -53,6 +64,7 @@ def adaptive_map(field, lattice, seeds0, params_L, params_LQ, n_levels: int, p: 
     return res
 
 
+@B._on_stream
 def hilbert_map(lattice, R: int, thr: float, passes: int, shift: int, trace_fn, *, stream=None):
     """The paper's own refinement loop (reading A17): orchestration only, every step is a
     libqsl call.  Level-0 samples ordered along the Hilbert curve; per pass a refinement on the curve (a new sample halfway

@@ -155,3 +155,38 @@ def test_refinement_configs_full_size_level0(name):
     flagged = int((cb >= 0).sum())
     assert flagged << ndim == at and 0 < flagged <= max_flagged
     fg.destroy()
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg5"])
+def test_refined_levels_full_size_sampled(name):
+    """BASELINE.json configs[2] / [4] at full size, the product they deliver: `adaptive_map` as
+    bench.py runs it (level 0 L-only, FLEDGE, p95, 4 / 3 levels), and at every refined level the L + Q trace of a sample
+    of the children (every k-th child plus one contiguous run) compared element by element with the oracle tracing the
+    same seed positions, at the north_star gates (99.9 %).  The children sit on the quasi-connectivity boundaries."""
+    cfg = qi.make_config(name)
+    lat = cfg["lattice"]
+    fg = gpu_field(cfg["grid"], cfg["B"], cfg["sample_type"], 0)
+    fc = cpu_field(cfg["grid"], cfg["B"], cfg["sample_type"], 0)
+    mk = lambda m: qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=m, step_frac=cfg["step_frac"],
+                                         max_steps=cfg["max_steps"], null_eps=cfg["null_eps"])
+    picked = {}
+
+    def on_level(level, coords, seeds, out):
+        n = int(seeds.shape[0])
+        idx = _sample(n, max(1, n // 6000))
+        picked[level] = (n, seeds[torch.from_numpy(idx).cuda()].cpu().numpy(), _pick(out, idx))
+
+    res = qsl.adaptive_map(fg, lat, torch.from_numpy(cfg["seeds"]).cuda(), mk(qsl.QSL_TRACE_L), mk(qsl.QSL_TRACE_LQ),
+                           cfg["levels"], cfg["p"], outputs=qsl.DEFAULT_OUTPUTS, on_level=on_level, keep=("L",))
+    torch.cuda.synchronize()
+    assert sorted(picked) == list(range(1, cfg["levels"] + 1)), "every level must have refined"
+    sizes = [picked[l][0] for l in sorted(picked)]
+    assert all(b > a for a, b in zip(sizes, sizes[1:])), sizes          # the boundaries' measure grows with the resolution
+    assert sum(int(s.shape[0]) for s in res["seeds"][1:]) == sum(sizes)
+    for level in sorted(picked):
+        n, seeds, g = picked[level]
+        c = oracle.trace(fc, seeds, cfg["box_lo"], cfg["box_hi"], mode=oracle.TRACE_LQ, step_frac=cfg["step_frac"],
+                         max_steps=cfg["max_steps"], null_eps=cfg["null_eps"])
+        rep = compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], label="%s level %d of %d children" % (name, level, n))
+        assert rep["n"] >= 6000
+    fg.destroy()

@@ -159,3 +159,31 @@ def test_paper_loop_on_a_traced_field():
     m = qsl.qsl_hilbert_convert(lat, R, R, got["keys"], got["Q"])
     assert m.shape == (int(lat.n[1]) << R, int(lat.n[0]) << R) and bool(torch.isfinite(m).all())
     f.destroy()
+
+
+def test_hilbert_map_on_a_non_default_stream():
+    """the loop on a side stream (default stream kept busy) gives the sample set of the default-stream run."""
+    cfg = qi.make_config("cfg3", 1.0 / 16)
+    lat, grid = cfg["lattice"], cfg["grid"]
+    dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda() for a in cfg["B"]]
+    f = qsl.qsl_field_create(grid.nx, grid.ny, grid.nz, *dev, lo=grid.lo, hi=grid.hi)
+    p = qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], max_steps=cfg["max_steps"])
+
+    def tg(seeds):                                                             # stream=None: torch's current stream
+        o = qsl.qsl_trace(f, seeds, p, outputs=("L", "q_perp"))
+        return o["L"], o["q_perp"]
+
+    ref = qsl.hilbert_map(lat, 2, 0.3, 2, 3, tg)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    busy = torch.empty(1 << 26, dtype=torch.float32, device="cuda")
+    for _ in range(8):
+        busy.normal_()
+    got = qsl.hilbert_map(lat, 2, 0.3, 2, 3, tg, stream=side)
+    side.synchronize()
+    assert got["counts"] == ref["counts"]
+    for k in ("keys", "coords", "L", "Q"):
+        assert torch.equal(got[k].view(torch.int64 if got[k].dtype == torch.float64 else got[k].dtype),
+                           ref[k].view(torch.int64 if ref[k].dtype == torch.float64 else ref[k].dtype)), k
+    torch.cuda.synchronize()
+    f.destroy()
