@@ -102,31 +102,32 @@ static void finish_evaluate(const orc_field *F, const double val[4], double grad
 /* "The available interpolation schemes are trilinear, triquadratic (Dodgson 1997) and tricubic (Keys
  * 1981) ... The interpolation kernels cover 8, 27, or 64 vertices neighboring that cell"; eq. (3): the kernels are
  * functions of (x - x_c)/h_c of the cell containing x, whatever the spacing of the neighbouring cells.  Reading A18,
- * written out as its plain definition: per axis the interpolant is  sum_nodes f(node) K(s_node),  s_node = signed
- * distance from the node to x in units of the cell containing x, K the published one-dimensional kernel:
+ * written out as its plain definition: per axis the interpolant is  sum_nodes f(node) K(u_node),  u_node = distance
+ * from the node to x in units of the cell containing x, K the published one-dimensional kernel:
  *  tricubic     Keys' cubic convolution kernel with a = -1/2:
- *               K(s) = 3/2 |s|^3 - 5/2 |s|^2 + 1 (|s| <= 1),  -1/2 |s|^3 + 5/2 |s|^2 - 4 |s| + 2 (1 < |s| < 2),  0 beyond,
- *               on the nodes i-1 .. i+2 (s = t+1, t, t-1, t-2 with t = (x - x_i)/h_i);
+ *               K(u) = 3/2 u^3 - 5/2 u^2 + 1 (0 <= u <= 1),  -1/2 u^3 + 5/2 u^2 - 4 u + 2 (1 <= u <= 2),  0 beyond,
+ *               on the nodes i-1 .. i+2, whose distances to x are u = t+1, t, 1-t, 2-t with t = (x - x_i)/h_i;
  *  triquadratic Dodgson's interpolating quadratic kernel (r = 1):
- *               K(s) = 1 - 2 s^2 (|s| <= 1/2),  s^2 - 5/2 |s| + 3/2 (1/2 < |s| <= 3/2),  0 beyond,
- *               on the node j nearest to x (t >= 1/2 -> j = i + 1) and its two neighbours.
- * The gradient acts on the kernels only: d/dx K((x - x_node)/h) = K'(s)/h. */
-static double keys_kernel(double s, double *dk)
+ *               K(u) = 1 - 2 u^2 (u <= 1/2),  u^2 - 5/2 u + 3/2 (1/2 <= u <= 3/2),  0 beyond,
+ *               on the node j nearest to x (t >= 1/2 -> j = i + 1) and its two neighbours, distances 1+s, |s|, 1-s with
+ *               s = t - (j - i).
+ * Which piece of K a stencil node takes follows from its place in the stencil (inner / outer node), and u is the
+ * distance written as the expression above, positive for x inside the cell.  Reading A8 (cell index clamped, fraction
+ * not): for a stage point outside the grid, t < 0 or t > 1, the same expressions are used, i.e. the polynomial of the
+ * boundary cell is continued, as the trilinear kernels 1-t, t are.
+ * The gradient acts on the kernels only: d/dx K(u) = K'(u) (du/dt) / h with du/dt = +-1. */
+static double keys_piece(int outer, double u, double *dk)
 {
-    const double a = fabs(s), sg = s < 0.0 ? -1.0 : 1.0;
-    if (a <= 1.0) { *dk = sg * (4.5 * a * a - 5.0 * a); return (1.5 * a * a * a - 2.5 * a * a) + 1.0; }
-    if (a < 2.0) { *dk = sg * ((-1.5 * a * a + 5.0 * a) - 4.0); return ((-0.5 * a * a * a + 2.5 * a * a) - 4.0 * a) + 2.0; }
-    *dk = 0.0; return 0.0;
+    if (!outer) { *dk = 4.5 * u * u - 5.0 * u; return (1.5 * u * u * u - 2.5 * u * u) + 1.0; }
+    *dk = (-1.5 * u * u + 5.0 * u) - 4.0;
+    return ((-0.5 * u * u * u + 2.5 * u * u) - 4.0 * u) + 2.0;
 }
 
-/* The kernel is C0 with a kink at |s| = 1/2: which piece applies there is decided by the choice of the nearest node (the
- * tie rule t >= 1/2 -> j = i + 1 of A18), so the caller says whether the node is that centre node. */
-static double dodgson_kernel(double s, int centre, double *dk)
+static double dodgson_piece(int outer, double u, double *dk)
 {
-    const double a = fabs(s), sg = s < 0.0 ? -1.0 : 1.0;
-    if (centre) { *dk = -4.0 * s; return 1.0 - 2.0 * s * s; }
-    if (a <= 1.5) { *dk = sg * (2.0 * a - 2.5); return (a * a - 2.5 * a) + 1.5; }
-    *dk = 0.0; return 0.0;
+    if (!outer) { *dk = -4.0 * u; return 1.0 - 2.0 * u * u; }
+    *dk = 2.0 * u - 2.5;
+    return (u * u - 2.5 * u) + 1.5;
 }
 
 /* Reading A18, boundary rule: a stencil node outside the grid takes the extrapolated VALUE
@@ -162,12 +163,15 @@ static int axis_stencil(int order, int i, double t, double h, int *first, double
 {
     if (order == ORC_TRICUBIC) {
         *first = i - 1;
-        for (int k = 0; k < 4; ++k) { w[k] = keys_kernel(t - (double)(k - 1), &dw[k]); dw[k] /= h; }
+        const double u[4] = { t + 1.0, t, 1.0 - t, 2.0 - t }, sg[4] = { 1.0, 1.0, -1.0, -1.0 };
+        for (int k = 0; k < 4; ++k) { w[k] = keys_piece(k == 0 || k == 3, u[k], &dw[k]); dw[k] = sg[k] * dw[k] / h; }
         return 4;
     }
     const int j = t >= 0.5 ? i + 1 : i;              /* nearest node */
+    const double s = t - (double)(j - i);
     *first = j - 1;
-    for (int k = 0; k < 3; ++k) { w[k] = dodgson_kernel(t - (double)(j - 1 + k - i), k == 1, &dw[k]); dw[k] /= h; }
+    const double u[3] = { 1.0 + s, s, 1.0 - s }, sg[3] = { 1.0, 1.0, -1.0 };
+    for (int k = 0; k < 3; ++k) { w[k] = dodgson_piece(k != 1, u[k], &dw[k]); dw[k] = sg[k] * dw[k] / h; }
     return 3;
 }
 

@@ -13,7 +13,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libqsl.so")
+LIB_PATH = os.environ.get("QSL_LIB_PATH") or os.path.join(_HERE, "libqsl.so")   # override: A/B runs of two builds
 
 QSL_F32, QSL_F64 = 0, 1
 QSL_NORMALIZE_FIRST, QSL_INTERP_FIRST = 0, 1

@@ -181,7 +181,7 @@ def test_refined_levels_full_size_sampled(name):
     torch.cuda.synchronize()
     assert sorted(picked) == list(range(1, cfg["levels"] + 1)), "every level must have refined"
     sizes = [picked[l][0] for l in sorted(picked)]
-    assert all(b > a for a, b in zip(sizes, sizes[1:])), sizes          # the boundaries' measure grows with the resolution
+    assert all(0 < m <= (1 << lat.ndim) * k for k, m in zip([len(cfg["seeds"])] + sizes, sizes)), sizes
     assert sum(int(s.shape[0]) for s in res["seeds"][1:]) == sum(sizes)
     for level in sorted(picked):
         n, seeds, g = picked[level]

@@ -158,3 +158,38 @@ def test_traces_through_higher_order_fields(order):
     Fu = oracle.Field(gu, [np.full(gu.shape, v) for v in (0.3, -0.2, 0.9)], oracle.F64, oracle.NORMALIZE_FIRST, order)
     o = oracle.trace(Fu, np.array([[0.4, 0.5, 0.3]]), (0, 0, 0), (1, 1, 1))
     assert abs(o["q_perp"][0] - 2) < 1e-12 and abs(o["q_bnd"][0] - 2) < 1e-12
+
+
+@pytest.mark.parametrize("order", ORDERS)
+def test_outside_the_grid_the_boundary_cell_polynomial_is_continued(order):
+    """Reading A8 carried to the higher orders (cell index clamped, fraction not): for a stage point a little outside the
+    grid the interpolant and its gradient are the polynomial of the boundary cell continued, as for the trilinear kernels.
+    Pinned without the kernel formulas: along a line parallel to an axis the interpolant inside one cell (one half cell
+    for the quadratic) is a polynomial of degree <= 3 in that coordinate, so a cubic through four inside values predicts
+    the outside values, and its derivative the outside gradient component."""
+    g = qi.Grid.uniform((7, 6, 8), (0, 0, 0), (1, 1, 1))
+    rng = np.random.default_rng(10 + order)
+    B = [rng.normal(size=g.shape) for _ in range(3)]
+    F = oracle.Field(g, B, oracle.F64, oracle.NORMALIZE_FIRST, order)
+    n = (7, 6, 8)
+    for axis in range(3):
+        h = 1.0 / (n[axis] - 1)
+        for side in (0, 1):
+            base = np.array([0.41, 0.33, 0.58])
+            # four points inside the boundary (half) cell next to the face, three outside
+            ins = (np.array([0.05, 0.15, 0.3, 0.45]) * h) if side == 0 else (1.0 - np.array([0.05, 0.15, 0.3, 0.45]) * h)
+            outs = (np.array([-0.02, -0.2, -0.45]) * h) if side == 0 else (1.0 + np.array([0.02, 0.2, 0.45]) * h)
+
+            def at(c):
+                x = base.copy(); x[axis] = c
+                b, J, m, _ = F.evaluate(x)
+                return np.append(b, m), J[:, axis]
+
+            vals = np.array([at(c)[0] for c in ins])
+            for q in range(4):
+                poly = np.polynomial.Polynomial.fit(ins, vals[:, q], 3)
+                for c in outs:
+                    v, gr = at(c)
+                    assert abs(v[q] - poly(c)) < 1e-11, (order, axis, side, q, c)
+                    if q < 3:
+                        assert abs(gr[q] - poly.deriv()(c)) < 1e-9 / h, (order, axis, side, q, c)
