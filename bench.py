@@ -281,6 +281,13 @@ class Workload:
                                              max_steps=cfg["max_steps"], null_eps=cfg["null_eps"], flags=args.flags,
                                              arith=qsl.QSL_ARITH_F32 if self.f32 else qsl.QSL_ARITH_F64)
         self.pL, self.pLQ = mk(qsl.QSL_TRACE_L), mk(qsl.QSL_TRACE_LQ)
+        # samples handed out by hilbert_map are already ordered along a space-filling curve: no Morton sort inside qsl_trace
+        args_flags = args.flags
+        mkn = lambda m: qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=m, step_frac=cfg["step_frac"],
+                                              max_steps=cfg["max_steps"], null_eps=cfg["null_eps"],
+                                              flags=args_flags | qsl.QSL_FLAG_NO_SORT,
+                                              arith=qsl.QSL_ARITH_F32 if self.f32 else qsl.QSL_ARITH_F64)
+        self.pL_curve, self.pLQ_curve = mkn(qsl.QSL_TRACE_L), mkn(qsl.QSL_TRACE_LQ)
         self.outs = ("end_f", "end_b", "L", "q_perp", "q_bnd", "face_f", "face_b", "status")
         self.out_bufs, self.host_out, self.host_res, self.hstate = {}, {}, {}, {}
         self.tot = torch.zeros(1, dtype=torch.int64, device="cuda")
@@ -311,7 +318,6 @@ class Workload:
         r = qsl.adaptive_map(self.field, self.lat, self.seeds, self.pL, self.pLQ, self.levels, self.cfg["p"])
         self.last = {"L": r["L0"]}
         self.level_sizes = [self.n] + [int(s.shape[0]) for s in r["seeds"][1:]]
-        self.rmap = r
         return sum(self.level_sizes), r["steps_by_mode"]
 
     def hilbert_step(self):
@@ -324,10 +330,10 @@ class Workload:
         def tf(sd):
             calls[0] += 1
             if calls[0] == 1:
-                o = qsl.qsl_trace(self.field, sd, self.pL, outputs=("L",), total_steps=self.tot)
+                o = qsl.qsl_trace(self.field, sd, self.pL_curve, outputs=("L",), total_steps=self.tot)
                 acc[0:1] += self.tot
                 return o["L"], torch.full_like(o["L"], float("nan"))
-            o = qsl.qsl_trace(self.field, sd, self.pLQ, outputs=("L", "q_perp"), total_steps=self.tot)
+            o = qsl.qsl_trace(self.field, sd, self.pLQ_curve, outputs=("L", "q_perp"), total_steps=self.tot)
             acc[1:2] += self.tot
             return o["L"], o["q_perp"]
 

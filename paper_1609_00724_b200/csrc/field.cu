@@ -79,50 +79,59 @@ __global__ void __launch_bounds__(256) pack_kernel(long long n, const double *__
 // The coefficients are finite differences of the 8 corner samples (converted exactly to fp64) divided by the cell
 // edges; 24 doubles = 192 B per cell, component-major, cell index (k (ny-1) + j)(nx-1) + i.
 // O4 = double4 (192 B per cell, the fp64 kernels) or float4 (coefficients rounded to fp32, 96 B per cell, QSL_ARITH_F32).
+// Each block builds the entries of CT_THREADS consecutive cells (one thread per cell: 8 corner gathers that neighbouring
+// threads share through L1) into a shared-memory tile and then writes the tile - one contiguous run of global memory -
+// with fully coalesced stores; a thread storing its own 192 bytes directly makes every warp store touch 32 lines.
+constexpr int CT_THREADS = 128;
+constexpr int CT_PAD = 25;                       // tile row stride in coefficients: conflict-free column writes
 template <typename S4, typename O4>
-__global__ void __launch_bounds__(256) cell_table_kernel(FieldView fv, O4 *__restrict__ cells)
+__global__ void __launch_bounds__(CT_THREADS) cell_table_kernel(FieldView fv, O4 *__restrict__ cells)
 {
+    using E = decltype(O4().x);
+    __shared__ E tile[CT_THREADS * CT_PAD];
     const int cx = fv.nx - 1, cy = fv.ny - 1, cz = fv.nz - 1;
     const long long n_cells = (long long)cx * cy * cz;
-    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long n_tiles = (n_cells + CT_THREADS - 1) / CT_THREADS;
     const S4 *__restrict__ smp = (const S4 *)fv.samples;
-    for (; p < n_cells; p += stride) {
-        const int i = (int)(p % cx), j = (int)((p / cx) % cy), k = (int)(p / ((long long)cx * cy));
-        const double ihx = 1.0 / (fv.axis[0][i + 1] - fv.axis[0][i]), ihy = 1.0 / (fv.axis[1][j + 1] - fv.axis[1][j]),
-                     ihz = 1.0 / (fv.axis[2][k + 1] - fv.axis[2][k]);
-        const size_t base = ((size_t)k * fv.ny + j) * fv.nx + i, sy = (size_t)fv.nx, sz = (size_t)fv.nx * fv.ny;
-        const S4 s[8] = { smp[base], smp[base + 1], smp[base + sy], smp[base + sy + 1],
-                          smp[base + sz], smp[base + sz + 1], smp[base + sz + sy], smp[base + sz + sy + 1] };
-        double a[24];
+    E *__restrict__ out = reinterpret_cast<E *>(cells);
+    for (long long tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
+        const long long p = tl * CT_THREADS + threadIdx.x;
+        if (p < n_cells) {
+            const int i = (int)(p % cx), j = (int)((p / cx) % cy), k = (int)(p / ((long long)cx * cy));
+            const double ihx = 1.0 / (fv.axis[0][i + 1] - fv.axis[0][i]), ihy = 1.0 / (fv.axis[1][j + 1] - fv.axis[1][j]),
+                         ihz = 1.0 / (fv.axis[2][k + 1] - fv.axis[2][k]);
+            const size_t base = ((size_t)k * fv.ny + j) * fv.nx + i, sy = (size_t)fv.nx, sz = (size_t)fv.nx * fv.ny;
+            const S4 s[8] = { smp[base], smp[base + 1], smp[base + sy], smp[base + sy + 1],
+                              smp[base + sz], smp[base + sz + 1], smp[base + sz + sy], smp[base + sz + sy + 1] };
+            E *row = tile + threadIdx.x * CT_PAD;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            double v[8];
+            for (int c = 0; c < 3; ++c) {
+                double v[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) v[q] = c == 0 ? (double)s[q].x : (c == 1 ? (double)s[q].y : (double)s[q].z);
-            // finite differences along x, then y, then z (in place): v[m] becomes the coefficient of monomial m in t
+                for (int q = 0; q < 8; ++q) v[q] = c == 0 ? (double)s[q].x : (c == 1 ? (double)s[q].y : (double)s[q].z);
+                // finite differences along x, then y, then z (in place): v[m] becomes the coefficient of monomial m in t
 #pragma unroll
-            for (int q = 0; q < 8; q += 2) v[q + 1] -= v[q];
+                for (int q = 0; q < 8; q += 2) v[q + 1] -= v[q];
 #pragma unroll
-            for (int q = 0; q < 8; q += 4) { v[q + 2] -= v[q]; v[q + 3] -= v[q + 1]; }
+                for (int q = 0; q < 8; q += 4) { v[q + 2] -= v[q]; v[q + 3] -= v[q + 1]; }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) v[q + 4] -= v[q];
-            a[8 * c + 0] = v[0];
-            a[8 * c + 1] = v[1] * ihx;
-            a[8 * c + 2] = v[2] * ihy;
-            a[8 * c + 3] = v[3] * (ihx * ihy);
-            a[8 * c + 4] = v[4] * ihz;
-            a[8 * c + 5] = v[5] * (ihx * ihz);
-            a[8 * c + 6] = v[6] * (ihy * ihz);
-            a[8 * c + 7] = v[7] * ((ihx * ihy) * ihz);
+                for (int q = 0; q < 4; ++q) v[q + 4] -= v[q];
+                row[8 * c + 0] = (E)v[0];
+                row[8 * c + 1] = (E)(v[1] * ihx);
+                row[8 * c + 2] = (E)(v[2] * ihy);
+                row[8 * c + 3] = (E)(v[3] * (ihx * ihy));
+                row[8 * c + 4] = (E)(v[4] * ihz);
+                row[8 * c + 5] = (E)(v[5] * (ihx * ihz));
+                row[8 * c + 6] = (E)(v[6] * (ihy * ihz));
+                row[8 * c + 7] = (E)(v[7] * ((ihx * ihy) * ihz));
+            }
         }
-        O4 *o = cells + (size_t)p * 6;
-#pragma unroll
-        for (int q = 0; q < 6; ++q) {
-            O4 w;
-            w.x = (decltype(w.x))a[4 * q]; w.y = (decltype(w.x))a[4 * q + 1]; w.z = (decltype(w.x))a[4 * q + 2]; w.w = (decltype(w.x))a[4 * q + 3];
-            o[q] = w;
-        }
+        __syncthreads();
+        const long long first = tl * CT_THREADS;
+        const int live = (int)min((long long)CT_THREADS, n_cells - first) * 24;   // coefficients in this tile
+        E *__restrict__ dst = out + first * 24;
+        for (int g = threadIdx.x; g < live; g += CT_THREADS) dst[g] = tile[(g / 24) * CT_PAD + g % 24];
+        __syncthreads();
     }
 }
 
@@ -247,11 +256,11 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
         e = cudaMalloc(&f->d_cells, cbytes);
         if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
         f->bytes += cbytes;
-        const long long want = (n_cells + threads - 1) / threads, cap = (long long)sm_count() * 16;
+        const long long want = (n_cells + CT_THREADS - 1) / CT_THREADS, cap = (long long)sm_count() * 16;
         const int cblocks = (int)(want < cap ? want : cap);
         count_launch();
-        if (d->sample_type == QSL_F32) cell_table_kernel<float4, double4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
-        else cell_table_kernel<double4, double4><<<cblocks, threads, 0, s>>>(f->view, (double4 *)f->d_cells);
+        if (d->sample_type == QSL_F32) cell_table_kernel<float4, double4><<<cblocks, CT_THREADS, 0, s>>>(f->view, (double4 *)f->d_cells);
+        else cell_table_kernel<double4, double4><<<cblocks, CT_THREADS, 0, s>>>(f->view, (double4 *)f->d_cells);
         e = cudaGetLastError();
         if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
         f->view.cells = f->d_cells;
@@ -263,10 +272,10 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
         e = cudaMalloc(&f->d_cells32, cbytes);
         if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
         f->bytes += cbytes;
-        const long long want = (n_cells + threads - 1) / threads, cap = (long long)sm_count() * 16;
+        const long long want = (n_cells + CT_THREADS - 1) / CT_THREADS, cap = (long long)sm_count() * 16;
         const int cblocks = (int)(want < cap ? want : cap);
         count_launch();
-        cell_table_kernel<float4, float4><<<cblocks, threads, 0, s>>>(f->view, (float4 *)f->d_cells32);
+        cell_table_kernel<float4, float4><<<cblocks, CT_THREADS, 0, s>>>(f->view, (float4 *)f->d_cells32);
         e = cudaGetLastError();
         if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
     }

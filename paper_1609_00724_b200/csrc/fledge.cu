@@ -12,8 +12,11 @@ namespace qsl {
 constexpr int FL_THREADS = 128;
 constexpr int FL_VALID = 30;   // outputs per warp: lanes 1..30; lanes 0 and 31 carry the halo columns
 
+constexpr int FL_ROWS = 32;    // rows (axis 1) one warp marches over, keeping a rolling window of three rows in registers
+
 // Folds the axis-1 / axis-2 taps of one column.  a[o2][o1] are the clamped neighbours of the column.
 // A: smooth x smooth, B: diff along axis 1 (smooth along 2), C: diff along axis 2 (smooth along 1).
+// (used by the sparse levels, where every neighbour is a look-up)
 template <int NDIM>
 __device__ __forceinline__ void fold_column(const double a[3][3], double &A, double &B, double &C)
 {
@@ -51,35 +54,54 @@ __device__ __forceinline__ double combine_lanes(double A, double B, double C)
     return sqrt(ss);
 }
 
+// One row of one column: the axis-2 taps folded (3-D), or the value itself (2-D).  P: [1,2,1] along axis 2, D: [-1,0,1]
+// along axis 2, cen: the value at the row itself.
+template <int NDIM>
+__device__ __forceinline__ void load_row(const double *__restrict__ L, long long d0, long long d1, long long d2, long long cc,
+                                         long long y, long long c2, double &P, double &D, double &cen)
+{
+    if (NDIM == 2) {
+        cen = __ldg(L + y * d0 + cc);
+        P = cen; D = 0.0;
+    } else {
+        const long long zm = max(c2 - 1, 0ll), zp = min(c2 + 1, d2 - 1);
+        const double lm = __ldg(L + (zm * d1 + y) * d0 + cc), lp = __ldg(L + (zp * d1 + y) * d0 + cc);
+        cen = __ldg(L + (c2 * d1 + y) * d0 + cc);
+        P = (lm + lp) + 2.0 * cen;
+        D = lp - lm;
+    }
+}
+
+// Dense map.  A warp owns a strip of FL_VALID columns (axis 0; lanes 0 and 31 carry the halo columns) of one axis-2 plane
+// and marches over FL_ROWS rows of axis 1 with the folded rows y-1, y, y+1 in registers: every value is loaded once per
+// strip and plane it contributes to (3 loads per output in 3-D, 1 in 2-D, + the halo) instead of 9 / 3.
 template <int NDIM>
 __global__ void __launch_bounds__(FL_THREADS) fledge_dense_kernel(long long d0, long long d1, long long d2,
                                                                   const double *__restrict__ L, double *__restrict__ S)
 {
     const unsigned lane = threadIdx.x & 31u;
     const long long strips = (d0 + FL_VALID - 1) / FL_VALID;
-    const long long tasks = strips * d1 * d2;
+    const long long bands = (d1 + FL_ROWS - 1) / FL_ROWS;
+    const long long tasks = strips * bands * d2;
     const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
     for (long long t = (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); t < tasks; t += warps) {
-        const long long strip = t % strips, row = t / strips;
-        const long long c1 = row % d1, c2 = row / d1;
+        const long long strip = t % strips, rest = t / strips;
+        const long long band = rest % bands, c2 = rest / bands;
         const long long col = strip * FL_VALID - 1 + lane;               // lane 0 / 31 = halo
         const long long cc = min(max(col, 0ll), d0 - 1);                 // edge replication
-        double a[3][3];
-#pragma unroll
-        for (int o2 = 0; o2 < (NDIM == 3 ? 3 : 1); ++o2) {
-            const long long z = NDIM == 3 ? min(max(c2 + o2 - 1, 0ll), d2 - 1) : 0;
-#pragma unroll
-            for (int o1 = 0; o1 < 3; ++o1) {
-                const long long y = min(max(c1 + o1 - 1, 0ll), d1 - 1);
-                a[o2][o1] = __ldg(L + (z * d1 + y) * d0 + cc);
-            }
+        const long long y0 = band * FL_ROWS, y1 = min(y0 + FL_ROWS, d1);
+        double P0, D0, c0, P1, D1, c1, P2, D2, cn;
+        load_row<NDIM>(L, d0, d1, d2, cc, max(y0 - 1, 0ll), c2, P0, D0, c0);
+        load_row<NDIM>(L, d0, d1, d2, cc, y0, c2, P1, D1, c1);
+        for (long long y = y0; y < y1; ++y) {
+            load_row<NDIM>(L, d0, d1, d2, cc, min(y + 1, d1 - 1), c2, P2, D2, cn);
+            const double A = (P0 + P2) + 2.0 * P1, B = P2 - P0, C = (D0 + D2) + 2.0 * D1;
+            double s = combine_lanes<NDIM>(A, B, C);
+            // the centre tap has weight 0 in every G_d; O6 still lets a non-finite L anywhere in the stencil poison S
+            if (!isfinite(c1)) s = __longlong_as_double(0x7ff8000000000000ll);
+            if (lane >= 1 && lane <= FL_VALID && col < d0) S[(c2 * d1 + y) * d0 + col] = s;
+            P0 = P1; D0 = D1; P1 = P2; D1 = D2; c1 = cn;
         }
-        double A, B, C;
-        fold_column<NDIM>(a, A, B, C);
-        double s = combine_lanes<NDIM>(A, B, C);
-        // the centre tap has weight 0 in every G_d; O6 still lets a non-finite L anywhere in the stencil poison S
-        if (!isfinite(a[NDIM == 3 ? 1 : 0][1])) s = __longlong_as_double(0x7ff8000000000000ll);
-        if (lane >= 1 && lane <= FL_VALID && col < d0) S[(c2 * d1 + c1) * d0 + col] = s;
     }
 }
 
@@ -158,7 +180,7 @@ extern "C" int qsl_fledge_dense(int ndim, const long long dims[3], const double 
     if (d0 < 1 || d1 < 1 || d2 < 1) return QSL_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     const long long strips = (d0 + FL_VALID - 1) / FL_VALID;
-    const long long tasks = strips * d1 * d2;
+    const long long tasks = strips * ((d1 + FL_ROWS - 1) / FL_ROWS) * d2;
     const int wpb = FL_THREADS / 32;
     long long blocks = (tasks + wpb - 1) / wpb;
     const long long cap = (long long)sm_count() * 32;      // a multiple of the SM count; warps stride over the tasks

@@ -110,9 +110,9 @@ template <typename K>
 static int radix_sort_pairs_t(K *keys, uint32_t *vals, K *keys_tmp, uint32_t *vals_tmp, long long n, int key_bits,
                               cudaStream_t s)
 {
-    // sorts in place (an even number of passes ping-pongs back into keys / vals)
-    int passes = (key_bits + 7) / 8;
-    if (passes & 1) ++passes;
+    // sorts in place: an even number of passes ping-pongs back into keys / vals, an odd number ends with two copies
+    // (cheaper than a whole extra pass over zero digits)
+    const int passes = (key_bits + 7) / 8;
     const long long n_chunks = (n + SORT_CHUNK - 1) / SORT_CHUNK;
     const long long table = 256 * n_chunks;
     void *counts = nullptr, *offsets = nullptr, *tiles = nullptr, *total = nullptr;
@@ -136,6 +136,10 @@ static int radix_sort_pairs_t(K *keys, uint32_t *vals, K *keys_tmp, uint32_t *va
             e = cudaGetLastError();
             K *t = ki; ki = ko; ko = t;
             uint32_t *u = vi; vi = vo; vo = u;
+        }
+        if (e == cudaSuccess && ki != keys) {
+            e = cudaMemcpyAsync(keys, ki, sizeof(K) * (size_t)n, cudaMemcpyDeviceToDevice, s);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(vals, vi, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, s);
         }
         if (e != cudaSuccess) rc = record_cuda(e);
     }

@@ -90,12 +90,35 @@ static __global__ void __launch_bounds__(SCAN_THREADS) scan_tiles(long long n, c
     }
 }
 
+// Small inputs: one block does the whole scan (one launch instead of three).
+static __global__ void __launch_bounds__(1024) scan_small_u32(long long n, const uint32_t *__restrict__ in,
+                                                       unsigned long long *__restrict__ out,
+                                                       unsigned long long *__restrict__ total_out)
+{
+    unsigned long long carry = 0;
+    for (long long base = 0; base < n; base += blockDim.x) {
+        const long long i = base + threadIdx.x;
+        const unsigned long long x = i < n ? in[i] : 0ull;
+        unsigned long long total;
+        const unsigned long long ex = block_exclusive_scan(x, total);
+        if (i < n) out[i] = carry + ex;
+        carry += total;
+    }
+    if (threadIdx.x == 0 && total_out) *total_out = carry;
+}
+constexpr long long SCAN_SMALL = 32768;
+
 // out[i] = sum_{j<i} in[i]; *total (device, optional) = sum of all.  `tile_sums` scratch: ceil(n / SCAN_TILE) entries.
 static inline cudaError_t exclusive_scan_u32(long long n, const uint32_t *in, unsigned long long *out,
                                              unsigned long long *tile_sums, unsigned long long *total, cudaStream_t s)
 {
     const long long tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     if (tiles == 0) return cudaMemsetAsync(total, 0, sizeof(unsigned long long), s);
+    if (n <= SCAN_SMALL) {
+        count_launch();
+        scan_small_u32<<<1, 1024, 0, s>>>(n, in, out, total);
+        return cudaGetLastError();
+    }
     count_launch();
     scan_tile_sums<<<(unsigned)tiles, SCAN_THREADS, 0, s>>>(n, in, tile_sums);
     count_launch();

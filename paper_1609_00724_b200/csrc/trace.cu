@@ -63,7 +63,7 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
     if (!f || !p || !out || n < 0 || (n > 0 && !seeds)) return QSL_EINVAL;
     if (p->method != QSL_RK4 && p->method != QSL_EULER && p->method != QSL_CK45) return QSL_EINVAL;
     // the adaptive stepper runs in fp64 on the fp64 cell table only, with a positive tolerance
-    if (p->method == QSL_CK45 && (!f->view.cells || f->view.spherical || p->arith != QSL_ARITH_F64 || !(p->tol > 0.0)))
+    if (p->method == QSL_CK45 && (!f->view.cells || p->arith != QSL_ARITH_F64 || !(p->tol > 0.0)))
         return QSL_EINVAL;
     if (p->mode != QSL_TRACE_L && p->mode != QSL_TRACE_LQ) return QSL_EINVAL;
     if (p->arith != QSL_ARITH_F64 && p->arith != QSL_ARITH_F32) return QSL_EINVAL;

@@ -55,6 +55,7 @@ struct LineState2 {
     uint32_t nsteps, slot;
     int phase;
     bool back;
+    double sth, cth;      // SPH: (sin, cos) of the latitude y[1] of the line's current point (metric_shift)
 
     // Cell search (reading A8: index clamped, offsets not) and load of the cell's 24 coefficients (six 256-bit loads).
     __device__ __forceinline__ void relocate(const TraceArgs &A, const double x[3])
@@ -162,13 +163,23 @@ struct LineState2 {
         }
     }
 
+    // SPH: the line's point moves by dt in latitude: rotate (sth, cth) and pull it back onto the unit circle (one Newton
+    // step of 1/sqrt), so that rounding never accumulates in the modulus; the phase error grows like sqrt(steps) ulp.
+    __device__ __forceinline__ void move_anchor(double dt)
+    {
+        double s, c;
+        sincos_shift(sth, cth, dt, s, c);
+        const double f = fma(-0.5, fma(s, s, fma(c, c, -1.0)), 1.0);
+        sth = s * f; cth = c * f;
+    }
+
     // b -> coordinate rates (and |b| of the unscaled vector), k -> coordinate deviation rates, at the point pt
     __device__ __forceinline__ double to_rates(const double *pt, double b[3], double *k)
     {
         const double bn = norm3_fast(b);
         if (SPH) {
             double mf[3];
-            metric<SPH>(pt, mf);
+            metric_shift(pt[2], sth, cth, pt[1] - y[1], mf);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 b[c] *= mf[c];
@@ -190,6 +201,7 @@ struct LineState2 {
         const uint32_t si = A.perm[pos];
         const double x[3] = { A.seeds[3 * (size_t)si], A.seeds[3 * (size_t)si + 1], A.seeds[3 * (size_t)si + 2] };
         L = 0.0; lam = 0.0; nsteps = 0; phase = 0;
+        if (SPH) sincos(x[1], &sth, &cth); else { sth = 0.0; cth = 1.0; }
 #pragma unroll
         for (int c = 0; c < NV; ++c) y[c] = c < 3 ? x[c] : 0.0;
         if (!inside_box(A, x)) { finish(A, 255, REC_SEED_OUTSIDE); return false; }
@@ -201,7 +213,7 @@ struct LineState2 {
             y[3 % NV] = b0.x; y[4 % NV] = b0.y; y[5 % NV] = b1.x; y[6 % NV] = b1.y; y[7 % NV] = b2.x; y[8 % NV] = b2.y;
             if (SPH) {   // orthonormal pair -> coordinate deviations (eq. 8 inverted)
                 double mf[3];
-                metric<SPH>(x, mf);
+                metric_shift(x[2], sth, cth, 0.0, mf);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) { y[(3 + c) % NV] *= mf[c]; y[(6 + c) % NV] *= mf[c]; }
             }
@@ -253,7 +265,7 @@ struct LineState2 {
                 if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, 255, REC_CAP); return true; }
                 h = STRETCHED ? A.step_frac * fmin(hc[0], fmin(hc[1], hc[2])) : A.h_uniform;
                 if (SPH)   // physical cell edges (r cos(theta) h_phi, r h_theta, h_r) at the start of the step
-                    h = A.step_frac * fmin(y[2] * cos(y[1]) * A.fv.h[0], fmin(y[2] * A.fv.h[1], A.fv.h[2]));
+                    h = A.step_frac * fmin(y[2] * cth * A.fv.h[0], fmin(y[2] * A.fv.h[1], A.fv.h[2]));
                 if (lam + h > A.max_length) h = A.max_length - lam;
                 hs = h;
             } else {
@@ -351,6 +363,7 @@ struct LineState2 {
         // ys = trial end, accL = trial length
         if (phase == 0) {
             if (inside_box(A, ys)) {
+                if (SPH) move_anchor(ys[1] - y[1]);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) y[c] = ys[c];
                 L = accL; lam += h; ++nsteps;

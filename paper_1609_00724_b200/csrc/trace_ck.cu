@@ -3,7 +3,7 @@
 
 namespace qsl {
 
-template <bool DEV, bool STRETCHED, bool INTERP>
+template <bool DEV, bool STRETCHED, bool INTERP, bool SPH = false>
 static int launch_trace_ck_variant(TraceArgs &A, double tol, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s)
 {
     const long long n_items = 2 * A.n;
@@ -11,7 +11,7 @@ static int launch_trace_ck_variant(TraceArgs &A, double tol, bool refill, cudaEv
     long long blocks = (n_items + threads - 1) / threads;
     if (refill) {
         int per_sm = 0;
-        QSL_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_ck_kernel<DEV, STRETCHED, INTERP, true>, threads, 0));
+        QSL_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace_ck_kernel<DEV, STRETCHED, INTERP, true, SPH>, threads, 0));
         if (per_sm < 1) per_sm = 1;
         const long long resident = (long long)sm_count() * per_sm;   // persistent: grid = SMs x resident CTAs
         if (blocks > resident) blocks = resident;
@@ -30,8 +30,8 @@ static int launch_trace_ck_variant(TraceArgs &A, double tol, bool refill, cudaEv
         if (e == cudaSuccess && ev0) e = cudaEventRecord(ev0, s);
         if (e == cudaSuccess) {
             count_launch();
-            if (refill) trace_ck_kernel<DEV, STRETCHED, INTERP, true><<<(unsigned)blocks, threads, 0, s>>>(A, tol);
-            else trace_ck_kernel<DEV, STRETCHED, INTERP, false><<<(unsigned)blocks, threads, 0, s>>>(A, tol);
+            if (refill) trace_ck_kernel<DEV, STRETCHED, INTERP, true, SPH><<<(unsigned)blocks, threads, 0, s>>>(A, tol);
+            else trace_ck_kernel<DEV, STRETCHED, INTERP, false, SPH><<<(unsigned)blocks, threads, 0, s>>>(A, tol);
             e = cudaGetLastError();
         }
         if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, s);
@@ -44,6 +44,9 @@ static int launch_trace_ck_variant(TraceArgs &A, double tol, bool refill, cudaEv
 int launch_trace_ck(TraceArgs &A, double tol, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s)
 {
     const bool st = A.fv.stretched != 0, in = A.fv.interp_mode == QSL_INTERP_FIRST;
+    if (A.fv.spherical)   // uniform axes, paper mode (qsl_field_create guarantees it)
+        return dev ? launch_trace_ck_variant<true, false, false, true>(A, tol, refill, ev0, ev1, s)
+                   : launch_trace_ck_variant<false, false, false, true>(A, tol, refill, ev0, ev1, s);
 #define QSL_DISPATCH(D, ST, IN) \
     if (dev == D && st == ST && in == IN) return launch_trace_ck_variant<D, ST, IN>(A, tol, refill, ev0, ev1, s);
     QSL_DISPATCH(false, false, false) QSL_DISPATCH(false, false, true) QSL_DISPATCH(false, true, false) QSL_DISPATCH(false, true, true)

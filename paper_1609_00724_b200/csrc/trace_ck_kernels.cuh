@@ -14,9 +14,11 @@
 
 namespace qsl {
 
-template <bool DEV, bool STRETCHED, bool INTERP>
-struct LineStateCK : LineState2<DEV, STRETCHED, INTERP> {
-    using Base = LineState2<DEV, STRETCHED, INTERP>;
+// SPH: spherical geometry (reading A19) exactly as in the fixed-step kernel: coordinate rates = orthonormal components x
+// metric factors; the step unit and the error unit hmin are the physical cell edges at the start of the step.
+template <bool DEV, bool STRETCHED, bool INTERP, bool SPH = false>
+struct LineStateCK : LineState2<DEV, STRETCHED, INTERP, SPH> {
+    using Base = LineState2<DEV, STRETCHED, INTERP, SPH>;
     static constexpr int NV = Base::NV;
     int j;                     // controller state: h = h0 2^j
     double hp, hfull, bound, xt[3];
@@ -28,9 +30,9 @@ struct LineStateCK : LineState2<DEV, STRETCHED, INTERP> {
         double d[3], b[3];
         this->enter_cell(A, ys, d);
         this->stage(d, ys, b, k);
+        bn = SPH ? this->to_rates(ys, b, k) : norm3_fast(b);
 #pragma unroll
         for (int c = 0; c < 3; ++c) k[c] = b[c];
-        bn = norm3_fast(b);
     }
 
     __device__ bool advance_ck(const TraceArgs &A, double tol)
@@ -67,6 +69,7 @@ struct LineStateCK : LineState2<DEV, STRETCHED, INTERP> {
             if (!(n1 >= A.null_eps)) { this->finish(A, 255, this->nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL); return true; }
             if ((long long)this->nsteps >= A.max_steps || this->lam >= A.max_length) { this->finish(A, 255, REC_CAP); return true; }
             hmin = STRETCHED ? fmin(this->hc[0], fmin(this->hc[1], this->hc[2])) : fmin(A.fv.h[0], fmin(A.fv.h[1], A.fv.h[2]));
+            if (SPH) hmin = fmin(this->y[2] * this->cth * A.fv.h[0], fmin(this->y[2] * A.fv.h[1], A.fv.h[2]));
             h = (A.step_frac * hmin) * __hiloint2double((1023 + j) << 20, 0);      // exact scaling by 2^j
             if (this->lam + h > A.max_length) h = A.max_length - this->lam;
             hs = h;
@@ -99,6 +102,7 @@ struct LineStateCK : LineState2<DEV, STRETCHED, INTERP> {
             const double en = emax / (tol * hmin);
             if (en > 1.0 && j > -20) { --j; return false; }                 // reject: halve, retry from y
             if (inside_box(A, ys)) {
+                if (SPH) this->move_anchor(ys[1] - this->y[1]);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) this->y[c] = ys[c];
                 this->L = Ln; this->lam += h; ++this->nsteps;
@@ -137,10 +141,10 @@ struct LineStateCK : LineState2<DEV, STRETCHED, INTERP> {
     }
 };
 
-template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL>
+template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL, bool SPH = false>
 __global__ void __launch_bounds__(128, 2) trace_ck_kernel(const TraceArgs A, const double tol)
 {
-    LineStateCK<DEV, STRETCHED, INTERP> ls;
+    LineStateCK<DEV, STRETCHED, INTERP, SPH> ls;
     const long long n_items = 2 * A.n;
     unsigned long long my_steps = 0;
     if (!REFILL) {

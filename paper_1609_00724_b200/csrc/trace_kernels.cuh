@@ -332,6 +332,47 @@ __device__ __forceinline__ void metric(const double *u, double mf[3])
     else { mf[0] = 1.0; mf[1] = 1.0; mf[2] = 1.0; }
 }
 
+// The same metric factors without a call to cos() per evaluation point.  The cell-table kernel carries (sin, cos) of the
+// latitude of the line's current point; a stage point's latitude differs from it by dt = O(step / r), so
+// cos(theta + dt) = cos(theta) cos(dt) - sin(theta) sin(dt) with cos(dt), sin(dt) from their Taylor polynomials through
+// dt^8 / dt^9 (truncation below 2^-64 for |dt| <= 1/16; anything larger falls back to sincos()).  1 / (r cos theta) is one
+// hardware reciprocal seed + two Newton steps (within an ulp), and 1 / r = cos(theta) / (r cos(theta)).  The oracle calls
+// cos() and divides (reading A19): the difference is a few ulp of the metric factors, far below the parity gates.
+__device__ __forceinline__ void sincos_small(double dt, double &s, double &c)
+{
+    const double t2 = dt * dt;
+    c = fma(t2, fma(t2, fma(t2, fma(t2, 1.0 / 40320.0, -1.0 / 720.0), 1.0 / 24.0), -0.5), 1.0);
+    s = dt * fma(t2, fma(t2, fma(t2, fma(t2, 1.0 / 362880.0, -1.0 / 5040.0), 1.0 / 120.0), -1.0 / 6.0), 1.0);
+}
+__device__ __forceinline__ double rcp_fast(double d)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    r = fma(r, fma(-d, r, 1.0), r);
+    return fma(r, fma(-d, r, 1.0), r);
+}
+// (sin, cos) of theta0 + dt from (st0, ct0) = (sin, cos)(theta0)
+__device__ __forceinline__ void sincos_shift(double st0, double ct0, double dt, double &s, double &c)
+{
+    if (fabs(dt) <= 0.0625) {
+        double sd, cd;
+        sincos_small(dt, sd, cd);
+        s = fma(st0, cd, ct0 * sd);
+        c = fma(ct0, cd, -(st0 * sd));
+    } else {
+        // far from the anchor (never on the path of a fixed-step line): exact functions of the sum of the two angles
+        const double th = atan2(st0, ct0) + dt;
+        sincos(th, &s, &c);
+    }
+}
+__device__ __forceinline__ void metric_shift(double r, double st0, double ct0, double dt, double mf[3])
+{
+    double s, c;
+    sincos_shift(st0, ct0, dt, s, c);
+    const double q = rcp_fast(r * c);
+    mf[0] = q; mf[1] = q * c; mf[2] = 1.0;
+}
+
 template <typename S, bool DEV, bool STRETCHED, bool INTERP, int ORDER = 1, bool SPH = false>
 struct LineState {
     static constexpr int NV = DEV ? 9 : 3;

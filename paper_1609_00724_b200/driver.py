@@ -70,7 +70,8 @@ def hilbert_map(lattice, R: int, thr: float, passes: int, shift: int, trace_fn, 
     libqsl call.  Level-0 samples ordered along the Hilbert curve; per pass a refinement on the curve (a new sample halfway
     along the curve wherever the field-line length of two successive samples differs by more than `thr`) and, if
     `shift` != 0, the same on the curve shifted by `shift` fine cells, after which the samples go back to the original
-    order.  trace_fn(seeds CUDA float64 (m, 3)) -> (L, Q), CUDA float64 (m,) each - e.g. a closure over qsl_trace.
+    order.  trace_fn(seeds CUDA float64 (m, 3)) -> (L, Q), CUDA float64 (m,) each - e.g. a closure over qsl_trace; every
+    batch it receives is ordered along the (shifted) curve, so the closure may pass QSL_FLAG_NO_SORT.
 
     Returns dict(keys int64 (n,), coords int32 (n, ndim), L, Q, counts): the samples in curve order and the number of
     samples after level 0 and after every (sub-)pass.  Feed keys and Q to qsl_hilbert_convert for the rectilinear map.

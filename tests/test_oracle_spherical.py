@@ -83,3 +83,29 @@ def test_S3_cartesian_limit_reproduces_the_cartesian_oracle():
         assert np.allclose(os_["L"], oc["L"], rtol=2e-4)
         assert np.allclose(os_["q_perp"], oc["q_perp"], rtol=2e-3) and np.allclose(os_["q_bnd"], oc["q_bnd"], rtol=2e-3)
         assert np.abs(os_["nsteps_f"].astype(int) - oc["nsteps_f"]).max() <= 2
+
+
+def test_S4_cash_karp_in_spherical_geometry():
+    """The adaptive stepper in spherical geometry (the paper's own combination): the monopole keeps
+    Q = 2 and L = r_max - r_min with fewer steps than the fixed-step rule, and a dipole line keeps the closed-form invariant
+    r / cos^2(theta) from foot point to foot point at every tolerance (a missing or wrong metric factor in any of the six
+    stages bends the line at O(1))."""
+    g = qi.Grid.uniform((9, 11, 33), (0.1, -0.3, 1.0), (0.9, 0.5, 3.0))
+    F = oracle.Field(g, _cubes(g, lambda p, t, r: (0 * r, 0 * r, 1 / r ** 2)), oracle.F64, oracle.NORMALIZE_FIRST,
+                     oracle.TRILINEAR, oracle.SPHERICAL)
+    seeds = np.array([[0.33, 0.11, g.zs[7]], [0.71, -0.22, g.zs[20]]])
+    o = oracle.trace(F, seeds, g.lo, g.hi, method=oracle.CK45, tol=1e-2)
+    assert np.allclose(o["L"], 2.0, atol=1e-11) and np.abs(o["q_perp"] - 2).max() < 1e-9
+    assert int(o["nsteps_f"].sum() + o["nsteps_b"].sum()) < int(sum(oracle.trace(F, seeds, g.lo, g.hi)[k].sum() for k in ("nsteps_f", "nsteps_b")))
+    g = qi.Grid.uniform((5, 161, 161), (0.0, -1.0, 1.0), (0.4, 1.0, 3.0))
+    F = oracle.Field(g, _cubes(g, _dipole), oracle.F64, oracle.NORMALIZE_FIRST, oracle.TRILINEAR, oracle.SPHERICAL)
+    seeds = np.array([[0.2, 0.5, 1.0], [0.2, 0.62, 1.0]])
+    errs = []
+    for tol in (1e-2, 1e-4, 1e-6):
+        o = oracle.trace(F, seeds, g.lo, g.hi, method=oracle.CK45, tol=tol, max_steps=100000)
+        inv0 = seeds[:, 2] / np.cos(seeds[:, 1]) ** 2
+        end = np.where((o["nsteps_f"] > 1)[:, None], o["end_f"], o["end_b"])
+        assert np.all(np.where(o["nsteps_f"] > 1, o["face_f"], o["face_b"]) == 4)        # closed lines: back on r = 1
+        assert np.all(np.sign(end[:, 1]) == -np.sign(seeds[:, 1]))                        # in the other hemisphere
+        errs.append(np.abs(end[:, 2] / np.cos(end[:, 1]) ** 2 - inv0).max())
+    assert max(errs) < 1e-6, errs                                   # floor set by the trilinear interpolant on 161 nodes
