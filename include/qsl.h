@@ -200,7 +200,9 @@ int qsl_debug_sort_pairs(unsigned int *keys, unsigned int *vals, long long n, in
 int qsl_hilbert_bits(const qsl_lattice *lat, int R);
 /* Level-0 samples in dense order (c2 n1 + c1) n0 + c0: fine cell c0 2^R + 2^(R-1) and its centre (seeds: n*3 fp64).      */
 int qsl_hilbert_level0(const qsl_lattice *lat, int R, unsigned int *coords, double *seeds, void *stream);
-/* keys[i] = position along the curve of `bits` bits per axis of the cell coords[i] + shift; and the inverse.             */
+/* keys[i] = position along the curve of `bits` bits per axis of the cell coords[i] + shift; and the inverse.  coords[i] +
+ * shift must stay below 2^bits (the caller's duty; shift >= 2^bits is rejected with QSL_EINVAL, and qsl_hilbert_refine
+ * rejects a shift larger than the cube of the un-shifted curve, which is what its one extra bit per axis can hold).      */
 int qsl_hilbert_keys(int ndim, int bits, int shift, long long n, const unsigned int *coords, unsigned long long *keys,
                      void *stream);
 int qsl_hilbert_cells(int ndim, int bits, int shift, long long n, const unsigned long long *keys, unsigned int *coords,
@@ -228,7 +230,9 @@ int qsl_hilbert_merge(long long n_old, long long n_new, const long long *left, i
 int qsl_hilbert_convert(const qsl_lattice *lat, int R, int r, long long n, const unsigned long long *keys, const double *Q,
                         double *out, void *stream);
 
-/* ---- measurement hooks (bench.py) ------------------------------------------------------------------ */
+/* ---- measurement hooks (bench.py) ------------------------------------------------------------------ *
+ * Threading: the library keeps per-process state without locks (last CUDA error, launch counter, the profiling event
+ * pool below, one private stream-ordered scratch pool per device): drive it from one host thread at a time.             */
 /* qsl_profile_enable(1): every later qsl_trace records a CUDA event pair around its trace kernel (the dominant
  * kernel) on the caller's stream (up to 256 launches between two reads).  qsl_profile_trace_kernel_ms waits for the pairs
  * recorded since the previous read (or enable), returns their summed device time in milliseconds and their number per

@@ -25,14 +25,26 @@ TRACE_L, TRACE_LQ = 0, 1
 ST_SEED_OUTSIDE, ST_NULL_AT_SEED, ST_STALL_F, ST_STALL_B, ST_CAP_F, ST_CAP_B, ST_OPEN = 1, 2, 4, 8, 16, 32, 64
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (-O2 -ffp-contract=off: arithmetic exactly as written)."""
-    if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC):
-        return _SO
-    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c11", "-Wall", "-shared", "-fPIC",
-           _SRC[0], "-o", _SO, "-lm"]
-    subprocess.run(cmd, check=True)
-    return _SO
+_SO_SAN = os.path.join(_HERE, "libqsl_oracle_san.so")
+
+
+def build(force: bool = False, sanitize: bool = False) -> str:
+    """Compile the oracle with gcc (-O2 -ffp-contract=off: arithmetic exactly as written).
+    sanitize=True builds a second library with -fsanitize=address,undefined: it is loaded when the
+    environment variable QSL_ORACLE_SANITIZE=1 is set, in a process started with LD_PRELOAD=<sanitizer_runtime()>."""
+    so = _SO_SAN if sanitize else _SO
+    if not force and os.path.exists(so) and all(os.path.getmtime(so) >= os.path.getmtime(s) for s in _SRC):
+        return so
+    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c11", "-Wall", "-shared", "-fPIC"]
+    if sanitize:
+        cmd += ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+    subprocess.run(cmd + [_SRC[0], "-o", so, "-lm"], check=True)
+    return so
+
+
+def sanitizer_runtime() -> str:
+    """Path of gcc's libasan.so, to be LD_PRELOADed by a process that loads the sanitized oracle."""
+    return subprocess.run(["gcc", "-print-file-name=libasan.so"], check=True, capture_output=True, text=True).stdout.strip()
 
 
 _dp = C.POINTER(C.c_double)
@@ -63,8 +75,8 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        build()
-        _lib = C.CDLL(_SO)
+        san = os.environ.get("QSL_ORACLE_SANITIZE") == "1"
+        _lib = C.CDLL(build(sanitize=san))
         _lib.orc_select.restype = C.c_double
         _lib.orc_refine.restype = C.c_longlong
     return _lib

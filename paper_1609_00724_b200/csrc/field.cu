@@ -17,20 +17,43 @@ int record_cuda(cudaError_t e)
     return e == cudaErrorMemoryAllocation ? QSL_ENOMEM : QSL_ECUDA;
 }
 
+// Scratch comes from a PRIVATE stream-ordered memory pool per device (release threshold = never: repeated calls do not go
+// back to the OS), so that the library does not change the behaviour of the device's default pool under other users of
+// cudaMallocAsync in the process.  The per-device table is filled on first use; the hooks that read it (and
+// g_last_cuda_error, the launch counter and the profiling event pool of trace.cu) are not thread-safe: one host thread
+// drives the library at a time.
+constexpr int MAX_DEVICES = 64;
+static cudaMemPool_t g_pool[MAX_DEVICES];
+static bool g_pool_made[MAX_DEVICES];
+static int g_sm_count[MAX_DEVICES];
+
+static int current_device()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return -1;
+    return dev;
+}
+
 int scratch_alloc(void **p, size_t bytes, cudaStream_t s)
 {
-    static bool pool_set = false;
-    if (!pool_set) {
-        int dev = 0;
-        cudaMemPool_t pool;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            uint64_t keep = UINT64_MAX;  // keep freed scratch in the pool: repeated calls never go back to the OS
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
-        pool_set = true;
-    }
     if (bytes == 0) bytes = 16;
-    QSL_CUDA(cudaMallocAsync(p, bytes, s));
+    const int dev = current_device();
+    if (dev >= 0 && !g_pool_made[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        if (cudaMemPoolCreate(&g_pool[dev], &props) == cudaSuccess) {
+            uint64_t keep = UINT64_MAX;
+            cudaMemPoolSetAttribute(g_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+            g_pool_made[dev] = true;
+        } else {
+            cudaGetLastError();
+        }
+    }
+    if (dev >= 0 && g_pool_made[dev]) QSL_CUDA(cudaMallocFromPoolAsync(p, bytes, g_pool[dev], s));
+    else QSL_CUDA(cudaMallocAsync(p, bytes, s));      // no private pool: the device's default pool, untouched
     return QSL_OK;
 }
 void scratch_free(void *p, cudaStream_t s)
@@ -40,13 +63,12 @@ void scratch_free(void *p, cudaStream_t s)
 
 int sm_count()
 {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            n = 148;
-    }
-    return n;
+    const int dev = current_device();
+    if (dev < 0) return 148;
+    if (g_sm_count[dev] == 0 &&
+        cudaDeviceGetAttribute(&g_sm_count[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        g_sm_count[dev] = 148;
+    return g_sm_count[dev];
 }
 
 // One thread per node.  All arithmetic is explicit-rounding fp64 (no FMA contraction) so that the packed samples are

@@ -358,6 +358,7 @@ int qsl_hilbert_level0(const qsl_lattice *lat, int R, unsigned int *coords, doub
 int qsl_hilbert_keys(int ndim, int bits, int shift, long long n, const unsigned int *coords, unsigned long long *keys, void *stream)
 {
     if ((ndim != 2 && ndim != 3) || bits < 1 || bits * ndim > 63 || bits > 31 || shift < 0 || n < 0) return QSL_EINVAL;
+    if ((long long)shift >= (1ll << bits)) return QSL_EINVAL;      // coords + shift would leave the curve's cube
     if (n == 0) return QSL_OK;
     if (!coords || !keys) return QSL_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
@@ -371,6 +372,7 @@ int qsl_hilbert_keys(int ndim, int bits, int shift, long long n, const unsigned 
 int qsl_hilbert_cells(int ndim, int bits, int shift, long long n, const unsigned long long *keys, unsigned int *coords, void *stream)
 {
     if ((ndim != 2 && ndim != 3) || bits < 1 || bits * ndim > 63 || bits > 31 || shift < 0 || n < 0) return QSL_EINVAL;
+    if ((long long)shift >= (1ll << bits)) return QSL_EINVAL;      // coords + shift would leave the curve's cube
     if (n == 0) return QSL_OK;
     if (!coords || !keys) return QSL_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
@@ -420,6 +422,8 @@ int qsl_hilbert_refine(const qsl_lattice *lat, int R, int shift, long long n, co
     *n_new = 0;
     if (n < 2) return QSL_OK;
     if (!keys || !L || (capacity > 0 && (!left || !new_coords || !new_seeds))) return QSL_EINVAL;
+    // the shifted curve has one bit more per axis than the lattice's cube: shifts up to the size of that cube fit
+    if ((long long)shift > (1ll << curve_bits(A))) return QSL_EINVAL;
     const int bits = curve_bits(A) + (shift ? 1 : 0);
     if (bits * A.ndim > 63) return QSL_ERANGE;
     cudaStream_t s = (cudaStream_t)stream;

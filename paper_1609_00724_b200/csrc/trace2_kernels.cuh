@@ -85,7 +85,8 @@ struct LineState2 {
     // sufficient one on the high words of the bit patterns, 0 <= d < h: one unsigned integer compare per axis on the
     // integer pipe instead of two DSETP on the FP64 pipe.  It is false for negative d (sign bit), -0.0, NaN and for d
     // within 2^-20 (relative) below h: a false negative only costs a redundant search, which finds the right cell.
-    // (A branch-free variant with predicated neighbour loads was measured and dropped: profiles/r1c.)
+    // (A branch-free variant with predicated neighbour loads was slower in round 1; its numbers were not kept.  What was
+    // measured on this path since - look-ahead staging in shared memory, register caps - is in profiles/r2b.)
     __device__ __forceinline__ void enter_cell(const TraceArgs &A, const double x[3], double d[3])
     {
         d[0] = x[0] - x0[0]; d[1] = x[1] - x0[1]; d[2] = x[2] - x0[2];

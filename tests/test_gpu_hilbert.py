@@ -34,6 +34,22 @@ def test_keys_and_cells_bit_exact(nd, bits, shift):
     assert np.array_equal(back, c.astype(np.int32))
 
 
+def test_shift_out_of_range_is_rejected():
+    """a shift that would push cells out of the curve's cube must be an error, not wrong keys."""
+    c = torch.zeros((4, 2), dtype=torch.int32, device="cuda")
+    with pytest.raises(qsl.QslError):
+        qsl.qsl_hilbert_keys(c, 3, 8)
+    k = qsl.qsl_hilbert_keys(c, 3, 7)
+    with pytest.raises(qsl.QslError):
+        qsl.qsl_hilbert_cells(k, 2, 3, 8)
+    lat = _lat(2, (8, 4))
+    bits = qsl.qsl_hilbert_bits(lat, 1)                                        # 4 bits: cube of 16 cells per axis
+    keys = torch.arange(4, dtype=torch.int64, device="cuda")
+    L = torch.ones(4, dtype=torch.float64, device="cuda")
+    with pytest.raises(qsl.QslError):
+        qsl.qsl_hilbert_refine(lat, 1, (1 << bits) + 1, keys, L, 0.1)
+
+
 @pytest.mark.parametrize("n", [0, 1, 5, 4097, 100003])
 def test_sort_keys64_and_gather(n):
     rng = np.random.default_rng(n)
