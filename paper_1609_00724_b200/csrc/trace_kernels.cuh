@@ -336,8 +336,8 @@ __device__ __forceinline__ void metric(const double *u, double mf[3])
 // latitude of the line's current point; a stage point's latitude differs from it by dt = O(step / r), so
 // cos(theta + dt) = cos(theta) cos(dt) - sin(theta) sin(dt) with cos(dt), sin(dt) from their Taylor polynomials through
 // dt^8 / dt^9 (truncation below 2^-64 for |dt| <= 1/16; anything larger falls back to sincos()).  1 / (r cos theta) is one
-// hardware reciprocal seed + two Newton steps (within an ulp), and 1 / r = cos(theta) / (r cos(theta)).  The oracle calls
-// cos() and divides (reading A19): the difference is a few ulp of the metric factors, far below the parity gates.
+// hardware reciprocal seed + two Newton steps (within an ulp), and 1 / r = cos(theta) / (r cos(theta)).  The plain
+// definition (reading A19: cos() and two divisions) differs by a few ulp of the metric factors, far below the parity gates.
 __device__ __forceinline__ void sincos_small(double dt, double &s, double &c)
 {
     const double t2 = dt * dt;
