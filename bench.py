@@ -47,6 +47,7 @@ FLOPS_PER_STEP = {"LQ": 800, "L": 400}
 # fp32 arithmetic) as a fraction of peak.  Keyed by (workload, arithmetic); absent -> null in the bench line.
 NCU_CAPTURES = {
     ("cfg2", "f64"): {"dram_bytes": 789848320, "pipe_active": 0.484, "source": "profiles/r1b_cell_table_kernel.md (capture e)"},
+    ("cfg4", "f64"): {"dram_bytes": 41683301000, "pipe_active": 0.517, "source": "profiles/r2a_cfg4_trace_kernel.md"},
 }
 DEFAULT_WORKLOAD = "cfg4"
 SELECT_PASSES = 8          # radix passes of qsl_select (select_refine.cu), for the streaming byte count
@@ -235,6 +236,7 @@ def workload_config(cfg, args, **extra):
          "seed_lattice": [int(v) for v in lat.n], "n_seeds": int(len(cfg["seeds"])),
          "trace_mode": "L+Q" if cfg["mode"] == 1 else "L", "refine_levels": int(cfg["levels"]),
          "step_rule": "RK4, h = 0.25 x smallest cell edge", "parallelism": "replicas x%d" % args.gpus,
+         "interpolation": {1: "trilinear", 2: "triquadratic (Dodgson)", 3: "tricubic (Keys)"}[int(getattr(args, "interp_order", 1))],
          "l2": "flushed between timed steps (256 MiB write)"}
     if int(cfg["levels"]) > 0:
         c["refine"] = ("hilbert: length jump > %g between successive samples along the Hilbert curve, %d passes + shifted "
@@ -268,8 +270,10 @@ class Workload:
         self.f32 = args.arith == "f32" and cfg["sample_type"] == "f32"
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record()
+        self.order = int(getattr(args, "interp_order", 1))
         self.field = qsl.qsl_field_create(g.nx, g.ny, g.nz, *dev, lo=g.lo, hi=g.hi, sample_type=st,
-                                          layout=qsl.QSL_LAYOUT_CELL_TABLE_F32 if self.f32 else qsl.QSL_LAYOUT_CELL_TABLE)
+                                          layout=qsl.QSL_LAYOUT_CELL_TABLE_F32 if self.f32 else qsl.QSL_LAYOUT_CELL_TABLE,
+                                          interp_order=0 if self.order == 1 else self.order)
         ev1.record(); ev1.synchronize()
         self.field_create_ms = ev0.elapsed_time(ev1)
         del dev
@@ -438,6 +442,22 @@ def alu_roofline(W, T, peak_fma):
         "true_flops_achieved_tflops": flops / (k_ms * 1e-3) / 1e12}
 
 
+def gather_roofline(W, T, qsl):
+    """--interp-order 2 / 3 (and any run of the corner-gather kernel): the trace kernel against the L1 gather rate.
+    Algorithmic bytes: 4 stage evaluations x (order + 1)^3 stencil samples of 16 B (fp32) / 32 B (fp64) per RK4 step;
+    peak = divergent gathers of that sample size over an L1-resident (64 KiB) footprint, measured by qsl_peak_gather."""
+    sb = 16 if W.cfg["sample_type"] == "f32" else 32
+    ns = (W.order + 1) ** 3
+    k_ms = T["kern_ms"][0] + T["kern_ms"][1]
+    achieved = sum(T["rk_by_mode"]) * 4.0 * ns * sb / (k_ms * 1e-3) / 1e9
+    peak = qsl.qsl_peak_gather(sb, 64 << 10) * sb / 1e9
+    return {"bound": "l1_gather", "kernel": "trace_kernel<ORDER = %d> (corner / stencil gather kernel; all %d launches of the timed region)"
+                                            % (W.order, sum(T["kern_n"])),
+            "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+            "kernel_ms": k_ms / T["steps"], "kernel_share_of_step": k_ms / T["dev_ms"],
+            "convention": "4 evaluations x %d samples x %d B gathered per RK4 step / qsl_peak_gather(%d B, 64 KiB footprint)" % (ns, sb, sb)}
+
+
 def streaming_block(qsl, torch, W):
     """the HBM-streaming stages as GB/s against MEASURED_PEAKS.json hbm_gbs.  Each C-ABI call is timed with
     CUDA events (best of 5 after 2 warm-ups, L2 not flushed: every input is larger than L2) on synthetic maps of the size of
@@ -505,14 +525,26 @@ def streaming_block(qsl, torch, W):
     put("radix_sort_pairs", best(sort) - t_copy, n * 8 * 2 * SORT_PASSES + n * 4 * SORT_PASSES,
         "6.7e7 (key, index) pairs, 30-bit keys: %d passes x (histogram read 4 B + scatter read 8 B + write 8 B)" % SORT_PASSES)
     del keys, vals, k2, v2
-    # field pack + per-cell table: the whole qsl_field_create of this run's workload
+    # field pack + per-cell table: the whole qsl_field_create call of this run's workload (allocation included), warm
     g = W.cfg["grid"]
     nodes = g.nx * g.ny * g.nz
     cells = (g.nx - 1) * (g.ny - 1) * (g.nz - 1)
     sb = 16 if W.cfg["sample_type"] == "f32" else 32
-    put("field_create", W.field_create_ms, nodes * (24 + sb) + cells * (96 if W.f32 else 192),
-        "pack_kernel + cell_table_kernel of %s (cold, one call): 24 B in + %d B out per node, %d B out per cell"
-        % (W.name, sb, 96 if W.f32 else 192))
+    dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda() for a in W.cfg["B"]]
+    st = qsl.QSL_F32 if W.cfg["sample_type"] == "f32" else qsl.QSL_F64
+    ts = []
+    for _ in range(3):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        f = qsl.qsl_field_create(g.nx, g.ny, g.nz, *dev, lo=g.lo, hi=g.hi, sample_type=st,
+                                 layout=qsl.QSL_LAYOUT_CELL_TABLE_F32 if W.f32 else qsl.QSL_LAYOUT_CELL_TABLE)
+        b.record(); b.synchronize()
+        ts.append(a.elapsed_time(b))
+        f.destroy()
+    del dev
+    put("field_create", min(ts), nodes * (24 + sb) + cells * (96 if W.f32 else 192),
+        "whole qsl_field_create call of %s (pack_kernel + cell_table_kernel + cudaMalloc of the arrays + axis upload with its host "
+        "synchronisation), best of 3: 24 B in + %d B out per node, %d B out per cell" % (W.name, sb, 96 if W.f32 else 192))
     torch.cuda.empty_cache()
     return out
 
@@ -542,6 +574,9 @@ def main():
                          "own Hilbert-curve mid-point insertion on length jumps (PAPER.md:194-206; DESIGN.md reading A17)")
     ap.add_argument("--hilbert-thr", type=float, default=0.05, help="field-line-length jump threshold of --refine hilbert")
     ap.add_argument("--hilbert-shift", type=int, default=5, help="shift of the second curve in fine cells (0 = no shifted pass)")
+    ap.add_argument("--interp-order", type=int, default=1, choices=[1, 2, 3],
+                    help="1 trilinear (cell-table kernel, default), 2 triquadratic (Dodgson), 3 tricubic (Keys): PAPER.md:91-93; the "
+                         "higher orders run in the stencil-gather kernel and are reported against the L1 gather rate")
     ap.add_argument("--e2e-chunks", type=int, default=0,
                     help="pieces the end-to-end path pipelines over two streams; 0 = one piece per 4 M lines (at most 8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -569,6 +604,8 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if args.arith == "f32" and args.workload not in ("cfg4", "cfg5"):
         raise SystemExit("--arith f32 needs an fp32-sampled workload (cfg4, cfg5)")
+    if args.interp_order != 1 and args.arith == "f32":
+        raise SystemExit("--interp-order 2 / 3 run in fp64 arithmetic")
 
     def barrier():
         if dist is not None:
@@ -624,6 +661,8 @@ def main():
     if rank == 0:
         peak_fma = qsl.qsl_peak_fma(not f32)           # DFMA/s (FFMA/s with --arith f32), measured on this device
         roofline = alu_roofline(W, T, peak_fma)
+        if W.order != 1:
+            roofline = dict(gather_roofline(W, T, qsl), alu=roofline)
         k_ms = T["kern_ms"][0] + T["kern_ms"][1]
         # the other candidate bounds of SURVEY.md 8(d): divergent gathers of table entries through L1 / L2.  Algorithmic
         # traffic: a line enters a new cell every ~2.5 steps at h = 0.25 cell and then reads one table entry (192 B fp64,
@@ -663,7 +702,7 @@ def main():
         "roofline_frac": alu_roofline(Wm, Tm, peak_fma)["frac"], "kernel_ms": (Tm["kern_ms"][0] + Tm["kern_ms"][1]) / Tm["steps"],
         "steps": Tm["steps"], "warmup": Tm["warmup"], "workload": WORKLOADS[name]}
     per_config = None
-    if rank == 0 and world == 1 and (not args.no_per_config):
+    if rank == 0 and world == 1 and (not args.no_per_config) and args.interp_order == 1 and args.scale == 1.0:
         per_config = {args.workload: summary(args.workload, T, W)}
         W.close()
         for name in sorted(WORKLOADS):
