@@ -48,6 +48,8 @@ FLOPS_PER_STEP = {"LQ": 800, "L": 400}
 NCU_CAPTURES = {
     ("cfg2", "f64"): {"dram_bytes": 789848320, "pipe_active": 0.484, "source": "profiles/r1b_cell_table_kernel.md (capture e)"},
     ("cfg4", "f64"): {"dram_bytes": 41683301000, "pipe_active": 0.517, "source": "profiles/r2a_cfg4_trace_kernel.md"},
+    ("cfg5", "f64"): {"dram_bytes": 344820435000, "pipe_active": 0.443,
+                      "source": "profiles/r2a_cfg5_level0_trace_kernel.md (the level-0 L-only launch, 9 % of the step)"},
 }
 DEFAULT_WORKLOAD = "cfg4"
 SELECT_PASSES = 8          # radix passes of qsl_select (select_refine.cu), for the streaming byte count

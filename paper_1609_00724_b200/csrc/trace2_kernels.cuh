@@ -71,7 +71,9 @@ struct LineState2 {
             x0[1] = fma((double)j, A.fv.h[1], A.fv.lo[1]);
             x0[2] = fma((double)k, A.fv.h[2], A.fv.lo[2]);
         }
-        const double4 *__restrict__ p = (const double4 *)A.fv.cells + (((size_t)k * (A.fv.ny - 1) + j) * (A.fv.nx - 1) + i) * 6;
+        // the cell count is below 2^31 (qsl_field_create): the index in 32-bit arithmetic, one wide multiply for the address
+        const unsigned lin = ((unsigned)k * (unsigned)(A.fv.ny - 1) + (unsigned)j) * (unsigned)(A.fv.nx - 1) + (unsigned)i;
+        const double4 *__restrict__ p = (const double4 *)A.fv.cells + (size_t)lin * 6;
 #pragma unroll
         for (int q = 0; q < 6; ++q) {
             const double4 v = load_cell4(p + q);
@@ -254,9 +256,16 @@ struct LineState2 {
 #define T ((size_t)gridDim.x * blockDim.x)
         double b[3], k[NV], d[3], bn, hs, h = 0.0;
         double acc[NV], accL, ys[NV];
+        // trial end: position xn; the deviation components of the trial end are y[c] + fc * inc[c], formed in place when
+        // the attempt is committed (accepted trial step or final landing step) - no other phase needs them
+        double xn[3], inc[NV], fc;
         {
             double p0[3] = { y[0], y[1], y[2] };
-            if (phase >= 2) { p0[0] = st[(ST_XT + 0) * T]; p0[1] = st[(ST_XT + 1) * T]; p0[2] = st[(ST_XT + 2) * T]; }
+            // warp-uniform test first: without it the address arithmetic of the (predicated) stash loads is issued in
+            // every attempt, although a lane is in a landing phase in only ~1 attempt of 10
+            if (__any_sync(__activemask(), phase >= 2)) {
+                if (phase >= 2) { p0[0] = st[(ST_XT + 0) * T]; p0[1] = st[(ST_XT + 1) * T]; p0[2] = st[(ST_XT + 2) * T]; }
+            }
             enter_cell(A, p0, d);
             stage(d, y, b, k);
             bn = SPH ? to_rates(p0, b, k) : norm3_fast(b);
@@ -301,7 +310,10 @@ struct LineState2 {
         const double shs = back ? -hs : hs;
         if (A.method == QSL_EULER) {
 #pragma unroll
-            for (int c = 0; c < NV; ++c) ys[c] = fma(shs, c < 3 ? b[c] : k[c], y[c]);
+            for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
+#pragma unroll
+            for (int c = 3; c < NV; ++c) inc[c] = k[c];
+            fc = shs;
             accL = fma(hs, bn, L);
         } else {
             // RK4 (reading A5): k2 = f(y + h/2 k1), k3 = f(y + h/2 k2), k4 = f(y + h k3), y+ = y + h/6 (k1 + 2 k2 + 2 k3 + k4)
@@ -350,36 +362,36 @@ struct LineState2 {
             if (SPH) bnS = to_rates(ys, b, k);
             {
                 const double fL = hs * (1.0 / 6.0), f = back ? -fL : fL;
-                double xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(f, fma(1.0, b[c], acc[c]), y[c]);
                 // the trial end is where the next attempt starts if it is accepted: enter its cell now
                 enter_cell(A, xn, d);
                 bn = SPH ? bnS : norm3_fast(b);
 #pragma unroll
-                for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, fma(1.0, k[c], acc[c]), y[c]);
+                for (int c = 3; c < NV; ++c) inc[c] = fma(1.0, k[c], acc[c]);
+                fc = f;
                 accL = fma(fL, fma(1.0, bn, accL), L);
             }
         }
-        // ys = trial end, accL = trial length
+        // xn = trial end, accL = trial length
         if (phase == 0) {
-            if (inside_box(A, ys)) {
-                if (SPH) move_anchor(ys[1] - y[1]);
+            if (inside_box(A, xn)) {
+                if (SPH) move_anchor(xn[1] - y[1]);
 #pragma unroll
-                for (int c = 0; c < NV; ++c) y[c] = ys[c];
+                for (int c = 0; c < NV; ++c) y[c] = c < 3 ? xn[c] : fma(fc, inc[c], y[c]);
                 L = accL; lam += h; ++nsteps;
                 return false;
             }
             // first face crossed by the chord: smallest fraction, tie -> lowest axis (reading A4)
-            double phi = INFINITY; int ax = -1, fc = 255; double bd = 0.0;
+            double phi = INFINITY; int ax = -1, face = 255; double bd = 0.0;
 #pragma unroll
             for (int dd = 0; dd < 3; ++dd) {
-                if (ys[dd] < A.box_lo[dd]) {
-                    const double f = (A.box_lo[dd] - y[dd]) / (ys[dd] - y[dd]);
-                    if (f < phi) { phi = f; ax = dd; fc = 2 * dd; bd = A.box_lo[dd]; }
-                } else if (ys[dd] > A.box_hi[dd]) {
-                    const double f = (A.box_hi[dd] - y[dd]) / (ys[dd] - y[dd]);
-                    if (f < phi) { phi = f; ax = dd; fc = 2 * dd + 1; bd = A.box_hi[dd]; }
+                if (xn[dd] < A.box_lo[dd]) {
+                    const double f = (A.box_lo[dd] - y[dd]) / (xn[dd] - y[dd]);
+                    if (f < phi) { phi = f; ax = dd; face = 2 * dd; bd = A.box_lo[dd]; }
+                } else if (xn[dd] > A.box_hi[dd]) {
+                    const double f = (A.box_hi[dd] - y[dd]) / (xn[dd] - y[dd]);
+                    if (f < phi) { phi = f; ax = dd; face = 2 * dd + 1; bd = A.box_hi[dd]; }
                 }
             }
             if (ax < 0) { finish(A, 255, REC_STALL); return true; }   // non-finite trial point
@@ -388,28 +400,28 @@ struct LineState2 {
                 // the line starts on the face it leaves through (photospheric seeds): hp = 0, every Newton residual is
                 // exactly 0, so the landing of O4 ends where it started: one zero-length step
                 ++nsteps;
-                finish(A, fc, 0);
+                finish(A, face, 0);
                 return true;
             }
             st[ST_HP * T] = phi * h; st[ST_BOUND * T] = bd; st[ST_HFULL * T] = h;
-            st[ST_AXIS_FACE * T] = __hiloint2double(ax, fc);
+            st[ST_AXIS_FACE * T] = __hiloint2double(ax, face);
             phase = 1;
             return false;
         }
         if (phase < 4) {
-            st[(ST_XT + 0) * T] = ys[0]; st[(ST_XT + 1) * T] = ys[1]; st[(ST_XT + 2) * T] = ys[2];
+            st[(ST_XT + 0) * T] = xn[0]; st[(ST_XT + 1) * T] = xn[1]; st[(ST_XT + 2) * T] = xn[2];
             ++phase;
             return false;
         }
         // phase 4: final landing step
         const double af = st[ST_AXIS_FACE * T];
-        const int axis = __double2hiint(af), fc = __double2loint(af);
+        const int axis = __double2hiint(af), face = __double2loint(af);
         const double bound = st[ST_BOUND * T];
 #pragma unroll
-        for (int c = 0; c < NV; ++c) y[c] = ys[c];
+        for (int c = 0; c < NV; ++c) y[c] = c < 3 ? xn[c] : fma(fc, inc[c], y[c]);
         if (axis == 0) y[0] = bound; else if (axis == 1) y[1] = bound; else y[2] = bound;
         L = accL; lam += st[ST_HP * T]; ++nsteps;
-        finish(A, fc, 0);
+        finish(A, face, 0);
         return true;
 #undef st
 #undef T
