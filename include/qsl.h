@@ -78,7 +78,8 @@ typedef struct {
                                     QSL_LAYOUT_NODES_ONLY: packed samples only; qsl_trace then gathers 8 corners per
                                     RK stage (the slower QSL_FLAG_KERNEL_V1 path), for fields too large for the table.
                                     QSL_LAYOUT_CELL_TABLE_F32: the same coefficients rounded to fp32 (96 B per cell),
-                                    the table of QSL_ARITH_F32; fp32 samples on a uniform grid only (else QSL_EINVAL);
+                                    the table of QSL_ARITH_F32; fp32 samples on a uniform grid only (else QSL_EINVAL;
+                                    Cartesian or spherical);
                                     QSL_ARITH_F64 traces of such a field run the corner kernel.
                                     QSL_LAYOUT_CELL_TABLES_BOTH: the fp64 and the fp32 table                          */
     int interp_order;            /* QSL_TRILINEAR (0, default; eq. 3-4) | QSL_TRIQUADRATIC (Dodgson 1997, 27
@@ -91,9 +92,10 @@ typedef struct {
                                     (phi^, theta^, r^) (PAPER.md:83-87 eq. 2, :111).  Seeds, trace box and end points are
                                     then (phi, theta, r); lines follow eq. (2), deviations eq. (6)-(7) as printed (without
                                     the metric-derivative terms), Q uses eq. (8); dev_f / dev_b are coordinate
-                                    deviations.  Uniform axes, QSL_NORMALIZE_FIRST, QSL_TRILINEAR, fp64, RK4 / Euler only
-                                    (else QSL_EINVAL); the cell-table kernel (fp64 table layouts) and the gather kernel
-                                    (QSL_LAYOUT_NODES_ONLY / QSL_FLAG_KERNEL_V1) both carry the geometry                  */
+                                    deviations.  Uniform axes, QSL_NORMALIZE_FIRST, QSL_TRILINEAR only (else QSL_EINVAL).
+                                    fp64 arithmetic: RK4 / Euler / CK45 in the cell-table kernels (fp64 table layouts), RK4 /
+                                    Euler in the gather kernel (QSL_LAYOUT_NODES_ONLY / QSL_FLAG_KERNEL_V1); fp32 arithmetic
+                                    (QSL_ARITH_F32, RK4 / Euler) on the fp32 table layouts of an fp32-sampled field         */
 } qsl_grid_desc;
 
 /* Packs the three component cubes (DEVICE, fp64, nx*ny*nz each) into one AoS array of (b^x, b^y, b^z, |B|) samples

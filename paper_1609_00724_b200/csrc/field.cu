@@ -157,6 +157,15 @@ __global__ void __launch_bounds__(CT_THREADS) cell_table_kernel(FieldView fv, O4
     }
 }
 
+__global__ void row_sincos_kernel(int n, const double *__restrict__ theta, float2 *__restrict__ out)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    double sn, cs;
+    sincos(theta[j], &sn, &cs);
+    out[j] = make_float2((float)sn, (float)cs);
+}
+
 }  // namespace qsl
 
 using namespace qsl;
@@ -206,7 +215,7 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     }
     const bool want64 = !ho && (d->layout == QSL_LAYOUT_CELL_TABLE || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH);
     const bool want32 = !ho && (d->layout == QSL_LAYOUT_CELL_TABLE_F32 || d->layout == QSL_LAYOUT_CELL_TABLES_BOTH);
-    if (want32 && (d->sample_type != QSL_F32 || d->stretched || sph)) return QSL_EINVAL;   // fp32 arithmetic: fp32 samples, uniform Cartesian grid
+    if (want32 && (d->sample_type != QSL_F32 || d->stretched)) return QSL_EINVAL;   // fp32 arithmetic: fp32 samples, uniform grid
     const long long n = (long long)d->nx * d->ny * d->nz;
     if (n >= (1ll << 31)) return QSL_ERANGE;   // node index is 32-bit inside the gather
     const int dims[3] = { d->nx, d->ny, d->nz };
@@ -227,7 +236,9 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
     f->d_samples = nullptr;
     f->d_cells = nullptr;
     f->d_cells32 = nullptr;
+    f->d_row_sc = nullptr;
     f->view.cells = nullptr;
+    f->view.row_sc = nullptr;
     for (int a = 0; a < 3; ++a) f->d_axis[a] = nullptr;
     f->sample_type = d->sample_type;
     f->n_nodes = n;
@@ -300,6 +311,17 @@ int qsl_field_create(qsl_field **out, const qsl_grid_desc *d, const double *bx, 
         cell_table_kernel<float4, float4><<<cblocks, CT_THREADS, 0, s>>>(f->view, (float4 *)f->d_cells32);
         e = cudaGetLastError();
         if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+        if (sph) {
+            // (sin, cos) of the latitude of every node row, in fp64 and rounded once: the fp32 kernel's frame (reading A19)
+            e = cudaMalloc(&f->d_row_sc, sizeof(float2) * (size_t)d->ny);
+            if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+            f->bytes += sizeof(float2) * (size_t)d->ny;
+            count_launch();
+            row_sincos_kernel<<<(d->ny + 127) / 128, 128, 0, s>>>(d->ny, f->d_axis[1], (float2 *)f->d_row_sc);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) { qsl_field_destroy(f); return record_cuda(e); }
+            f->view.row_sc = (const float2 *)f->d_row_sc;
+        }
     }
     *out = f;
     return QSL_OK;
@@ -311,6 +333,7 @@ int qsl_field_destroy(qsl_field *f)
     if (f->d_samples) cudaFree(f->d_samples);
     if (f->d_cells) cudaFree(f->d_cells);
     if (f->d_cells32) cudaFree(f->d_cells32);
+    if (f->d_row_sc) cudaFree(f->d_row_sc);
     for (int a = 0; a < 3; ++a)
         if (f->d_axis[a]) cudaFree(f->d_axis[a]);
     delete f;

@@ -39,6 +39,7 @@ struct FieldView {
     double lo[3], hi[3];
     double h[3];              // uniform spacing (hi - lo)/(n - 1)
     const double *axis[3];    // device node coordinates (always present)
+    const float2 *row_sc;     // spherical fields with the fp32 table: (sin, cos) of the latitude of node row j, else NULL
 };
 
 // Sort (key, value) pairs by 32-bit key, ascending, stable.  Hand-written LSD radix sort (order.cu).
@@ -56,6 +57,7 @@ struct qsl_field {
     void *d_samples;
     void *d_cells;
     void *d_cells32;          // fp32 coefficient table of the QSL_ARITH_F32 kernel, or NULL
+    void *d_row_sc;           // float2[ny] behind view.row_sc, or NULL
     double *d_axis[3];
     int sample_type;
     long long n_nodes;

@@ -6,7 +6,7 @@
 
 namespace qsl {
 
-template <typename T, typename S, bool DEV, bool INTERP>
+template <typename T, typename S, bool DEV, bool INTERP, bool SPH = false>
 static int launch_trace3_variant(Trace3Args<T> &A, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s)
 {
     const long long n_items = 2 * A.T0.n;
@@ -14,7 +14,7 @@ static int launch_trace3_variant(Trace3Args<T> &A, bool refill, cudaEvent_t ev0,
     long long blocks = (n_items + threads - 1) / threads;
     if (refill) {
         int per_sm = 0;
-        QSL_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace3_kernel<T, DEV, INTERP, true>, threads, 0));
+        QSL_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace3_kernel<T, DEV, INTERP, true, SPH>, threads, 0));
         if (per_sm < 1) per_sm = 1;
         const long long resident = (long long)sm_count() * per_sm;   // persistent: grid = SMs x resident CTAs
         if (blocks > resident) blocks = resident;
@@ -34,8 +34,8 @@ static int launch_trace3_variant(Trace3Args<T> &A, bool refill, cudaEvent_t ev0,
         if (e == cudaSuccess && ev0) e = cudaEventRecord(ev0, s);
         if (e == cudaSuccess) {
             count_launch();
-            if (refill) trace3_kernel<T, DEV, INTERP, true><<<(unsigned)blocks, threads, 0, s>>>(A);
-            else trace3_kernel<T, DEV, INTERP, false><<<(unsigned)blocks, threads, 0, s>>>(A);
+            if (refill) trace3_kernel<T, DEV, INTERP, true, SPH><<<(unsigned)blocks, threads, 0, s>>>(A);
+            else trace3_kernel<T, DEV, INTERP, false, SPH><<<(unsigned)blocks, threads, 0, s>>>(A);
             e = cudaGetLastError();
         }
         if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, s);
@@ -83,7 +83,18 @@ static int launch_trace3_t(const TraceArgs &G, const void *cells, bool dev, bool
     A.cell_sz = (dims[0] - 1) * (dims[1] - 1);
     A.null_eps = (T)G.null_eps;
     A.stash = nullptr;
+    A.row_sc = G.fv.row_sc;
+    A.step_frac = (T)G.step_frac;
     const bool in = G.fv.interp_mode == QSL_INTERP_FIRST;
+    if (G.fv.spherical) {       // fp32 arithmetic only (uniform axes, paper mode: qsl_field_create guarantees both)
+        if constexpr (sizeof(T) == 4) {
+            if (!G.fv.row_sc || in) return QSL_EINVAL;
+            return dev ? launch_trace3_variant<T, S, true, false, true>(A, refill, ev0, ev1, s)
+                       : launch_trace3_variant<T, S, false, false, true>(A, refill, ev0, ev1, s);
+        } else {
+            return QSL_EINVAL;
+        }
+    }
     if (dev) return in ? launch_trace3_variant<T, S, true, true>(A, refill, ev0, ev1, s) : launch_trace3_variant<T, S, true, false>(A, refill, ev0, ev1, s);
     return in ? launch_trace3_variant<T, S, false, true>(A, refill, ev0, ev1, s) : launch_trace3_variant<T, S, false, false>(A, refill, ev0, ev1, s);
 }

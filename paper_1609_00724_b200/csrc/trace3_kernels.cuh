@@ -25,6 +25,7 @@ template <> struct Real3<float> {
     // bit pattern for the "0 <= p < h" test (one unsigned compare per axis): exact in fp32
     static __device__ __forceinline__ unsigned bits(float v) { return (unsigned)__float_as_int(v); }
     static __device__ __forceinline__ float rsqrt_seed(float n2) { return rsqrtf(fmaxf(n2, 7.8886e-31f)); }
+    static __device__ __forceinline__ float rcp(float v) { return __frcp_rn(v); }
 };
 template <> struct Real3<double> {
     using V4 = double4;
@@ -42,6 +43,7 @@ template <> struct Real3<double> {
         asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(fmax(n2, 0x1p-600)));
         return r;
     }
+    static __device__ __forceinline__ double rcp(double v) { return 1.0 / v; }
 };
 
 template <typename T>
@@ -58,6 +60,10 @@ struct Trace3Args {
     T off_lo[3], off_hi[3];      // offsets of box_lo / box_hi from the origins of cells cl / ch
     T null_eps;
     T *stash;                    // per-thread landing scratch, STASH3_SLOTS x n_threads
+    // spherical geometry (reading A19; SPH instantiations): (sin, cos) of the latitude of every row of cells (fp64
+    // sincos rounded to fp32, built by qsl_field_create), and the step fraction (the step is sized per attempt)
+    const float2 *row_sc;
+    T step_frac;
 };
 
 enum { S3_K1 = 0, S3_BN = 9, S3_DXT = 10, S3_HP = 13, S3_HFULL = 14, S3_AXIS_FACE = 15, STASH3_SLOTS = 16 };
@@ -77,11 +83,16 @@ __device__ __forceinline__ T norm3r_fast(const T v[3])
     return fma(fma(-s1, s1, n2), h1, s1);
 }
 
-template <typename T, bool DEV, bool INTERP>
+// SPH: spherical geometry (reading A19) in the cell frame.  The frame carries the radius of the cell's origin and
+// (sin, cos) of its latitude; a point at offsets p has r = rc + p_r and cos(theta) = cc cos(p_theta) - sc sin(p_theta)
+// with short polynomials of the offset (|p_theta| < 2 h_theta; terms through p^6 / p^5: below the fp32 ulp for cell
+// edges up to 0.3 rad), so no evaluation calls a trigonometric function.
+template <typename T, bool DEV, bool INTERP, bool SPH = false>
 struct LineState3 {
     using Args = Trace3Args<T>;
     static constexpr int NV = DEV ? 9 : 3;
     T a[24];             // cached cell: monomial coefficients
+    T rc, sc, cc;        // SPH: radius and (sin, cos) of the latitude of the origin of cell C
     int C[3];                // its index = the frame of every offset below
     T y[NV];             // y[0..2]: offset of the line's point from the origin of cell C; delta1, delta2
     double L, lam;
@@ -97,6 +108,36 @@ struct LineState3 {
             const typename Real3<T>::V4 v = Real3<T>::load(p + q);
             a[4 * q] = v.x; a[4 * q + 1] = v.y; a[4 * q + 2] = v.z; a[4 * q + 3] = v.w;
         }
+        if (SPH) {
+            rc = (T)fma((double)C[2], A.T0.fv.h[2], A.T0.fv.lo[2]);
+            const float2 v = __ldg(A.row_sc + C[1]);
+            sc = (T)v.x; cc = (T)v.y;
+        }
+    }
+
+    // SPH: r cos(theta) and r of the point at offsets p of the frame
+    __device__ __forceinline__ void polar(const T p[3], T &rcos, T &r) const
+    {
+        const T d = p[1], d2 = d * d;
+        const T cd = fma(d2, fma(d2, fma(d2, T(-1.0 / 720.0), T(1.0 / 24.0)), T(-0.5)), T(1.));
+        const T sd = d * fma(d2, fma(d2, T(1.0 / 120.0), T(-1.0 / 6.0)), T(1.));
+        r = rc + p[2];
+        rcos = r * fma(cc, cd, -(sc * sd));
+    }
+
+    // |b| of the field vector and, with SPH, b -> coordinate rates and k -> coordinate deviation rates at offsets p:
+    // orthonormal components x (1 / (r cos theta), 1 / r, 1)  (PAPER.md:83-85 eq. 2, :125-135 eq. 6-7)
+    __device__ __forceinline__ T to_rates(const T p[3], T b[3], T *k) const
+    {
+        const T bn = norm3r_fast<T>(b);
+        if (SPH) {
+            T rcos, r;
+            polar(p, rcos, r);
+            const T m0 = Real3<T>::rcp(rcos), m1 = Real3<T>::rcp(r);
+            b[0] *= m0; b[1] *= m1;
+            if (DEV) { k[3 % NV] *= m0; k[4 % NV] *= m1; k[6 % NV] *= m0; k[7 % NV] *= m1; }
+        }
+        return bn;
     }
 
     // Makes the cached cell the one containing the point at offsets p (reading A8: the index is clamped to the grid,
@@ -211,6 +252,12 @@ struct LineState3 {
             y[6 % NV] = (T)b1.y; y[7 % NV] = (T)b2.x; y[8 % NV] = (T)b2.y;
         }
         load_cell(A);
+        if (SPH && DEV) {     // orthonormal pair -> coordinate deviations (eq. 8 inverted)
+            T rcos, r;
+            polar(y, rcos, r);
+            const T m0 = Real3<T>::rcp(rcos), m1 = Real3<T>::rcp(r);
+            y[3 % NV] *= m0; y[4 % NV] *= m1; y[6 % NV] *= m0; y[7 % NV] *= m1;
+        }
         return true;
     }
 
@@ -280,11 +327,16 @@ struct LineState3 {
             if (phase >= 2) { p0[0] += st[(S3_DXT + 0) * TT]; p0[1] += st[(S3_DXT + 1) * TT]; p0[2] += st[(S3_DXT + 2) * TT]; }
             enter_cell(A, p0);
             stage(p0, y, b, k);
-            bn = norm3r_fast<T>(b);
+            bn = to_rates(p0, b, k);
             if (phase == 0) {
                 if (!(bn >= A.null_eps)) { finish(A, 255, nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL, -1); return true; }
                 if ((long long)nsteps >= G.max_steps || lam >= G.max_length) { finish(A, 255, REC_CAP, -1); return true; }
                 h = A.h_step;
+                if (SPH) {   // physical cell edges (r cos(theta) h_phi, r h_theta, h_r) at the start of the step
+                    T rcos, r;
+                    polar(y, rcos, r);
+                    h = A.step_frac * fmin(rcos * A.hf[0], fmin(r * A.hf[1], A.hf[2]));
+                }
                 if (lam + (double)h > G.max_length) h = (T)(G.max_length - lam);
                 hs = h;
             } else {
@@ -332,12 +384,14 @@ struct LineState3 {
             accL = bn;
             // ---- stage 2
             stage(ys, ys, b, k);
+            T bnS = T(0.);             // SPH: |b| is taken before the scaling to coordinate rates
+            if (SPH) bnS = to_rates(ys, b, k);
             {
                 T xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
                 enter_cell(A, xn);
-                bn = norm3r_fast<T>(b);
+                bn = SPH ? bnS : norm3r_fast<T>(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) {
                     const T kc = c < 3 ? b[c] : k[c];
@@ -347,12 +401,13 @@ struct LineState3 {
             }
             // ---- stage 3
             stage(ys, ys, b, k);
+            if (SPH) bnS = to_rates(ys, b, k);
             {
                 T xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
                 enter_cell(A, xn);
-                bn = norm3r_fast<T>(b);
+                bn = SPH ? bnS : norm3r_fast<T>(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) {
                     const T kc = c < 3 ? b[c] : k[c];
@@ -362,13 +417,14 @@ struct LineState3 {
             }
             // ---- stage 4
             stage(ys, ys, b, k);
+            if (SPH) bnS = to_rates(ys, b, k);
             {
                 const T fL = hs * (T(1.0) / T(6.0)), f = back ? -fL : fL;
                 T xn[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) xn[c] = fma(f, b[c] + acc[c], y[c]);
                 enter_cell(A, xn);             // the trial end is where the next attempt starts if it is accepted
-                bn = norm3r_fast<T>(b);
+                bn = SPH ? bnS : norm3r_fast<T>(b);
 #pragma unroll
                 for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, k[c] + acc[c], y[c]);
                 accL = fL * (bn + accL);
@@ -473,12 +529,12 @@ __global__ void __launch_bounds__(128) seed_basis3_kernel(const TraceArgs A, dou
 #endif
 // Persistent grid, work items (one direction of one line) popped from a global counter with a warp-aggregated atomic; a
 // lane whose line ended refills at once (same queue as trace2_kernel).
-template <typename T, bool DEV, bool INTERP, bool REFILL>
+template <typename T, bool DEV, bool INTERP, bool REFILL, bool SPH = false>
 __global__ void __launch_bounds__(QSL_T3_THREADS, sizeof(T) == 4 ? (DEV ? QSL_T3_MIN_BLOCKS_LQ : QSL_T3_MIN_BLOCKS_L)
                                                                   : (DEV ? QSL_T3_MIN_BLOCKS_LQ64 : QSL_T3_MIN_BLOCKS_L64))
     trace3_kernel(const Trace3Args<T> A)
 {
-    LineState3<T, DEV, INTERP> ls;
+    LineState3<T, DEV, INTERP, SPH> ls;
     const long long n_items = 2 * A.T0.n;
     unsigned long long my_steps = 0;
     if (!REFILL) {

@@ -79,6 +79,45 @@ def test_sph_wedge_cash_karp(mode, tol):
     assert np.abs(gg["q_perp"] - 2).max() < 1e-9 and np.abs(gg["L"] - 2).max() < 1e-11
 
 
+@pytest.mark.parametrize("mode", [qsl.QSL_TRACE_LQ, qsl.QSL_TRACE_L])
+@pytest.mark.parametrize("method", [qsl.QSL_RK4, qsl.QSL_EULER])
+def test_sph_wedge_fp32_arithmetic(mode, method):
+    """QSL_ARITH_F32 in spherical geometry (the cell-frame kernel with the frame's radius and latitude sin / cos): the gates
+    of reading A6 against the fp64 oracle on the same fp32-rounded samples."""
+    from tests.test_gpu_trace_f32 import compare_f32
+    g = qi.Grid.uniform((48, 40, 44), (0.0, -0.9, 1.0), (2.0, 0.9, 2.4))
+    B = _cubes(g, _dipole_plus)
+    rng = np.random.default_rng(7)
+    n = 4000
+    seeds = np.stack([rng.uniform(0.1, 1.9, n), rng.uniform(-0.8, 0.8, n), rng.uniform(1.0, 2.2, n)], 1)
+    seeds[:500, 2] = 1.0
+    dev = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda() for a in B]
+    fg = qsl.qsl_field_create(g.nx, g.ny, g.nz, *dev, lo=g.lo, hi=g.hi, sample_type=qsl.QSL_F32, geometry=SPH,
+                              layout=qsl.QSL_LAYOUT_CELL_TABLES_BOTH)
+    kw = dict(method=method, mode=mode, max_steps=50000, step_frac=0.2 if method == qsl.QSL_EULER else 0.25)
+    tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    res = qsl.qsl_trace(fg, torch.from_numpy(seeds).cuda(), qsl.make_trace_params(g.lo, g.hi, arith=qsl.QSL_ARITH_F32, **kw),
+                        total_steps=tot)
+    torch.cuda.synchronize()
+    gg = {k: v.cpu().numpy() for k, v in res.items()}
+    gg["total_steps"] = int(tot.item())
+    for k in ("status", "nsteps_f", "nsteps_b"):
+        gg[k] = gg[k].view(np.uint32)
+    fc = oracle.Field(g, B, oracle.F32, oracle.NORMALIZE_FIRST, oracle.TRILINEAR, oracle.SPHERICAL)
+    c = oracle.trace(fc, seeds, g.lo, g.hi, **kw)
+    rep = compare_f32(gg, c, g.lo, g.hi, with_q=mode == qsl.QSL_TRACE_LQ, label="sph wedge f32 arithmetic")
+    assert rep["end_med"] < 1e-6 and rep["L_med"] < 1e-6
+    # the fp64 table of the same field gives the fp64 result at the north_star gates
+    g64 = qsl.qsl_trace(fg, torch.from_numpy(seeds).cuda(), qsl.make_trace_params(g.lo, g.hi, **kw), total_steps=tot)
+    torch.cuda.synchronize()
+    g64 = {k: v.cpu().numpy() for k, v in g64.items()}
+    g64["total_steps"] = int(tot.item())
+    for k in ("status", "nsteps_f", "nsteps_b"):
+        g64[k] = g64[k].view(np.uint32)
+    compare_trace(g64, c, g.lo, g.hi, with_q=mode == qsl.QSL_TRACE_LQ, label="sph wedge f32 samples, f64 arithmetic")
+    fg.destroy()
+
+
 def test_sph_cartesian_limit_euler_caps_inner_box():
     R0, p0, t0 = 1.0e5, 0.3, 0.2
     c0 = math.cos(t0)
@@ -119,7 +158,7 @@ def test_sph_argument_errors():
         qsl.qsl_field_create(5, 5, 5, z, z, z, xs=[0, .1, .3, .6, 1], ys=[0, .1, .3, .6, 1], zs=[1, 1.1, 1.3, 1.6, 2], geometry=SPH)
     f = qsl.qsl_field_create(5, 5, 5, z, z, z, **kw)
     seeds = torch.tensor([[0.5, 0.5, 1.5]], dtype=torch.float64, device="cuda")
-    for bad in (dict(arith=qsl.QSL_ARITH_F32),):
+    for bad in (dict(arith=qsl.QSL_ARITH_F32),):                  # fp64 samples have no fp32 table
         with pytest.raises(qsl.QslError):
             qsl.qsl_trace(f, seeds, qsl.make_trace_params((0, 0, 1), (1, 1, 2), **bad))
     # the cell-frame kernel does not carry the geometry: the flag is ignored, the result is the spherical one
