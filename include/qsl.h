@@ -93,8 +93,8 @@ typedef struct {
                                     then (phi, theta, r); lines follow eq. (2), deviations eq. (6)-(7) as printed (without
                                     the metric-derivative terms), Q uses eq. (8); dev_f / dev_b are coordinate
                                     deviations.  Uniform axes, QSL_NORMALIZE_FIRST, QSL_TRILINEAR only (else QSL_EINVAL).
-                                    fp64 arithmetic: RK4 / Euler / CK45 in the cell-table kernels (fp64 table layouts), RK4 /
-                                    Euler in the gather kernel (QSL_LAYOUT_NODES_ONLY / QSL_FLAG_KERNEL_V1); fp32 arithmetic
+                                    fp64 arithmetic: RK4 / Euler / CK45 in the cell-table kernels (fp64 table layouts) and in the
+                                    gather kernels (QSL_LAYOUT_NODES_ONLY / QSL_FLAG_KERNEL_V1); fp32 arithmetic
                                     (QSL_ARITH_F32, RK4 / Euler) on the fp32 table layouts of an fp32-sampled field         */
 } qsl_grid_desc;
 
@@ -113,7 +113,7 @@ long long qsl_field_bytes(const qsl_field *f);
 /* ---- trace (PAPER.md:79 eq. 1; :119 eq. 5; :141 integrators; :156-176 eq. 9-11 Q; :163 boundaries; :165 cap) --- */
 typedef struct {
     double box_lo[3], box_hi[3]; /* trace box, inside the grid box; may be smaller (raised lower boundary) */
-    int method;                  /* QSL_RK4 | QSL_EULER | QSL_CK45 (fp64 arithmetic on the fp64 cell table only)   */
+    int method;                  /* QSL_RK4 | QSL_EULER | QSL_CK45 (fp64 arithmetic; every layout, order and geometry) */
     double step_frac;            /* h = step_frac * min_d h_c,d of the cell containing x; > 0   */
     int mode;                    /* QSL_TRACE_L | QSL_TRACE_LQ                                                      */
     int arith;                   /* QSL_ARITH_F64 | QSL_ARITH_F32                                                   */

@@ -10,6 +10,8 @@ cudaError_t launch_trace_f32(const TraceArgs &A, bool dev, bool refill, cudaStre
 cudaError_t launch_trace_f64(const TraceArgs &A, bool dev, bool refill, cudaStream_t s);
 int launch_trace2(TraceArgs &A, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 int launch_trace_ck(TraceArgs &A, double tol, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
+cudaError_t launch_trace_ckg_f32(const TraceArgs &A, double tol, bool dev, cudaStream_t s);
+cudaError_t launch_trace_ckg_f64(const TraceArgs &A, double tol, bool dev, cudaStream_t s);
 int launch_trace3(const TraceArgs &T, const void *cells32, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 int launch_trace3_f64(const TraceArgs &T, bool samples_f32, bool dev, bool refill, cudaEvent_t ev0, cudaEvent_t ev1, cudaStream_t s);
 cudaError_t launch_epilogue_f32(const EpilogueArgs &E, cudaStream_t s);
@@ -62,9 +64,8 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
 {
     if (!f || !p || !out || n < 0 || (n > 0 && !seeds)) return QSL_EINVAL;
     if (p->method != QSL_RK4 && p->method != QSL_EULER && p->method != QSL_CK45) return QSL_EINVAL;
-    // the adaptive stepper runs in fp64 on the fp64 cell table only, with a positive tolerance
-    if (p->method == QSL_CK45 && (!f->view.cells || p->arith != QSL_ARITH_F64 || !(p->tol > 0.0)))
-        return QSL_EINVAL;
+    // the adaptive stepper runs in fp64 arithmetic, with a positive tolerance
+    if (p->method == QSL_CK45 && (p->arith != QSL_ARITH_F64 || !(p->tol > 0.0))) return QSL_EINVAL;
     if (p->mode != QSL_TRACE_L && p->mode != QSL_TRACE_LQ) return QSL_EINVAL;
     if (p->arith != QSL_ARITH_F64 && p->arith != QSL_ARITH_F32) return QSL_EINVAL;
     // fp32 arithmetic (reading A6): needs the fp32 coefficient table (QSL_LAYOUT_CELL_TABLE_F32 / _BOTH), which
@@ -105,9 +106,16 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
         e = cudaMemsetAsync(queue, 0, sizeof(unsigned long long), s);
         const bool dev = p->mode == QSL_TRACE_LQ;
         const bool v2 = f->view.cells != nullptr && !(p->flags & QSL_FLAG_KERNEL_V1);
-        if (e == cudaSuccess && p->method == QSL_CK45) {
+        if (e == cudaSuccess && p->method == QSL_CK45 && v2) {
             const int ps = prof_slot(p->mode);
             rc = launch_trace_ck(A, p->tol, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);
+        } else if (e == cudaSuccess && p->method == QSL_CK45) {
+            // no per-cell table (nodes-only layout, higher-order interpolation) or QSL_FLAG_KERNEL_V1: the gather kernel
+            const int ps = prof_slot(p->mode);
+            if (ps >= 0) e = cudaEventRecord(g_ev0[ps], s);
+            if (e == cudaSuccess)
+                e = f->sample_type == QSL_F32 ? launch_trace_ckg_f32(A, p->tol, dev, s) : launch_trace_ckg_f64(A, p->tol, dev, s);
+            if (e == cudaSuccess && ps >= 0) e = cudaEventRecord(g_ev1[ps], s);
         } else if (e == cudaSuccess && p->arith == QSL_ARITH_F32) {
             const int ps = prof_slot(p->mode);
             rc = launch_trace3(A, f->d_cells32, dev, refill, ps >= 0 ? g_ev0[ps] : nullptr, ps >= 0 ? g_ev1[ps] : nullptr, s);

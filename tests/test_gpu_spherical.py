@@ -56,9 +56,10 @@ def test_sph_wedge_field(st, mode, flags):
     assert (c["face_f"] == 4).mean() > 0.2 and (c["status"] & oracle.ST_OPEN).mean() > 0.05      # closed and open lines
 
 
+@pytest.mark.parametrize("flags", KERNELS)
 @pytest.mark.parametrize("mode", [qsl.QSL_TRACE_LQ, qsl.QSL_TRACE_L])
 @pytest.mark.parametrize("tol", [1e-2, 1e-5])
-def test_sph_wedge_cash_karp(mode, tol):
+def test_sph_wedge_cash_karp(mode, tol, flags):
     """The paper's own workload class: a spherical wedge traced with the adaptive Cash-Karp stepper (PAPER.md:141-143,
     :232-254).  Same controller decisions on both sides (reading A16), so per-line step counts agree."""
     g = qi.Grid.uniform((48, 40, 44), (0.0, -0.9, 1.0), (2.0, 0.9, 2.4))
@@ -67,14 +68,15 @@ def test_sph_wedge_cash_karp(mode, tol):
     n = 3000
     seeds = np.stack([rng.uniform(0.1, 1.9, n), rng.uniform(-0.8, 0.8, n), rng.uniform(1.0, 2.2, n)], 1)
     seeds[:400, 2] = 1.0
-    gg, c = run_both(g, B, "f64", seeds, g.lo, g.hi, geometry=SPH, mode=mode, max_steps=50000, method=qsl.QSL_CK45, tol=tol)
+    gg, c = run_both(g, B, "f64", seeds, g.lo, g.hi, geometry=SPH, mode=mode, max_steps=50000, method=qsl.QSL_CK45, tol=tol,
+                     flags=flags)
     rep = compare_trace(gg, c, g.lo, g.hi, with_q=mode == qsl.QSL_TRACE_LQ, label="wedge ck45 tol %g" % tol)
     assert rep["same_steps"] >= 0.999
     # the monopole with the adaptive stepper: radial lines, Q = 2
     g = qi.Grid.uniform((9, 11, 33), (0.1, -0.3, 1.0), (0.9, 0.5, 3.0))
     B = _cubes(g, lambda p, t, r: (0 * r, 0 * r, 1 / r ** 2))
     seeds = np.array([[0.33, 0.11, g.zs[7]], [0.71, -0.22, g.zs[20]], [0.5, 0.4, g.zs[1]]])
-    gg, c = run_both(g, B, "f64", seeds, g.lo, g.hi, geometry=SPH, method=qsl.QSL_CK45, tol=tol)
+    gg, c = run_both(g, B, "f64", seeds, g.lo, g.hi, geometry=SPH, method=qsl.QSL_CK45, tol=tol, flags=flags)
     compare_trace(gg, c, g.lo, g.hi, frac=1.0, label="monopole ck45")
     assert np.abs(gg["q_perp"] - 2).max() < 1e-9 and np.abs(gg["L"] - 2).max() < 1e-11
 

@@ -78,9 +78,44 @@ def test_ck_argument_errors():
     for kw in (dict(tol=0.0), dict(tol=float("nan")), dict(arith=qsl.QSL_ARITH_F32)):
         with pytest.raises(qsl.QslError):
             qsl.qsl_trace(f, seeds, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], method=CK, **kw))
+    # without a per-cell table (nodes-only layout) the adaptive stepper runs in the gather kernel: same result as the
+    # table kernel of the same field to rounding
+    a = qsl.qsl_trace(f, seeds, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], method=CK, max_steps=cfg["max_steps"]))
     f.destroy()
     f = qsl.qsl_field_create(grid.nx, grid.ny, grid.nz, *dev, lo=grid.lo, hi=grid.hi, sample_type=qsl.QSL_F32,
                              layout=qsl.QSL_LAYOUT_NODES_ONLY)
-    with pytest.raises(qsl.QslError):          # the adaptive stepper needs the fp64 cell table
-        qsl.qsl_trace(f, seeds, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], method=CK))
+    b = qsl.qsl_trace(f, seeds, qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], method=CK, max_steps=cfg["max_steps"]))
+    torch.cuda.synchronize()
+    assert torch.equal(a["nsteps_f"], b["nsteps_f"]) and torch.allclose(a["L"], b["L"], rtol=1e-10, atol=0)
+    assert torch.allclose(a["q_perp"], b["q_perp"], rtol=1e-7, atol=0)
     f.destroy()
+
+
+V1 = qsl.QSL_FLAG_KERNEL_V1
+
+
+@pytest.mark.parametrize("name,scale,st,order", [("cfg2", 1.0 / 8, "f64", 1), ("cfg4", 1.0 / 8, "f32", 1), ("cfg2", 1.0 / 8, "f64", 2),
+                                                 ("cfg2", 1.0 / 8, "f64", 3), ("cfg4", 1.0 / 8, "f32", 3)])
+@pytest.mark.parametrize("mode", [qsl.QSL_TRACE_LQ, qsl.QSL_TRACE_L])
+def test_ck_in_the_gather_kernel(name, scale, st, order, mode):
+    """QSL_CK45 on fields without a per-cell table (QSL_FLAG_KERNEL_V1 forces the gather kernel on a trilinear field; the
+    higher interpolation orders have no table at all): PAPER.md:91-93 with :141-143, the robustness checks the paper offers
+    both options for."""
+    cfg = qi.make_config(name, scale)
+    g, c = run_both(cfg["grid"], cfg["B"], st, cfg["seeds"], cfg["box_lo"], cfg["box_hi"], method=CK, mode=mode,
+                    max_steps=cfg["max_steps"], flags=V1 if order == 1 else 0, order=order, tol=1e-3)
+    rep = compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], with_q=mode == qsl.QSL_TRACE_LQ, label="ck gather %s order %d" % (name, order))
+    assert rep["same_steps"] >= 0.999
+
+
+def test_ck_in_the_gather_kernel_stretched_interp_first_caps():
+    g = qi.Grid.from_axes(qi.stretched_axis(40, -1, 1, 3.0), qi.stretched_axis(36, -1, 1, 0.4), qi.stretched_axis(44, 0, 1, 5.0))
+    B = qi.hyperbolic_field(g, 2.0)
+    rng = np.random.default_rng(23)
+    seeds = np.stack([rng.uniform(-0.5, 0.5, 500), rng.uniform(-0.5, 0.5, 500), rng.uniform(0, 0.9, 500)], 1)
+    lo, hi = (-1, -1, 0), (1, 1, 1)
+    for kw in (dict(interp_mode=0), dict(interp_mode=1), dict(order=3), dict(max_steps=3), dict(max_length=0.1)):
+        gg, c = run_both(g, B, "f64", seeds, lo, hi, method=CK, tol=1e-4, flags=0 if "order" in kw else V1, **kw)
+        compare_trace(gg, c, lo, hi, label="ck gather stretched " + str(kw))
+    gg, c = run_both(g, B, "f64", seeds, (-0.9, -0.8, 0.13), (0.85, 0.9, 0.77), method=CK, flags=V1)
+    compare_trace(gg, c, (-0.9, -0.8, 0.13), (0.85, 0.9, 0.77), label="ck gather inner box")
