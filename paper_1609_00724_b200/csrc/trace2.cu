@@ -16,12 +16,11 @@ static int launch_trace2_variant(TraceArgs &A, bool refill, cudaEvent_t ev0, cud
         const long long resident = (long long)sm_count() * per_sm;   // persistent: every CTA resident, grid = SMs x occupancy
         if (blocks > resident) blocks = resident;
     }
-    void *basis = nullptr, *stash = nullptr;
-    int rc = scratch_alloc(&stash, sizeof(double) * STASH_DOUBLES * (size_t)blocks * threads, s);
-    if (rc == QSL_OK && DEV) rc = scratch_alloc(&basis, sizeof(double) * 6 * (size_t)A.n, s);
+    void *basis = nullptr;
+    int rc = QSL_OK;
+    if (DEV) rc = scratch_alloc(&basis, sizeof(double) * 6 * (size_t)A.n, s);
     cudaError_t e = cudaSuccess;
     if (rc == QSL_OK) {
-        A.stash = (double *)stash;
         if (DEV) {
             count_launch();
             seed_basis_kernel<STRETCHED, INTERP><<<(unsigned)((A.n + 127) / 128), 128, 0, s>>>(A, (double *)basis);
@@ -35,10 +34,16 @@ static int launch_trace2_variant(TraceArgs &A, bool refill, cudaEvent_t ev0, cud
             else trace2_kernel<DEV, STRETCHED, INTERP, false, SPH><<<(unsigned)blocks, threads, 0, s>>>(A);
             e = cudaGetLastError();
         }
+        if (e == cudaSuccess) {
+            // the landings (reading A4) of all lines at once; part of the trace time
+            count_launch();
+            landing_kernel<DEV, STRETCHED, INTERP, SPH><<<(unsigned)((n_items + 127) / 128), 128, 0, s>>>(A);
+            e = cudaGetLastError();
+        }
         if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, s);
         if (e != cudaSuccess) rc = record_cuda(e);
     }
-    scratch_free(basis, s); scratch_free(stash, s);
+    scratch_free(basis, s);
     return rc;
 }
 

@@ -36,9 +36,9 @@ __device__ __forceinline__ double norm3_fast(const double v[3])
     return fma(fma(-s1, s1, n2), h1, s1);
 }
 
-// Per-thread scratch of the landing (reading A4), in global memory: used only by the last five attempts of a line, so
-// it must not occupy registers during the thousands of plain steps.  Layout [slot * n_threads + thread].
-enum { ST_K1 = 0, ST_BN = 9, ST_XT = 10, ST_HP = 13, ST_BOUND = 14, ST_HFULL = 15, ST_AXIS_FACE = 16, STASH_DOUBLES = 17 };
+// Record flag of the cell-table kernel: the trial step from the recorded state leaves the trace box, the landing of
+// reading A4 is still to be done (landing_kernel clears it).  Bits 8..11 are the REC_* status flags of trace_kernels.cuh.
+constexpr uint32_t REC_LANDING = 1u << 12;
 
 // SPH: spherical geometry (reading A19): the coordinate rates are the orthonormal components times the metric factors
 // (1/(r cos theta), 1/r, 1) of the evaluation point; |b| for L and the stall test is taken before the scaling.
@@ -192,6 +192,28 @@ struct LineState2 {
         return bn;
     }
 
+    // Starts a line at the seed x with the orthonormal pair bs (a^, b^; unused without DEV) for record slot sl.
+    // Returns false if the item ended at once (seed outside the trace box).
+    __device__ __forceinline__ bool start(const TraceArgs &A, const double x[3], const double *bs, uint32_t sl)
+    {
+        slot = sl;
+        back = (long long)sl >= A.n;
+        L = 0.0; lam = 0.0; nsteps = 0; phase = 0;
+        if (SPH) sincos(x[1], &sth, &cth); else { sth = 0.0; cth = 1.0; }
+#pragma unroll
+        for (int c = 0; c < NV; ++c) y[c] = c < 3 ? x[c] : bs[(c - 3) % 6];
+        if (!inside_box(A, x)) { finish(A, 255, REC_SEED_OUTSIDE); return false; }
+        x0[0] = x0[1] = x0[2] = __longlong_as_double(0x7ff8000000000000ll);    // no cell cached yet
+        hc[0] = hc[1] = hc[2] = 0.0;
+        if (DEV && SPH) {   // orthonormal pair -> coordinate deviations (eq. 8 inverted)
+            double mf[3];
+            metric_shift(x[2], sth, cth, 0.0, mf);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { y[(3 + c) % NV] *= mf[c]; y[(6 + c) % NV] *= mf[c]; }
+        }
+        return true;
+    }
+
     // Starts work item q.  Returns false if the item ended at once (seed outside the trace box).  The orthonormal pair
     // a^, b^ of O2 comes from seed_basis_kernel (one thread per seed, all lanes busy) instead of being built here by
     // the one or two lanes of a warp that happen to be refilling; a null at the seed is caught by the first attempt.
@@ -199,29 +221,15 @@ struct LineState2 {
     {
         long long pos; int dir;
         if (A.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= A.n ? 1 : 0; pos = q - (long long)dir * A.n; }
-        slot = (uint32_t)((long long)dir * A.n + pos);
-        back = dir != 0;
         const uint32_t si = A.perm[pos];
         const double x[3] = { A.seeds[3 * (size_t)si], A.seeds[3 * (size_t)si + 1], A.seeds[3 * (size_t)si + 2] };
-        L = 0.0; lam = 0.0; nsteps = 0; phase = 0;
-        if (SPH) sincos(x[1], &sth, &cth); else { sth = 0.0; cth = 1.0; }
-#pragma unroll
-        for (int c = 0; c < NV; ++c) y[c] = c < 3 ? x[c] : 0.0;
-        if (!inside_box(A, x)) { finish(A, 255, REC_SEED_OUTSIDE); return false; }
-        x0[0] = x0[1] = x0[2] = __longlong_as_double(0x7ff8000000000000ll);    // no cell cached yet
-        hc[0] = hc[1] = hc[2] = 0.0;
+        double bs[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
         if (DEV) {
             const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(A.basis + 6 * (size_t)pos);
             const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
-            y[3 % NV] = b0.x; y[4 % NV] = b0.y; y[5 % NV] = b1.x; y[6 % NV] = b1.y; y[7 % NV] = b2.x; y[8 % NV] = b2.y;
-            if (SPH) {   // orthonormal pair -> coordinate deviations (eq. 8 inverted)
-                double mf[3];
-                metric_shift(x[2], sth, cth, 0.0, mf);
-#pragma unroll
-                for (int c = 0; c < 3; ++c) { y[(3 + c) % NV] *= mf[c]; y[(6 + c) % NV] *= mf[c]; }
-            }
+            bs[0] = b0.x; bs[1] = b0.y; bs[2] = b1.x; bs[3] = b1.y; bs[4] = b2.x; bs[5] = b2.y;
         }
-        return true;
+        return start(A, x, bs, (uint32_t)((long long)dir * A.n + pos));
     }
 
     __device__ void finish(const TraceArgs &A, int face, uint32_t flags)
@@ -238,75 +246,24 @@ struct LineState2 {
         for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
     }
 
-    // One attempt = exactly four field evaluations for every lane, whatever its phase, so a warp never diverges on the
-    // integrator itself:
-    //   phase 0     trial RK4 step of size h from y; accepted if the trial end is inside the closed trace box, else the
-    //               chord fraction gives the first landing step size hp (reading A4) and the lane enters phase 1
-    //   phase 1     step of size hp from the same y (k1 is recomputed by the first evaluation and stashed); the trial end
-    //               xt is stashed too
-    //   phase 2..4  the first evaluation is spent at xt instead of y: one Newton update of hp from b(xt); k1 comes back
-    //               from the stash; step of size hp; phase 4 snaps the end onto the face and finishes the line
-    // i.e. hp0 -> step, Newton, step, Newton, step, Newton, final step: the three Newton updates of O4.
+    // Step size of a trial step from the current state (reading A5; spherical: physical cell edges, reading A19)
+    __device__ __forceinline__ double step_size(const TraceArgs &A) const
+    {
+        double h = STRETCHED ? A.step_frac * fmin(hc[0], fmin(hc[1], hc[2])) : A.h_uniform;
+        if (SPH) h = A.step_frac * fmin(y[2] * cth * A.fv.h[0], fmin(y[2] * A.fv.h[1], A.fv.h[2]));
+        if (lam + h > A.max_length) h = A.max_length - lam;
+        return h;
+    }
+
+    // One step of size hs from y given k1 = (b, k[3..]) and bn = |b| at y (both consumed): trial end xn, the deviation
+    // increments inc (trial end of component c >= 3 is y[c] + fc inc[c], formed only when the step is committed) and the
+    // trial length accL.  Four field evaluations per RK4 step in all; the cached cell on return is that of xn.
     // Within a stage the order is: polynomial + deviation products -> position of the next stage point -> enter_cell
     // for it (table loads in flight) -> |b|, accumulators.  The direction sign is folded into the step size.
-    __device__ bool advance(const TraceArgs &A)
+    __device__ __forceinline__ void trial(const TraceArgs &A, double hs, double b[3], double *k, double bn, double xn[3],
+                                          double *inc, double &fc, double &accL)
     {
-        // this thread's landing scratch and its stride: recomputed where needed (rare) rather than held in registers
-#define st (A.stash + ((size_t)blockIdx.x * blockDim.x + threadIdx.x))
-#define T ((size_t)gridDim.x * blockDim.x)
-        double b[3], k[NV], d[3], bn, hs, h = 0.0;
-        double acc[NV], accL, ys[NV];
-        // trial end: position xn; the deviation components of the trial end are y[c] + fc * inc[c], formed in place when
-        // the attempt is committed (accepted trial step or final landing step) - no other phase needs them
-        double xn[3], inc[NV], fc;
-        {
-            double p0[3] = { y[0], y[1], y[2] };
-            // warp-uniform test first: without it the address arithmetic of the (predicated) stash loads is issued in
-            // every attempt, although a lane is in a landing phase in only ~1 attempt of 10
-            if (__any_sync(__activemask(), phase >= 2)) {
-                if (phase >= 2) { p0[0] = st[(ST_XT + 0) * T]; p0[1] = st[(ST_XT + 1) * T]; p0[2] = st[(ST_XT + 2) * T]; }
-            }
-            enter_cell(A, p0, d);
-            stage(d, y, b, k);
-            bn = SPH ? to_rates(p0, b, k) : norm3_fast(b);
-            if (phase == 0) {
-                // O4: stall / caps are tested on k1 before the step; h from the cell containing x
-                if (!(bn >= A.null_eps)) { finish(A, 255, nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL); return true; }
-                if ((long long)nsteps >= A.max_steps || lam >= A.max_length) { finish(A, 255, REC_CAP); return true; }
-                h = STRETCHED ? A.step_frac * fmin(hc[0], fmin(hc[1], hc[2])) : A.h_uniform;
-                if (SPH)   // physical cell edges (r cos(theta) h_phi, r h_theta, h_r) at the start of the step
-                    h = A.step_frac * fmin(y[2] * cth * A.fv.h[0], fmin(y[2] * A.fv.h[1], A.fv.h[2]));
-                if (lam + h > A.max_length) h = A.max_length - lam;
-                hs = h;
-            } else {
-                double hp = st[ST_HP * T];
-                if (phase == 1) {
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) st[(ST_K1 + c) * T] = b[c];
-#pragma unroll
-                    for (int c = 3; c < NV; ++c) st[(ST_K1 + c) * T] = k[c];
-                    st[ST_BN * T] = bn;
-                } else {
-                    // Newton update of hp from the field at the previous trial end (clamped to [0, h_full])
-                    const int axis = __double2hiint(st[ST_AXIS_FACE * T]);
-                    const double bound = st[ST_BOUND * T], hfull = st[ST_HFULL * T];
-                    const double bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
-                    const double xd = axis == 0 ? p0[0] : (axis == 1 ? p0[1] : p0[2]);
-                    const double gg = back ? -bd : bd, r = xd - bound;
-                    if (gg != 0.0) {
-                        const double hn = hp - r / gg;
-                        if (hn == hn) hp = fmin(fmax(hn, 0.0), hfull);
-                    }
-                    st[ST_HP * T] = hp;
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) b[c] = st[(ST_K1 + c) * T];
-#pragma unroll
-                    for (int c = 3; c < NV; ++c) k[c] = st[(ST_K1 + c) * T];
-                    bn = st[ST_BN * T];
-                }
-                hs = hp;
-            }
-        }
+        double d[3], acc[NV], ys[NV];
         const double shs = back ? -hs : hs;
         if (A.method == QSL_EULER) {
 #pragma unroll
@@ -315,116 +272,156 @@ struct LineState2 {
             for (int c = 3; c < NV; ++c) inc[c] = k[c];
             fc = shs;
             accL = fma(hs, bn, L);
-        } else {
-            // RK4 (reading A5): k2 = f(y + h/2 k1), k3 = f(y + h/2 k2), k4 = f(y + h k3), y+ = y + h/6 (k1 + 2 k2 + 2 k3 + k4)
-            const double half = 0.5 * shs;
-            double bnS = 0.0;          // |b| of the unscaled field vector (spherical geometry only)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
-            enter_cell(A, ys, d);
-#pragma unroll
-            for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
-            accL = bn;
-            // ---- stage 2
-            stage(d, ys, b, k);
-            if (SPH) bnS = to_rates(ys, b, k);
-            {
-                double xn[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
-                enter_cell(A, xn, d);
-                bn = SPH ? bnS : norm3_fast(b);
-#pragma unroll
-                for (int c = 0; c < NV; ++c) {
-                    const double kc = c < 3 ? b[c] : k[c];
-                    acc[c] = fma(2.0, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(half, kc, y[c]);
-                }
-                accL = fma(2.0, bn, accL);
-            }
-            // ---- stage 3
-            stage(d, ys, b, k);
-            if (SPH) bnS = to_rates(ys, b, k);
-            {
-                double xn[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
-                enter_cell(A, xn, d);
-                bn = SPH ? bnS : norm3_fast(b);
-#pragma unroll
-                for (int c = 0; c < NV; ++c) {
-                    const double kc = c < 3 ? b[c] : k[c];
-                    acc[c] = fma(2.0, kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(shs, kc, y[c]);
-                }
-                accL = fma(2.0, bn, accL);
-            }
-            // ---- stage 4
-            stage(d, ys, b, k);
-            if (SPH) bnS = to_rates(ys, b, k);
-            {
-                const double fL = hs * (1.0 / 6.0), f = back ? -fL : fL;
-#pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fma(f, fma(1.0, b[c], acc[c]), y[c]);
-                // the trial end is where the next attempt starts if it is accepted: enter its cell now
-                enter_cell(A, xn, d);
-                bn = SPH ? bnS : norm3_fast(b);
-#pragma unroll
-                for (int c = 3; c < NV; ++c) inc[c] = fma(1.0, k[c], acc[c]);
-                fc = f;
-                accL = fma(fL, fma(1.0, bn, accL), L);
-            }
+            enter_cell(A, xn, d);
+            return;
         }
-        // xn = trial end, accL = trial length
-        if (phase == 0) {
-            if (inside_box(A, xn)) {
-                if (SPH) move_anchor(xn[1] - y[1]);
+        // RK4 (reading A5): k2 = f(y + h/2 k1), k3 = f(y + h/2 k2), k4 = f(y + h k3), y+ = y + h/6 (k1 + 2 k2 + 2 k3 + k4)
+        const double half = 0.5 * shs;
+        double bnS = 0.0;          // |b| of the unscaled field vector (spherical geometry only)
 #pragma unroll
-                for (int c = 0; c < NV; ++c) y[c] = c < 3 ? xn[c] : fma(fc, inc[c], y[c]);
-                L = accL; lam += h; ++nsteps;
-                return false;
-            }
-            // first face crossed by the chord: smallest fraction, tie -> lowest axis (reading A4)
-            double phi = INFINITY; int ax = -1, face = 255; double bd = 0.0;
+        for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
+        enter_cell(A, ys, d);
 #pragma unroll
-            for (int dd = 0; dd < 3; ++dd) {
-                if (xn[dd] < A.box_lo[dd]) {
-                    const double f = (A.box_lo[dd] - y[dd]) / (xn[dd] - y[dd]);
-                    if (f < phi) { phi = f; ax = dd; face = 2 * dd; bd = A.box_lo[dd]; }
-                } else if (xn[dd] > A.box_hi[dd]) {
-                    const double f = (A.box_hi[dd] - y[dd]) / (xn[dd] - y[dd]);
-                    if (f < phi) { phi = f; ax = dd; face = 2 * dd + 1; bd = A.box_hi[dd]; }
-                }
+        for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
+        accL = bn;
+        // ---- stage 2
+        stage(d, ys, b, k);
+        if (SPH) bnS = to_rates(ys, b, k);
+        {
+            double xs[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xs[c] = fma(half, b[c], y[c]);
+            enter_cell(A, xs, d);
+            bn = SPH ? bnS : norm3_fast(b);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) {
+                const double kc = c < 3 ? b[c] : k[c];
+                acc[c] = fma(2.0, kc, acc[c]); ys[c] = c < 3 ? xs[c] : fma(half, kc, y[c]);
             }
-            if (ax < 0) { finish(A, 255, REC_STALL); return true; }   // non-finite trial point
-            const double yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
-            if (yd == bd) {
-                // the line starts on the face it leaves through (photospheric seeds): hp = 0, every Newton residual is
-                // exactly 0, so the landing of O4 ends where it started: one zero-length step
-                ++nsteps;
-                finish(A, face, 0);
-                return true;
+            accL = fma(2.0, bn, accL);
+        }
+        // ---- stage 3
+        stage(d, ys, b, k);
+        if (SPH) bnS = to_rates(ys, b, k);
+        {
+            double xs[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xs[c] = fma(shs, b[c], y[c]);
+            enter_cell(A, xs, d);
+            bn = SPH ? bnS : norm3_fast(b);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) {
+                const double kc = c < 3 ? b[c] : k[c];
+                acc[c] = fma(2.0, kc, acc[c]); ys[c] = c < 3 ? xs[c] : fma(shs, kc, y[c]);
             }
-            st[ST_HP * T] = phi * h; st[ST_BOUND * T] = bd; st[ST_HFULL * T] = h;
-            st[ST_AXIS_FACE * T] = __hiloint2double(ax, face);
-            phase = 1;
+            accL = fma(2.0, bn, accL);
+        }
+        // ---- stage 4
+        stage(d, ys, b, k);
+        if (SPH) bnS = to_rates(ys, b, k);
+        {
+            const double fL = hs * (1.0 / 6.0), f = back ? -fL : fL;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xn[c] = fma(f, fma(1.0, b[c], acc[c]), y[c]);
+            // the trial end is where the next attempt starts if it is accepted: enter its cell now
+            enter_cell(A, xn, d);
+            bn = SPH ? bnS : norm3_fast(b);
+#pragma unroll
+            for (int c = 3; c < NV; ++c) inc[c] = fma(1.0, k[c], acc[c]);
+            fc = f;
+            accL = fma(fL, fma(1.0, bn, accL), L);
+        }
+    }
+
+    // One attempt of the trace kernel proper: a trial step from y, committed if its end is inside the closed trace box.
+    // A line whose trial step leaves the box is written to its record as it stands, flagged REC_LANDING, and the lane is
+    // free for the next work item: the landing of reading A4 (chord + three Newton updates + snap: five more steps'
+    // worth of evaluations, a state machine of its own) is done for all lines at once by landing_kernel, where every
+    // lane is in the same phase, instead of by one lane of a warp here while the other 31 wait.
+    // Returns true when the line has left this kernel (landing pending, stall, cap).
+    __device__ __forceinline__ bool advance(const TraceArgs &A)
+    {
+        double b[3], k[NV], d[3], xn[3], inc[NV], fc, accL;
+        enter_cell(A, y, d);
+        stage(d, y, b, k);
+        const double bn = SPH ? to_rates(y, b, k) : norm3_fast(b);
+        // O4: stall / caps are tested on k1 before the step; h from the cell containing x
+        if (!(bn >= A.null_eps) || (long long)nsteps >= A.max_steps || lam >= A.max_length) {
+            finish(A, 255, !(bn >= A.null_eps) ? (nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL) : REC_CAP);
+            return true;
+        }
+        const double h = step_size(A);
+        trial(A, h, b, k, bn, xn, inc, fc, accL);
+        if (inside_box(A, xn)) {
+            if (SPH) move_anchor(xn[1] - y[1]);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) y[c] = c < 3 ? xn[c] : fma(fc, inc[c], y[c]);
+            L = accL; lam += h; ++nsteps;
             return false;
         }
-        if (phase < 4) {
-            st[(ST_XT + 0) * T] = xn[0]; st[(ST_XT + 1) * T] = xn[1]; st[(ST_XT + 2) * T] = xn[2];
-            ++phase;
-            return false;
+        finish(A, 255, REC_LANDING);
+        return true;
+    }
+
+    // The landing of one line (reading A4), from the state the trace kernel recorded: the trial step is taken again
+    // (same arithmetic, same end), the chord gives the first landing step hp, then
+    //    step(hp), Newton, step(hp), Newton, step(hp), Newton, step(hp) -> snap onto the face
+    // with k1 at y computed once.  Returns the number of steps added to the line (1, or 0 if the trial point is not finite).
+    __device__ unsigned land(const TraceArgs &A)
+    {
+        double b1[3], k1[NV], b[3], k[NV], d[3], xn[3], inc[NV], fc, accL;
+        enter_cell(A, y, d);
+        stage(d, y, b1, k1);
+        const double bn1 = SPH ? to_rates(y, b1, k1) : norm3_fast(b1);
+        const double h = step_size(A);
+#pragma unroll
+        for (int c = 0; c < NV; ++c) { if (c < 3) b[c] = b1[c]; else k[c] = k1[c]; }
+        trial(A, h, b, k, bn1, xn, inc, fc, accL);
+        // first face crossed by the chord: smallest fraction, tie -> lowest axis (reading A4)
+        double phi = INFINITY; int ax = -1, face = 255; double bound = 0.0;
+#pragma unroll
+        for (int dd = 0; dd < 3; ++dd) {
+            if (xn[dd] < A.box_lo[dd]) {
+                const double f = (A.box_lo[dd] - y[dd]) / (xn[dd] - y[dd]);
+                if (f < phi) { phi = f; ax = dd; face = 2 * dd; bound = A.box_lo[dd]; }
+            } else if (xn[dd] > A.box_hi[dd]) {
+                const double f = (A.box_hi[dd] - y[dd]) / (xn[dd] - y[dd]);
+                if (f < phi) { phi = f; ax = dd; face = 2 * dd + 1; bound = A.box_hi[dd]; }
+            }
         }
-        // phase 4: final landing step
-        const double af = st[ST_AXIS_FACE * T];
-        const int axis = __double2hiint(af), face = __double2loint(af);
-        const double bound = st[ST_BOUND * T];
+        if (ax < 0) { finish(A, 255, REC_STALL); return 0; }   // non-finite trial point
+        const double yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
+        if (yd == bound) {
+            // the line starts on the face it leaves through (photospheric seeds): hp = 0, every Newton residual is
+            // exactly 0, so the landing of O4 ends where it started: one zero-length step
+            ++nsteps;
+            finish(A, face, 0);
+            return 1;
+        }
+        double hp = phi * h;
+        for (int it = 0; it < 4; ++it) {
+#pragma unroll
+            for (int c = 0; c < NV; ++c) { if (c < 3) b[c] = b1[c]; else k[c] = k1[c]; }
+            trial(A, hp, b, k, bn1, xn, inc, fc, accL);
+            if (it == 3) break;
+            // Newton update of hp from the field at the trial end (clamped to [0, h]); the cell of xn is cached
+            d[0] = xn[0] - x0[0]; d[1] = xn[1] - x0[1]; d[2] = xn[2] - x0[2];
+            stage(d, y, b, k);
+            if (SPH) to_rates(xn, b, k);
+            const double bd = ax == 0 ? b[0] : (ax == 1 ? b[1] : b[2]);
+            const double xd = ax == 0 ? xn[0] : (ax == 1 ? xn[1] : xn[2]);
+            const double gg = back ? -bd : bd, r = xd - bound;
+            if (gg != 0.0) {
+                const double hn = hp - r / gg;
+                if (hn == hn) hp = fmin(fmax(hn, 0.0), h);
+            }
+        }
 #pragma unroll
         for (int c = 0; c < NV; ++c) y[c] = c < 3 ? xn[c] : fma(fc, inc[c], y[c]);
-        if (axis == 0) y[0] = bound; else if (axis == 1) y[1] = bound; else y[2] = bound;
-        L = accL; lam += st[ST_HP * T]; ++nsteps;
+        if (ax == 0) y[0] = bound; else if (ax == 1) y[1] = bound; else y[2] = bound;
+        L = accL; lam += hp; ++nsteps;
         finish(A, face, 0);
-        return true;
-#undef st
-#undef T
+        return 1;
     }
 };
 
@@ -475,6 +472,15 @@ __global__ void __launch_bounds__(128) seed_basis_kernel(const TraceArgs A, doub
 #ifndef QSL_T2_MIN_BLOCKS_L
 #define QSL_T2_MIN_BLOCKS_L 4
 #endif
+#ifndef QSL_T2_POOL
+#define QSL_T2_POOL 1
+#endif
+// The persistent kernel (REFILL): work items are taken from the global counter by the WARP, up to 32 consecutive items
+// of the Morton order at a time, and their seeds (and orthonormal pairs) are staged in shared memory by all 32 lanes at
+// once; a lane whose line has ended takes the next staged item with a few LDS instead of going through three dependent
+// global round trips (counter -> permutation -> seed) while the other 31 lanes of its warp wait (profiles/r2d: 5 % of
+// the issue cycles of cfg2).  The chunk shrinks with the work left (remaining / (4 x warps of the grid), at least the
+// number of lanes waiting), so that at the end of a launch no warp sits on staged items other warps could be running.
 template <bool DEV, bool STRETCHED, bool INTERP, bool REFILL, bool SPH = false>
 __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : QSL_T2_MIN_BLOCKS_L) trace2_kernel(const TraceArgs A)
 {
@@ -487,6 +493,69 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
             while (!ls.advance(A)) {}
         }
         if (q < n_items) my_steps = ls.nsteps;
+    } else if (QSL_T2_POOL) {
+        constexpr int NP = DEV ? 9 : 3;
+        __shared__ double pool_v[QSL_T2_THREADS / 32][NP][32];
+        __shared__ uint32_t pool_slot[QSL_T2_THREADS / 32][32];
+        const unsigned lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+        const long long n_warps = (long long)gridDim.x * (QSL_T2_THREADS / 32);
+        int pool_n = 0, pool_head = 0;              // warp-uniform
+        long long left = n_items;                   // work left in the queue when this warp last looked
+        bool have = false, drained = false;         // drained: warp-uniform
+        while (true) {
+            unsigned need = __ballot_sync(0xffffffffu, !have);
+            while (need) {
+                if (pool_n == 0) {
+                    if (drained) break;
+                    long long want = left / (4 * n_warps);
+                    want = max((long long)__popc(need), min(want, 32ll));
+                    unsigned long long base = 0;
+                    if (lane == 0) base = atomicAdd(A.queue, (unsigned long long)want);
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    left = n_items - (long long)base;
+                    const int got = left <= 0 ? 0 : (int)min(left, want);
+                    left -= got;
+                    if (got < (int)want) drained = true;
+                    if ((int)lane < got) {
+                        const long long q = (long long)base + lane;
+                        long long pos; int dir;
+                        if (A.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= A.n ? 1 : 0; pos = q - (long long)dir * A.n; }
+                        const uint32_t si = A.perm[pos];
+                        pool_slot[w][lane] = (uint32_t)((long long)dir * A.n + pos);
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) pool_v[w][c][lane] = A.seeds[3 * (size_t)si + c];
+                        if (DEV) {
+                            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(A.basis + 6 * (size_t)pos);
+                            const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
+                            pool_v[w][3 % NP][lane] = b0.x; pool_v[w][4 % NP][lane] = b0.y; pool_v[w][5 % NP][lane] = b1.x;
+                            pool_v[w][6 % NP][lane] = b1.y; pool_v[w][7 % NP][lane] = b2.x; pool_v[w][8 % NP][lane] = b2.y;
+                        }
+                    }
+                    __syncwarp();
+                    pool_n = got; pool_head = 0;
+                    if (got == 0) break;
+                }
+                const int rank = __popc(need & ((1u << lane) - 1u));
+                if (!have && rank < pool_n) {
+                    const int e = pool_head + rank;
+                    const double x[3] = { pool_v[w][0][e], pool_v[w][1][e], pool_v[w][2][e] };
+                    double bs[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
+                    if (DEV) {
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) bs[c] = pool_v[w][(3 + c) % NP][e];
+                    }
+                    have = ls.start(A, x, bs, pool_slot[w][e]);
+                }
+                const int served = min(pool_n, __popc(need));
+                pool_head += served; pool_n -= served;
+                __syncwarp();
+                need = __ballot_sync(0xffffffffu, !have);
+            }
+            if (!__any_sync(0xffffffffu, have)) break;
+            if (have) {
+                if (ls.advance(A)) { my_steps += ls.nsteps; have = false; }
+            }
+        }
     } else {
         const unsigned lane = threadIdx.x & 31u;
         bool have = false, drained = false;
@@ -511,6 +580,38 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) my_steps += __shfl_xor_sync(0xffffffffu, my_steps, o);
         if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(A.total_steps, my_steps);
+    }
+}
+
+// The landings of all lines of a launch (reading A4): one thread per per-direction record, in the Morton order of the
+// seeds; a record without REC_LANDING (stall, cap, seed outside) is left as it is.  Every lane runs the same five steps.
+template <bool DEV, bool STRETCHED, bool INTERP, bool SPH = false>
+__global__ void __launch_bounds__(128) landing_kernel(const TraceArgs A)
+{
+    const long long sl = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned added = 0;
+    if (sl < 2 * A.n) {
+        const double2 *__restrict__ r2 = reinterpret_cast<const double2 *>(A.rec + (size_t)sl * REC_DOUBLES);
+        const double2 w5 = r2[5];
+        if ((uint32_t)__double2hiint(w5.x) & REC_LANDING) {
+            LineState2<DEV, STRETCHED, INTERP, SPH> ls;
+            constexpr int NV = LineState2<DEV, STRETCHED, INTERP, SPH>::NV;
+            double v[10];
+#pragma unroll
+            for (int c = 0; c < 5; ++c) { const double2 t = r2[c]; v[2 * c] = t.x; v[2 * c + 1] = t.y; }
+#pragma unroll
+            for (int c = 0; c < NV; ++c) ls.y[c] = v[c];
+            ls.L = v[9]; ls.lam = w5.y; ls.nsteps = (uint32_t)__double2loint(w5.x);
+            ls.slot = (uint32_t)sl; ls.back = sl >= A.n; ls.phase = 0;
+            if (SPH) sincos(ls.y[1], &ls.sth, &ls.cth); else { ls.sth = 0.0; ls.cth = 1.0; }
+            ls.x0[0] = ls.x0[1] = ls.x0[2] = __longlong_as_double(0x7ff8000000000000ll);
+            ls.hc[0] = ls.hc[1] = ls.hc[2] = 0.0;
+            added = ls.land(A);
+        }
+    }
+    if (A.total_steps) {
+        const unsigned m = __ballot_sync(0xffffffffu, added != 0);
+        if ((threadIdx.x & 31) == 0 && m) atomicAdd(A.total_steps, (unsigned long long)__popc(m));
     }
 }
 
