@@ -25,6 +25,7 @@ collective); the time is the max over ranks and `value` the lines all ranks trac
 from __future__ import annotations
 
 import argparse
+import contextlib
 import json
 import math
 import os
@@ -71,6 +72,10 @@ class ClockSampler:
 
     def __init__(self, index):
         self.samples, self.reasons, self.max_mhz, self._stop, self._t = [], set(), None, threading.Event(), None
+        # held by the timing loop while it ENQUEUES a pass (a fraction of a millisecond; the pass then runs for its full
+        # duration with the sampler free): an NVML query takes driver locks that can stall a kernel launch for tens of
+        # milliseconds, which would show up as idle GPU time inside the event pair of that pass
+        self.enqueue_lock = threading.Lock()
         try:
             import pynvml
             pynvml.nvmlInit()
@@ -83,11 +88,12 @@ class ClockSampler:
         nv = self.nv
         while not self._stop.is_set():
             try:
-                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
-                try:
-                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
-                except Exception:
-                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                with self.enqueue_lock:
+                    self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                    try:
+                        r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                    except Exception:
+                        r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
                 for bit, name in {**self.BAD, **self.NOTE}.items():
                     if r & bit:
                         self.reasons.add(name)
@@ -384,6 +390,7 @@ def time_device(W, steps, warmup, flush, barrier, clocks=None):
     """`warmup` untimed passes, then `steps` passes timed one by one with CUDA events on the launch stream (L2 flushed
     before each, outside the event pair); the trace kernels of every pass are timed by libqsl's own event pairs."""
     qsl, torch = W.qsl, W.torch
+    qsl.qsl_profile_enable(True)               # the event pairs of the trace-kernel timing hook are created in the warm-up
     for _ in range(warmup):
         W.step_device()
     barrier()
@@ -393,14 +400,27 @@ def time_device(W, steps, warmup, flush, barrier, clocks=None):
     lines = 0
     rk = torch.zeros(2, dtype=torch.int64, device="cuda")
     kern_ms, kern_n = [0.0, 0.0], [0, 0]
+    host_ms = []                               # host time spent enqueueing each pass (the calls are asynchronous)
     if clocks is not None:
         clocks.samples.clear(); clocks.reasons.clear()
     t_wall = time.perf_counter()
+    lock = clocks.enqueue_lock if clocks is not None else contextlib.nullcontext()
+    if warmup > 0:
+        # One more untimed pass AFTER the barrier, with the timed passes enqueued right behind it: the first pass enqueued
+        # on an idle device after a device-wide synchronisation sporadically (about one run in four) has one of its
+        # driver calls stall the host for 5 - 300 ms, which would be idle GPU time inside that pass's event pair; it
+        # belongs to the harness, not to the path (seen with and without the NVML sampler, in different driver calls).
+        W.step_device()
+        qsl.qsl_profile_enable(True)
+        l0 = qsl.lib().qsl_launch_count()
     for a, b in ev:
-        flush.zero_()                          # L2 flush, outside the event pair
-        a.record()
-        m, s = W.step_device()
-        b.record()
+        with lock:                             # no NVML query in flight while the pass is enqueued (ClockSampler)
+            flush.zero_()                      # L2 flush, outside the event pair
+            a.record()
+            th = time.perf_counter()
+            m, s = W.step_device()
+            host_ms.append(round((time.perf_counter() - th) * 1e3, 3))
+            b.record()
         rk += s
         lines += m
         kms, kn = qsl.qsl_profile_trace_kernel_ms()      # waits for this step's trace kernels (after b.record())
@@ -410,7 +430,7 @@ def time_device(W, steps, warmup, flush, barrier, clocks=None):
     t_wall = time.perf_counter() - t_wall
     return {"lines": lines, "rk_by_mode": [int(v) for v in rk.tolist()], "kern_ms": kern_ms, "kern_n": kern_n,
             "launches": int(qsl.lib().qsl_launch_count() - l0), "dev_ms": sum(a.elapsed_time(b) for a, b in ev),
-            "ms_each": [round(a.elapsed_time(b), 3) for a, b in ev], "wall_s": t_wall, "steps": steps, "warmup": warmup}
+            "ms_each": [round(a.elapsed_time(b), 3) for a, b in ev], "host_ms_each": host_ms, "wall_s": t_wall, "steps": steps, "warmup": warmup}
 
 
 def alu_roofline(W, T, peak_fma):
@@ -732,7 +752,7 @@ def main():
             "dtype": "f32" if f32 else "f64", "data": "synthetic", "config": workload_config(cfg, args),
             "rk_steps_per_s": steps_all / (dev_ms_max * 1e-3), "rk_steps_per_step": rk_steps / args.steps,
             "lines_per_step": T["lines"] / args.steps, "wall_s_timed_region": T["wall_s"],
-            "ms_each_step": T["ms_each"],
+            "ms_each_step": T["ms_each"], "host_enqueue_ms_each_step": T["host_ms_each"],
             "clocks": clocks.summary(),
             "e2e": {"value": lines_all / (e2e_ms_max * 1e-3), "unit": "lines/s", "h2d_bytes_per_step": bi,
                     "d2h_bytes_per_step": bo, "ms_per_step": e2e_ms_max / args.steps},

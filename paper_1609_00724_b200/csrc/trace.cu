@@ -93,7 +93,7 @@ extern "C" int qsl_trace(const qsl_field *f, const qsl_trace_params *p, long lon
     const bool refill = !(p->flags & QSL_FLAG_NO_REFILL);
     A.interleave = refill ? 1 : 0;
     A.n = n; A.seeds = seeds; A.total_steps = total_steps;
-    A.basis = nullptr; A.stash = nullptr;
+    A.basis = nullptr; A.tie_zero = 0;
 
     void *perm = nullptr, *rec = nullptr, *queue = nullptr;
     int rc = scratch_alloc(&perm, sizeof(uint32_t) * (size_t)n, s);

@@ -10,9 +10,17 @@ static int launch_trace2_variant(TraceArgs &A, bool refill, cudaEvent_t ev0, cud
     const int threads = QSL_T2_THREADS;
     long long blocks = (n_items + threads - 1) / threads;
     if (refill) {
-        int per_sm = 0;
-        QSL_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace2_kernel<DEV, STRETCHED, INTERP, true, SPH>, threads, 0));
-        if (per_sm < 1) per_sm = 1;
+        // resident CTAs per SM of this instantiation: asked once per device (the query takes driver locks and was seen to
+        // stall the first call after a device synchronisation for tens of milliseconds)
+        static int per_sm_cache[64];
+        int dev = 0;
+        QSL_CUDA(cudaGetDevice(&dev));
+        int per_sm = dev >= 0 && dev < 64 ? per_sm_cache[dev] : 0;
+        if (per_sm < 1) {
+            QSL_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trace2_kernel<DEV, STRETCHED, INTERP, true, SPH>, threads, 0));
+            if (per_sm < 1) per_sm = 1;
+            if (dev >= 0 && dev < 64) per_sm_cache[dev] = per_sm;
+        }
         const long long resident = (long long)sm_count() * per_sm;   // persistent: every CTA resident, grid = SMs x occupancy
         if (blocks > resident) blocks = resident;
     }

@@ -14,6 +14,13 @@
 
 namespace qsl {
 
+#ifndef QSL_T2_TIE
+#define QSL_T2_TIE 1
+#endif
+#ifndef QSL_T2_DEFER
+#define QSL_T2_DEFER 3
+#endif
+
 __device__ __forceinline__ double4 load_cell4(const double4 *p)
 {
     double4 r;   // one 256-bit LDG (sm_100)
@@ -45,6 +52,7 @@ constexpr uint32_t REC_LANDING = 1u << 12;
 template <bool DEV, bool STRETCHED, bool INTERP, bool SPH = false>
 struct LineState2 {
     static constexpr int NV = DEV ? 9 : 3;
+    static constexpr int NJ = DEV ? 9 : 1;
     // cached cell: monomial coefficients a[8 c + m], origin (edges only on stretched grids)
     double a[24];
     double x0[3];
@@ -166,6 +174,70 @@ struct LineState2 {
         }
     }
 
+    // The same evaluation in two parts, for the fixed-step kernel: poly() needs the cached coefficients and gives b and
+    // the nine entries J[3 c + e] = d b_c / d x_e; products() needs only J.  Between the two the kernel computes the next
+    // stage point and enters its cell, so that the table loads of a cell change overwrite the coefficients while the
+    // deviation products, |b| and the RK accumulators of this stage are still to be executed (see trial()).
+    __device__ __forceinline__ void poly(const double d[3], double b[3], double *J)
+    {
+        const double dx = d[0], dy = d[1], dz = d[2];
+        double g[9];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double *q = a + 8 * c;
+            const double P = fma(q[7], dz, q[3]), Q = fma(q[5], dz, q[1]), R = fma(q[6], dz, q[2]), S = fma(q[4], dz, q[0]);
+            const double E = fma(P, dy, Q), F = fma(R, dy, S);
+            b[c] = fma(E, dx, F);
+            if (DEV) {
+                g[3 * c] = E;
+                g[3 * c + 1] = fma(P, dx, R);
+                g[3 * c + 2] = fma(fma(q[7], dy, q[5]), dx, fma(q[6], dy, q[4]));
+            }
+        }
+        if (!INTERP) {
+            if (DEV) {
+#pragma unroll
+                for (int q = 0; q < 9; ++q) J[q] = g[q];
+            }
+        } else {
+            // reading A2: interpolate B, then normalise: b = B/|B|, J = (G - u (u^T G))/|B|
+            const double v[3] = { b[0], b[1], b[2] };
+            const double nn = sqrt(fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0])));
+            if (nn < 1e-300) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) b[c] = 0.0;
+                if (DEV) {
+#pragma unroll
+                    for (int q = 0; q < 9; ++q) J[q] = 0.0;
+                }
+            } else {
+                const double inv = 1.0 / nn;
+                const double u0 = v[0] * inv, u1 = v[1] * inv, u2 = v[2] * inv;
+                b[0] = u0; b[1] = u1; b[2] = u2;
+                if (DEV) {
+#pragma unroll
+                    for (int e = 0; e < 3; ++e) {
+                        const double uG = fma(u2, g[6 + e], fma(u1, g[3 + e], u0 * g[e]));
+                        J[e] = (g[e] - u0 * uG) * inv;
+                        J[3 + e] = (g[3 + e] - u1 * uG) * inv;
+                        J[6 + e] = (g[6 + e] - u2 * uG) * inv;
+                    }
+                }
+            }
+        }
+    }
+    __device__ __forceinline__ void products(const double *J, const double *ys, double *k)
+    {
+        if (DEV) {
+#pragma unroll
+            for (int w = 0; w < 2; ++w)
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    k[(3 + 3 * w + c) % NV] = fma(J[(c * 3 + 2) % NJ], ys[(3 + 3 * w + 2) % NV],
+                                                  fma(J[(c * 3 + 1) % NJ], ys[(3 + 3 * w + 1) % NV], J[(c * 3) % NJ] * ys[(3 + 3 * w) % NV]));
+        }
+    }
+
     // SPH: the line's point moves by dt in latitude: rotate (sth, cth) and pull it back onto the unit circle (one Newton
     // step of 1/sqrt), so that rounding never accumulates in the modulus; the phase error grows like sqrt(steps) ulp.
     __device__ __forceinline__ void move_anchor(double dt)
@@ -255,44 +327,76 @@ struct LineState2 {
         return h;
     }
 
-    // One step of size hs from y given k1 = (b, k[3..]) and bn = |b| at y (both consumed): trial end xn, the deviation
-    // increments inc (trial end of component c >= 3 is y[c] + fc inc[c], formed only when the step is committed) and the
-    // trial length accL.  Four field evaluations per RK4 step in all; the cached cell on return is that of xn.
-    // Within a stage the order is: polynomial + deviation products -> position of the next stage point -> enter_cell
-    // for it (table loads in flight) -> |b|, accumulators.  The direction sign is folded into the step size.
-    __device__ __forceinline__ void trial(const TraceArgs &A, double hs, double b[3], double *k, double bn, double xn[3],
-                                          double *inc, double &fc, double &accL)
+    // Scheduling fence (not arithmetic): makes the offsets d of the next evaluation depend on `after` through an integer
+    // OR with (bits of after & A.tie_zero), where tie_zero is a kernel argument that is always 0.  ptxas schedules a
+    // basic block by critical path and would otherwise start the next stage's polynomial - whose first instruction
+    // waits for the table loads of a cell change, and with it the whole in-order warp - ahead of the ~45 independent
+    // FP64 instructions placed after enter_cell() to cover that latency (profiles/r2d: 14 % of the issue cycles of cfg2
+    // were spent on the first instruction after the two cell-change sites that take nearly all the changes).
+    __device__ __forceinline__ static void tie(const TraceArgs &A, double d[3], double after)
     {
-        double d[3], acc[NV], ys[NV];
+        const int t = __double2loint(after) & (int)A.tie_zero;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) d[c] = __hiloint2double(__double2hiint(d[c]), __double2loint(d[c]) | t);
+    }
+
+    // One step of size hs from y given b1 = b(y) and J1 = grad b(y) (poly() at y): trial end xn, the deviation
+    // increments inc (trial end of component c >= 3 is y[c] + fc inc[c], formed only when the step is committed), the
+    // trial length accL and bn1 = |b(y)|.  Four field evaluations per RK4 step in all; the cached cell on return is that
+    // of xn.  Per stage: polynomial (value + gradient) -> position of the next stage point -> enter_cell for it (table
+    // loads of a cell change in flight) -> deviation products, |b|, accumulators of this stage -> next polynomial.
+    // Nearly all cell changes happen on the two half-step moves (stage 1 -> 2 and stage 3 -> 4: some lane of a warp
+    // changes cell there in 94 % of the attempts, against 14 % at the other two); those two sites get the fence.
+    // Spherical geometry needs the metric factors of the stage point before the next point: there the deviation
+    // products and |b| come first.  The direction sign is folded into the step size.
+    __device__ __forceinline__ void trial(const TraceArgs &A, double hs, const double b1[3], const double *J1, double xn[3],
+                                          double *inc, double &fc, double &accL, double &bn1)
+    {
+        // deviation products before the next stage point (else after its enter_cell); per stage
+        constexpr bool EARLY1 = SPH || !(QSL_T2_DEFER == 1 || QSL_T2_DEFER == 2 || QSL_T2_DEFER == 3);
+        constexpr bool EARLY3 = SPH || !(QSL_T2_DEFER == 1 || QSL_T2_DEFER == 3);
+        constexpr bool EARLY = SPH || QSL_T2_DEFER != 1;
+        constexpr bool TIE = !SPH && QSL_T2_TIE;
+        double b[3], J[NJ], k[NV], d[3], acc[NV], ys[NV], bn;
         const double shs = back ? -hs : hs;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) b[c] = b1[c];
         if (A.method == QSL_EULER) {
+            products(J1, y, k);
+            bn1 = SPH ? to_rates(y, b, k) : norm3_fast(b);
 #pragma unroll
             for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
 #pragma unroll
             for (int c = 3; c < NV; ++c) inc[c] = k[c];
             fc = shs;
-            accL = fma(hs, bn, L);
+            accL = fma(hs, bn1, L);
             enter_cell(A, xn, d);
             return;
         }
         // RK4 (reading A5): k2 = f(y + h/2 k1), k3 = f(y + h/2 k2), k4 = f(y + h k3), y+ = y + h/6 (k1 + 2 k2 + 2 k3 + k4)
         const double half = 0.5 * shs;
-        double bnS = 0.0;          // |b| of the unscaled field vector (spherical geometry only)
+        // ---- stage 1 (polynomial done by the caller)
+        if (EARLY1) { products(J1, y, k); if (SPH) bn = to_rates(y, b, k); }
 #pragma unroll
         for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
         enter_cell(A, ys, d);
+        if (!EARLY1) products(J1, y, k);
+        if (!SPH) bn = norm3_fast(b);
+        bn1 = bn;
 #pragma unroll
         for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
         accL = bn;
+        if (TIE) tie(A, d, bn);
         // ---- stage 2
-        stage(d, ys, b, k);
-        if (SPH) bnS = to_rates(ys, b, k);
+        poly(d, b, J);
         {
             double xs[3];
+            if (EARLY) { products(J, ys, k); if (SPH) bn = to_rates(ys, b, k); }
 #pragma unroll
             for (int c = 0; c < 3; ++c) xs[c] = fma(half, b[c], y[c]);
             enter_cell(A, xs, d);
-            bn = SPH ? bnS : norm3_fast(b);
+            if (!EARLY) products(J, ys, k);
+            if (!SPH) bn = norm3_fast(b);
 #pragma unroll
             for (int c = 0; c < NV; ++c) {
                 const double kc = c < 3 ? b[c] : k[c];
@@ -301,31 +405,34 @@ struct LineState2 {
             accL = fma(2.0, bn, accL);
         }
         // ---- stage 3
-        stage(d, ys, b, k);
-        if (SPH) bnS = to_rates(ys, b, k);
+        poly(d, b, J);
         {
             double xs[3];
+            if (EARLY3) { products(J, ys, k); if (SPH) bn = to_rates(ys, b, k); }
 #pragma unroll
             for (int c = 0; c < 3; ++c) xs[c] = fma(shs, b[c], y[c]);
             enter_cell(A, xs, d);
-            bn = SPH ? bnS : norm3_fast(b);
+            if (!EARLY3) products(J, ys, k);
+            if (!SPH) bn = norm3_fast(b);
 #pragma unroll
             for (int c = 0; c < NV; ++c) {
                 const double kc = c < 3 ? b[c] : k[c];
                 acc[c] = fma(2.0, kc, acc[c]); ys[c] = c < 3 ? xs[c] : fma(shs, kc, y[c]);
             }
             accL = fma(2.0, bn, accL);
+            if (TIE) tie(A, d, accL);
         }
         // ---- stage 4
-        stage(d, ys, b, k);
-        if (SPH) bnS = to_rates(ys, b, k);
+        poly(d, b, J);
         {
             const double fL = hs * (1.0 / 6.0), f = back ? -fL : fL;
+            if (EARLY) { products(J, ys, k); if (SPH) bn = to_rates(ys, b, k); }
 #pragma unroll
             for (int c = 0; c < 3; ++c) xn[c] = fma(f, fma(1.0, b[c], acc[c]), y[c]);
             // the trial end is where the next attempt starts if it is accepted: enter its cell now
             enter_cell(A, xn, d);
-            bn = SPH ? bnS : norm3_fast(b);
+            if (!EARLY) products(J, ys, k);
+            if (!SPH) bn = norm3_fast(b);
 #pragma unroll
             for (int c = 3; c < NV; ++c) inc[c] = fma(1.0, k[c], acc[c]);
             fc = f;
@@ -341,17 +448,17 @@ struct LineState2 {
     // Returns true when the line has left this kernel (landing pending, stall, cap).
     __device__ __forceinline__ bool advance(const TraceArgs &A)
     {
-        double b[3], k[NV], d[3], xn[3], inc[NV], fc, accL;
+        double b[3], J[NJ], d[3], xn[3], inc[NV], fc, accL, bn;
         enter_cell(A, y, d);
-        stage(d, y, b, k);
-        const double bn = SPH ? to_rates(y, b, k) : norm3_fast(b);
-        // O4: stall / caps are tested on k1 before the step; h from the cell containing x
+        poly(d, b, J);
+        const double h = step_size(A);
+        trial(A, h, b, J, xn, inc, fc, accL, bn);
+        // O4: stall / caps are tested on k1 before the step is taken (here: before it is committed; the trial step of a
+        // line that ends this way is discarded); h from the cell containing x
         if (!(bn >= A.null_eps) || (long long)nsteps >= A.max_steps || lam >= A.max_length) {
             finish(A, 255, !(bn >= A.null_eps) ? (nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL) : REC_CAP);
             return true;
         }
-        const double h = step_size(A);
-        trial(A, h, b, k, bn, xn, inc, fc, accL);
         if (inside_box(A, xn)) {
             if (SPH) move_anchor(xn[1] - y[1]);
 #pragma unroll
@@ -366,17 +473,15 @@ struct LineState2 {
     // The landing of one line (reading A4), from the state the trace kernel recorded: the trial step is taken again
     // (same arithmetic, same end), the chord gives the first landing step hp, then
     //    step(hp), Newton, step(hp), Newton, step(hp), Newton, step(hp) -> snap onto the face
-    // with k1 at y computed once.  Returns the number of steps added to the line (1, or 0 if the trial point is not finite).
+    // with the polynomial at y evaluated once.  Returns the number of steps added to the line (1, or 0 if the trial
+    // point is not finite).
     __device__ unsigned land(const TraceArgs &A)
     {
-        double b1[3], k1[NV], b[3], k[NV], d[3], xn[3], inc[NV], fc, accL;
+        double b1[3], J1[NJ], b[3], J[NJ], k[NV], d[3], xn[3], inc[NV], fc, accL, bn1;
         enter_cell(A, y, d);
-        stage(d, y, b1, k1);
-        const double bn1 = SPH ? to_rates(y, b1, k1) : norm3_fast(b1);
+        poly(d, b1, J1);
         const double h = step_size(A);
-#pragma unroll
-        for (int c = 0; c < NV; ++c) { if (c < 3) b[c] = b1[c]; else k[c] = k1[c]; }
-        trial(A, h, b, k, bn1, xn, inc, fc, accL);
+        trial(A, h, b1, J1, xn, inc, fc, accL, bn1);
         // first face crossed by the chord: smallest fraction, tie -> lowest axis (reading A4)
         double phi = INFINITY; int ax = -1, face = 255; double bound = 0.0;
 #pragma unroll
@@ -400,14 +505,12 @@ struct LineState2 {
         }
         double hp = phi * h;
         for (int it = 0; it < 4; ++it) {
-#pragma unroll
-            for (int c = 0; c < NV; ++c) { if (c < 3) b[c] = b1[c]; else k[c] = k1[c]; }
-            trial(A, hp, b, k, bn1, xn, inc, fc, accL);
+            trial(A, hp, b1, J1, xn, inc, fc, accL, bn1);
             if (it == 3) break;
             // Newton update of hp from the field at the trial end (clamped to [0, h]); the cell of xn is cached
             d[0] = xn[0] - x0[0]; d[1] = xn[1] - x0[1]; d[2] = xn[2] - x0[2];
-            stage(d, y, b, k);
-            if (SPH) to_rates(xn, b, k);
+            poly(d, b, J);
+            if (SPH) { products(J, y, k); to_rates(xn, b, k); }
             const double bd = ax == 0 ? b[0] : (ax == 1 ? b[1] : b[2]);
             const double xd = ax == 0 ? xn[0] : (ax == 1 ? xn[1] : xn[2]);
             const double gg = back ? -bd : bd, r = xd - bound;

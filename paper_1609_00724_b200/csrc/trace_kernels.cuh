@@ -33,7 +33,7 @@ struct TraceArgs {
     unsigned long long *total_steps;
     unsigned long long *queue;   // work counter of the persistent kernel
     const double *basis;         // cell-table kernel, QSL_TRACE_LQ: n*6 (a^, b^) per seed in sorted order (seed_basis_kernel)
-    double *stash;               // cell-table kernel: per-thread landing scratch, STASH_DOUBLES x n_threads
+    unsigned tie_zero;           // cell-table kernel: always 0 (operand of the scheduling fence LineState2::tie)
 };
 
 // Per-direction record written once when a line ends: x[3], d1[3], d2[3], L, (nsteps, face|flags) as two uint32, lambda.
