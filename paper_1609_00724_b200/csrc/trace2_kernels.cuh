@@ -14,6 +14,12 @@
 
 namespace qsl {
 
+#ifndef QSL_T2_HEADTEST
+#define QSL_T2_HEADTEST 0
+#endif
+#ifndef QSL_T2_CHUNK
+#define QSL_T2_CHUNK 8
+#endif
 #ifndef QSL_T2_TIE
 #define QSL_T2_TIE 1
 #endif
@@ -266,6 +272,8 @@ struct LineState2 {
 
     // Starts a line at the seed x with the orthonormal pair bs (a^, b^; unused without DEV) for record slot sl.
     // Returns false if the item ended at once (seed outside the trace box).
+    // FIRST_CELL: the cell of the seed is cached on return (the fixed-step kernel's advance() relies on it)
+    template <bool FIRST_CELL = false>
     __device__ __forceinline__ bool start(const TraceArgs &A, const double x[3], const double *bs, uint32_t sl)
     {
         slot = sl;
@@ -277,6 +285,7 @@ struct LineState2 {
         if (!inside_box(A, x)) { finish(A, 255, REC_SEED_OUTSIDE); return false; }
         x0[0] = x0[1] = x0[2] = __longlong_as_double(0x7ff8000000000000ll);    // no cell cached yet
         hc[0] = hc[1] = hc[2] = 0.0;
+        if (FIRST_CELL) relocate(A, x);
         if (DEV && SPH) {   // orthonormal pair -> coordinate deviations (eq. 8 inverted)
             double mf[3];
             metric_shift(x[2], sth, cth, 0.0, mf);
@@ -289,6 +298,7 @@ struct LineState2 {
     // Starts work item q.  Returns false if the item ended at once (seed outside the trace box).  The orthonormal pair
     // a^, b^ of O2 comes from seed_basis_kernel (one thread per seed, all lanes busy) instead of being built here by
     // the one or two lanes of a warp that happen to be refilling; a null at the seed is caught by the first attempt.
+    template <bool FIRST_CELL = false>
     __device__ bool init(const TraceArgs &A, long long q)
     {
         long long pos; int dir;
@@ -301,7 +311,7 @@ struct LineState2 {
             const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
             bs[0] = b0.x; bs[1] = b0.y; bs[2] = b1.x; bs[3] = b1.y; bs[4] = b2.x; bs[5] = b2.y;
         }
-        return start(A, x, bs, (uint32_t)((long long)dir * A.n + pos));
+        return start<FIRST_CELL>(A, x, bs, (uint32_t)((long long)dir * A.n + pos));
     }
 
     __device__ void finish(const TraceArgs &A, int face, uint32_t flags)
@@ -449,7 +459,12 @@ struct LineState2 {
     __device__ __forceinline__ bool advance(const TraceArgs &A)
     {
         double b[3], J[NJ], d[3], xn[3], inc[NV], fc, accL, bn;
-        enter_cell(A, y, d);
+        if (QSL_T2_HEADTEST) enter_cell(A, y, d);
+        else {
+            // the cell of y is the cached one: entered by the last stage of the previous attempt (y = its trial end) or,
+            // for a line that has just started, by start_cell()
+            d[0] = y[0] - x0[0]; d[1] = y[1] - x0[1]; d[2] = y[2] - x0[2];
+        }
         poly(d, b, J);
         const double h = step_size(A);
         trial(A, h, b, J, xn, inc, fc, accL, bn);
@@ -592,7 +607,7 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
     unsigned long long my_steps = 0;
     if (!REFILL) {
         const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-        if (q < n_items && ls.init(A, q)) {
+        if (q < n_items && ls.template init<!QSL_T2_HEADTEST>(A, q)) {
             while (!ls.advance(A)) {}
         }
         if (q < n_items) my_steps = ls.nsteps;
@@ -611,7 +626,7 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
                 if (pool_n == 0) {
                     if (drained) break;
                     long long want = left / (4 * n_warps);
-                    want = max((long long)__popc(need), min(want, 32ll));
+                    want = max((long long)__popc(need), min(want, (long long)QSL_T2_CHUNK));
                     unsigned long long base = 0;
                     if (lane == 0) base = atomicAdd(A.queue, (unsigned long long)want);
                     base = __shfl_sync(0xffffffffu, base, 0);
@@ -647,7 +662,7 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
 #pragma unroll
                         for (int c = 0; c < 6; ++c) bs[c] = pool_v[w][(3 + c) % NP][e];
                     }
-                    have = ls.start(A, x, bs, pool_slot[w][e]);
+                    have = ls.template start<!QSL_T2_HEADTEST>(A, x, bs, pool_slot[w][e]);
                 }
                 const int served = min(pool_n, __popc(need));
                 pool_head += served; pool_n -= served;
@@ -671,7 +686,7 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
                 base = __shfl_sync(m, base, leader);
                 const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
                 if (q >= n_items) drained = true;
-                else have = ls.init(A, q);
+                else have = ls.template init<!QSL_T2_HEADTEST>(A, q);
             }
             if (__all_sync(0xffffffffu, drained && !have)) break;
             if (have) {
