@@ -48,7 +48,7 @@ FLOPS_PER_STEP = {"LQ": 800, "L": 400}
 # fp32 arithmetic) as a fraction of peak.  Keyed by (workload, arithmetic); absent -> null in the bench line.
 NCU_CAPTURES = {
     ("cfg2", "f64"): {"dram_bytes": 789848320, "pipe_active": 0.484, "source": "profiles/r1b_cell_table_kernel.md (capture e)"},
-    ("cfg4", "f64"): {"dram_bytes": 41683301000, "pipe_active": 0.517, "source": "profiles/r2a_cfg4_trace_kernel.md"},
+    ("cfg4", "f64"): {"dram_bytes": 46995332000, "pipe_active": 0.643, "source": "profiles/r2d_cfg4_trace_kernel.md"},
     ("cfg5", "f64"): {"dram_bytes": 344820435000, "pipe_active": 0.443,
                       "source": "profiles/r2a_cfg5_level0_trace_kernel.md (the level-0 L-only launch, 9 % of the step)"},
 }
