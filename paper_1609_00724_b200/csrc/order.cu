@@ -3,9 +3,9 @@
 // the field cell they start in, so that the lanes of a warp gather from neighbouring cells.  The order never changes a
 // result: outputs are scattered back to the caller's order.
 //
-// The sort is a hand-written stable LSD radix sort on 32-bit keys (8-bit digits): per pass a per-warp-chunk digit
-// histogram, one exclusive scan of the (digit-major) count table, and a scatter in which every warp ranks its 32 keys
-// with __match_any_sync and keeps its running digit offsets in shared memory.
+// The sort is a hand-written stable LSD radix sort on 32- or 64-bit keys (8-bit digits): per pass a per-tile digit
+// histogram, one exclusive scan of the (digit-major) count table, and a scatter that sorts a tile of 4096 (64-bit keys: 2048) keys by the
+// digit in shared memory (warps rank their keys with __match_any_sync) and writes it out run by run.
 #include "qsl_internal.cuh"
 #include "scan.cuh"
 
@@ -13,7 +13,7 @@ namespace qsl {
 
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_CHUNK = 2048;                      // keys per warp per pass
+template <typename K> struct SortTile { static constexpr int value = sizeof(K) == 8 ? 2048 : 4096; };   // keys per block per pass (static shared memory <= 48 KB)
 
 __device__ __forceinline__ uint32_t spread3(uint32_t v)   // 10 bits -> every third bit
 {
@@ -58,51 +58,98 @@ __global__ void __launch_bounds__(256) iota_kernel(long long n, uint32_t *perm)
     if (i < n) perm[i] = (uint32_t)i;
 }
 
-// counts[digit * n_chunks + chunk] = number of keys of `chunk` whose current digit is `digit`
+// counts[digit * n_tiles + tile] = number of keys of `tile` whose current digit is `digit`.  One block per tile of
+// SORT_TILE keys; per-warp histograms in shared memory (no cross-warp atomics), summed at the end.
 template <typename K>
 __global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(long long n, const K *__restrict__ keys, int shift,
-                                                                 long long n_chunks, uint32_t *__restrict__ counts)
+                                                                 long long n_tiles, uint32_t *__restrict__ counts)
 {
+    constexpr int SORT_TILE = SortTile<K>::value;
     __shared__ uint32_t h[SORT_WARPS][256];
     const unsigned lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
     for (int b = lane; b < 256; b += 32) h[w][b] = 0;
     __syncwarp();
-    const long long chunk = (long long)blockIdx.x * SORT_WARPS + w;
-    if (chunk < n_chunks) {
-        const long long lo = chunk * SORT_CHUNK, hi = min(lo + SORT_CHUNK, n);
-        for (long long i = lo + lane; i < hi; i += 32) atomicAdd(&h[w][(uint32_t)(keys[i] >> shift) & 255u], 1u);
-        __syncwarp();
-        for (int b = lane; b < 256; b += 32) counts[(long long)b * n_chunks + chunk] = h[w][b];
-    }
+    const long long tile = blockIdx.x;
+    const long long lo = tile * SORT_TILE + (long long)w * (SORT_TILE / SORT_WARPS), hi = min(lo + SORT_TILE / SORT_WARPS, n);
+    for (long long i = lo + lane; i < hi; i += 32) atomicAdd(&h[w][(uint32_t)(keys[i] >> shift) & 255u], 1u);
+    __syncthreads();
+    uint32_t c = 0;
+#pragma unroll
+    for (int q = 0; q < SORT_WARPS; ++q) c += h[q][threadIdx.x];
+    counts[(long long)threadIdx.x * n_tiles + tile] = c;
 }
 
+// Scatter of one pass.  A block owns a tile of SORT_TILE consecutive keys (warp w the w-th eighth of it, 32 keys per
+// round, so that index order = (warp, round, lane) order and the ranking below is stable):
+//   1. every warp ranks its keys among the keys of the same digit it has seen so far (__match_any_sync per round + a
+//      running per-warp digit counter in shared memory);
+//   2. thread d adds up the eight warp counters of digit d (-> the warps' bases inside the digit) and a block-wide
+//      exclusive scan of the digit totals gives the place of digit d inside the tile;
+//   3. keys and values are written to shared memory at their place in the tile sorted by digit;
+//   4. the tile is written out in that order: entry e of digit d goes to offsets[d][tile] + (e - start of d in the
+//      tile), so neighbouring threads store to neighbouring addresses within a digit's run (16 keys on average for
+//      uniformly distributed digits, whole rows for the nearly sorted keys of a seed lattice) instead of 32 unrelated
+//      sectors per store instruction.
 template <typename K>
 __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(long long n, const K *__restrict__ keys,
-                                                                    const uint32_t *__restrict__ vals, int shift, long long n_chunks,
+                                                                    const uint32_t *__restrict__ vals, int shift, long long n_tiles,
                                                                     const unsigned long long *__restrict__ offsets,
                                                                     K *__restrict__ keys_out, uint32_t *__restrict__ vals_out)
 {
-    __shared__ unsigned long long base[SORT_WARPS][256];
+    constexpr int SORT_TILE = SortTile<K>::value;
+    constexpr int ROUNDS = SORT_TILE / SORT_THREADS;        // 32-key rounds per warp
+    __shared__ K s_key[SORT_TILE];
+    __shared__ uint32_t s_val[SORT_TILE];
+    __shared__ uint32_t cnt[SORT_WARPS][256];               // running digit counters, then the warps' bases inside a digit
+    __shared__ uint32_t d_start[256];                       // place of a digit inside the tile
+    __shared__ unsigned long long g_base[256];              // where the tile's keys of a digit go in the output
     const unsigned lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-    const long long chunk = (long long)blockIdx.x * SORT_WARPS + w;
-    if (chunk >= n_chunks) return;
-    for (int b = lane; b < 256; b += 32) base[w][b] = offsets[(long long)b * n_chunks + chunk];
+    const long long tile = blockIdx.x;
+    for (int b = lane; b < 256; b += 32) cnt[w][b] = 0;
+    g_base[threadIdx.x] = offsets[(long long)threadIdx.x * n_tiles + tile];
     __syncwarp();
-    const long long lo = chunk * SORT_CHUNK, hi = min(lo + SORT_CHUNK, n);
-    for (long long i0 = lo; i0 < hi; i0 += 32) {
-        const long long i = i0 + lane;
-        const bool live = i < hi;
-        const K k = live ? keys[i] : (K)0;
-        const uint32_t v = live ? vals[i] : 0u;
-        const uint32_t digit = live ? ((uint32_t)(k >> shift) & 255u) : 256u + lane;   // dead lanes match nobody
+    const long long lo = tile * SORT_TILE + (long long)w * (SORT_TILE / SORT_WARPS);
+    const long long tile_n = min((long long)SORT_TILE, n - tile * SORT_TILE);
+    K k[ROUNDS]; uint32_t v[ROUNDS]; uint32_t dr[ROUNDS];   // dr = digit | rank inside (warp, digit) << 8
+#pragma unroll
+    for (int r = 0; r < ROUNDS; ++r) {
+        const long long i = lo + r * 32 + lane;
+        const bool live = i < n;
+        k[r] = live ? keys[i] : (K)0;
+        v[r] = live ? vals[i] : 0u;
+        const uint32_t digit = live ? ((uint32_t)(k[r] >> shift) & 255u) : 256u + lane;   // dead lanes match nobody
         const unsigned peers = __match_any_sync(0xffffffffu, digit);
         const unsigned rank = __popc(peers & ((1u << lane) - 1u));
-        unsigned long long dst = 0;
-        if (live) dst = base[w][digit] + rank;                                    // stable: lanes in key order
+        uint32_t before = 0;
+        if (live) before = cnt[w][digit];
         __syncwarp();
-        if (live && rank == 0) base[w][digit] += __popc(peers);                   // one writer per digit
+        if (live && rank == 0) cnt[w][digit] = before + __popc(peers);                    // one writer per digit
         __syncwarp();
-        if (live) { keys_out[dst] = k; vals_out[dst] = v; }
+        dr[r] = live ? (digit | ((before + rank) << 8)) : 0xffffffffu;
+    }
+    __syncthreads();
+    {
+        // digit d = threadIdx.x: exclusive prefix over the warps, total -> exclusive scan over the digits
+        uint32_t run = 0;
+#pragma unroll
+        for (int q = 0; q < SORT_WARPS; ++q) { const uint32_t c = cnt[q][threadIdx.x]; cnt[q][threadIdx.x] = run; run += c; }
+        unsigned long long total;
+        d_start[threadIdx.x] = (uint32_t)block_exclusive_scan((unsigned long long)run, total);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < ROUNDS; ++r) {
+        if (dr[r] != 0xffffffffu) {
+            const uint32_t digit = dr[r] & 255u, e = d_start[digit] + cnt[w][digit] + (dr[r] >> 8);
+            s_key[e] = k[r]; s_val[e] = v[r];
+        }
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < tile_n; e += SORT_THREADS) {
+        const K kk = s_key[e];
+        const uint32_t digit = (uint32_t)(kk >> shift) & 255u;
+        const unsigned long long dst = g_base[digit] + (unsigned)(e - d_start[digit]);
+        keys_out[dst] = kk; vals_out[dst] = s_val[e];
     }
 }
 
@@ -113,7 +160,7 @@ static int radix_sort_pairs_t(K *keys, uint32_t *vals, K *keys_tmp, uint32_t *va
     // sorts in place: an even number of passes ping-pongs back into keys / vals, an odd number ends with two copies
     // (cheaper than a whole extra pass over zero digits)
     const int passes = (key_bits + 7) / 8;
-    const long long n_chunks = (n + SORT_CHUNK - 1) / SORT_CHUNK;
+    const long long n_chunks = (n + SortTile<K>::value - 1) / SortTile<K>::value;   // one block per tile
     const long long table = 256 * n_chunks;
     void *counts = nullptr, *offsets = nullptr, *tiles = nullptr, *total = nullptr;
     int rc = scratch_alloc(&counts, sizeof(uint32_t) * (size_t)table, s);
@@ -122,7 +169,7 @@ static int radix_sort_pairs_t(K *keys, uint32_t *vals, K *keys_tmp, uint32_t *va
     if (rc == QSL_OK) rc = scratch_alloc(&total, sizeof(unsigned long long), s);
     cudaError_t e = cudaSuccess;
     if (rc == QSL_OK) {
-        const unsigned blocks = (unsigned)((n_chunks + SORT_WARPS - 1) / SORT_WARPS);
+        const unsigned blocks = (unsigned)n_chunks;
         K *ki = keys, *ko = keys_tmp;
         uint32_t *vi = vals, *vo = vals_tmp;
         for (int p = 0; p < passes && e == cudaSuccess; ++p) {
