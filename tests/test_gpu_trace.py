@@ -176,3 +176,19 @@ def test_trace_host_pipelined_equals_one_call(chunks):
         assert h[k].is_pinned() and torch.equal(h[k], g[k].cpu()), k
     assert qsl.trace_host(fg, seeds_host[:0], p, outputs=("L",)) == {}
     fg.destroy()
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 7, 8, 9, 31, 32, 33, 257])
+@pytest.mark.parametrize("mode", [qsl.QSL_TRACE_L, qsl.QSL_TRACE_LQ])
+def test_small_launches_staging_and_landing_kernel(n, mode):
+    """Launch sizes around the staging chunk (8 items per counter pop) and the warp size: every line is traced once and
+    landed once (records written by the trace kernel and rewritten by the landing kernel), and total_steps is the sum
+    of the per-line step counts of both kernels."""
+    cfg = qi.make_config("cfg3", scale=0.25)
+    rng = np.random.default_rng(1000 + n)
+    seeds = cfg["seeds"][rng.choice(len(cfg["seeds"]), n, replace=False)]
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, cfg["box_lo"], cfg["box_hi"], mode=mode, max_steps=cfg["max_steps"])
+    compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], with_q=mode == qsl.QSL_TRACE_LQ, frac=1.0, label="small n=%d" % n)
+    assert np.array_equal(g["status"], c["status"])
+    assert g["total_steps"] == int(g["nsteps_f"].astype(np.int64).sum() + g["nsteps_b"].astype(np.int64).sum())
+    assert g["total_steps"] == int(c["nsteps_f"].astype(np.int64).sum() + c["nsteps_b"].astype(np.int64).sum())
