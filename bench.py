@@ -47,10 +47,10 @@ FLOPS_PER_STEP = {"LQ": 800, "L": 400}
 # dram__bytes_read.sum + dram__bytes_write.sum, pipe_active = sm__pipe_fp64_cycles_active (sm__pipe_fma_cycles_active for
 # fp32 arithmetic) as a fraction of peak.  Keyed by (workload, arithmetic); absent -> null in the bench line.
 NCU_CAPTURES = {
-    ("cfg2", "f64"): {"dram_bytes": 789848320, "pipe_active": 0.484, "source": "profiles/r1b_cell_table_kernel.md (capture e)"},
+    ("cfg2", "f64"): {"dram_bytes": 786209280, "pipe_active": 0.620, "source": "profiles/r2d_cfg4_trace_kernel.md (cfg2 capture)"},
     ("cfg4", "f64"): {"dram_bytes": 46995332000, "pipe_active": 0.643, "source": "profiles/r2d_cfg4_trace_kernel.md"},
-    ("cfg5", "f64"): {"dram_bytes": 344820435000, "pipe_active": 0.443,
-                      "source": "profiles/r2a_cfg5_level0_trace_kernel.md (the level-0 L-only launch, 9 % of the step)"},
+    ("cfg5", "f64"): {"dram_bytes": 626591608000, "pipe_active": 0.525,
+                      "source": "profiles/r2d_cfg4_trace_kernel.md (cfg5 level 0, the L-only launch)"},
 }
 DEFAULT_WORKLOAD = "cfg4"
 SELECT_PASSES = 8          # radix passes of qsl_select (select_refine.cu), for the streaming byte count
