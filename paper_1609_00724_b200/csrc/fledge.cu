@@ -108,11 +108,19 @@ __global__ void __launch_bounds__(FL_THREADS) fledge_dense_kernel(long long d0, 
 // Dense 3-D map, each value loaded once (+ halo): a warp owns a strip of FL_VALID columns x a band of FL3_ROWS rows and
 // marches along axis 2 over a chunk of FL3_PLANES planes, holding the raw values of its column for the rows of the band
 // (+ one halo row on either side) of the planes z-1, z, z+1 in registers.  Per plane step: FL3_ROWS + 2 loads per lane
-// for FL3_ROWS outputs (1.25 loads per output x 32 / 30 lanes) instead of 3.  The folds are taken in the order of the
+// for FL3_ROWS outputs instead of 3 per output.  Measured on a 512 x 512 x 256 map: 8 rows (168 registers) 0.48 ms,
+// 4 rows at 5 CTAs / SM 0.46 ms, 2 rows at 8 CTAs / SM (64 registers) 0.40 ms, the row-marching kernel 0.45 ms: the
+// kernel wants resident warps more than it wants fewer loads (the repeated loads hit L2).  The folds are taken in the order of the
 // kernel above (axis 2, then axis 1, then axis 0 across lanes), so both give the same bits.
-constexpr int FL3_ROWS = 8;
+#ifndef QSL_FL3_ROWS
+#define QSL_FL3_ROWS 2
+#endif
+#ifndef QSL_FL3_MINB
+#define QSL_FL3_MINB 8
+#endif
+constexpr int FL3_ROWS = QSL_FL3_ROWS;
 constexpr int FL3_PLANES = 64;
-__global__ void __launch_bounds__(FL_THREADS) fledge_dense3_kernel(long long d0, long long d1, long long d2,
+__global__ void __launch_bounds__(FL_THREADS, QSL_FL3_MINB) fledge_dense3_kernel(long long d0, long long d1, long long d2,
                                                                    const double *__restrict__ L, double *__restrict__ S)
 {
     constexpr int R = FL3_ROWS;
