@@ -49,10 +49,6 @@ __device__ __forceinline__ double norm3_fast(const double v[3])
     return fma(fma(-s1, s1, n2), h1, s1);
 }
 
-// Record flag of the cell-table kernel: the trial step from the recorded state leaves the trace box, the landing of
-// reading A4 is still to be done (landing_kernel clears it).  Bits 8..11 are the REC_* status flags of trace_kernels.cuh.
-constexpr uint32_t REC_LANDING = 1u << 12;
-
 // SPH: spherical geometry (reading A19): the coordinate rates are the orthonormal components times the metric factors
 // (1/(r cos theta), 1/r, 1) of the evaluation point; |b| for L and the stall test is taken before the scaling.
 template <bool DEV, bool STRETCHED, bool INTERP, bool SPH = false>

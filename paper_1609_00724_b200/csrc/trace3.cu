@@ -19,12 +19,11 @@ static int launch_trace3_variant(Trace3Args<T> &A, bool refill, cudaEvent_t ev0,
         const long long resident = (long long)sm_count() * per_sm;   // persistent: grid = SMs x resident CTAs
         if (blocks > resident) blocks = resident;
     }
-    void *basis = nullptr, *stash = nullptr;
-    int rc = scratch_alloc(&stash, sizeof(T) * STASH3_SLOTS * (size_t)blocks * threads, s);
-    if (rc == QSL_OK && DEV) rc = scratch_alloc(&basis, sizeof(double) * 6 * (size_t)A.T0.n, s);
+    void *basis = nullptr;
+    int rc = QSL_OK;
+    if (DEV) rc = scratch_alloc(&basis, sizeof(double) * 6 * (size_t)A.T0.n, s);
     cudaError_t e = cudaSuccess;
     if (rc == QSL_OK) {
-        A.stash = (T *)stash;
         if (DEV) {
             count_launch();
             seed_basis3_kernel<S, INTERP><<<(unsigned)((A.T0.n + 127) / 128), 128, 0, s>>>(A.T0, (double *)basis);
@@ -38,10 +37,16 @@ static int launch_trace3_variant(Trace3Args<T> &A, bool refill, cudaEvent_t ev0,
             else trace3_kernel<T, DEV, INTERP, false, SPH><<<(unsigned)blocks, threads, 0, s>>>(A);
             e = cudaGetLastError();
         }
+        if (e == cudaSuccess) {
+            // the landings (reading A4) of all lines at once; part of the trace time
+            count_launch();
+            landing3_kernel<T, DEV, INTERP, SPH><<<(unsigned)((n_items + 127) / 128), 128, 0, s>>>(A);
+            e = cudaGetLastError();
+        }
         if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, s);
         if (e != cudaSuccess) rc = record_cuda(e);
     }
-    scratch_free(basis, s); scratch_free(stash, s);
+    scratch_free(basis, s);
     return rc;
 }
 
@@ -82,7 +87,6 @@ static int launch_trace3_t(const TraceArgs &G, const void *cells, bool dev, bool
     A.cell_sy = dims[0] - 1;
     A.cell_sz = (dims[0] - 1) * (dims[1] - 1);
     A.null_eps = (T)G.null_eps;
-    A.stash = nullptr;
     A.row_sc = G.fv.row_sc;
     A.step_frac = (T)G.step_frac;
     const bool in = G.fv.interp_mode == QSL_INTERP_FIRST;

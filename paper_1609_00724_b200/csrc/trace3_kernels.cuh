@@ -59,14 +59,12 @@ struct Trace3Args {
     unsigned cw[3];              // max(ch - cl - 1, 0): number of cells strictly between them
     T off_lo[3], off_hi[3];      // offsets of box_lo / box_hi from the origins of cells cl / ch
     T null_eps;
-    T *stash;                    // per-thread landing scratch, STASH3_SLOTS x n_threads
     // spherical geometry (reading A19; SPH instantiations): (sin, cos) of the latitude of every row of cells (fp64
     // sincos rounded to fp32, built by qsl_field_create), and the step fraction (the step is sized per attempt)
     const float2 *row_sc;
     T step_frac;
 };
 
-enum { S3_K1 = 0, S3_BN = 9, S3_DXT = 10, S3_HP = 13, S3_HFULL = 14, S3_AXIS_FACE = 15, STASH3_SLOTS = 16 };
 
 // |v|, branch-free: hardware reciprocal square root of max(|v|^2, tiny) and one coupled Newton step (relative error
 // ~1e-7 in fp32, ~1e-13 in fp64).  |v|^2 = 0 gives exactly 0; NaN and overflow propagate (and then stop the line through
@@ -213,17 +211,14 @@ struct LineState3 {
         }
     }
 
-    // Starts work item q (false if it ended at once: seed outside the trace box).  The seed's cell is found once, in
-    // fp64, exactly as O1 does (floor of (x - lo)/h, clamped); the basis a^, b^ of O2 comes from seed_basis3_kernel.
-    __device__ bool init(const Args &A, long long q)
+    // Starts a line at the seed x with the orthonormal pair bs (a^, b^ of O2, from seed_basis3_kernel; unused without
+    // DEV) for record slot sl (false if it ended at once: seed outside the trace box).  The seed's cell is found once,
+    // in fp64, exactly as O1 does (floor of (x - lo)/h, clamped).
+    __device__ __forceinline__ bool start(const Args &A, const double x[3], const double *bs, uint32_t sl)
     {
         const TraceArgs &G = A.T0;
-        long long pos; int dir;
-        if (G.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= G.n ? 1 : 0; pos = q - (long long)dir * G.n; }
-        slot = (uint32_t)((long long)dir * G.n + pos);
-        back = dir != 0;
-        const uint32_t si = G.perm[pos];
-        const double x[3] = { G.seeds[3 * (size_t)si], G.seeds[3 * (size_t)si + 1], G.seeds[3 * (size_t)si + 2] };
+        slot = sl;
+        back = (long long)sl >= G.n;
         L = 0.0; lam = 0.0; nsteps = 0; phase = 0;
         if (!inside_box(G, x)) {
             double out[REC_DOUBLES];
@@ -235,22 +230,9 @@ struct LineState3 {
             for (int c = 0; c < REC_DOUBLES / 2; ++c) r2[c] = make_double2(out[2 * c], out[2 * c + 1]);
             return false;
         }
+        frame_of(A, x);
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            const double u = (x[d] - G.fv.lo[d]) * G.inv_h[d];
-            int i = (int)floor(u);
-            i = max(0, min(i, A.cmax[d]));
-            C[d] = i;
-            y[d] = (T)(x[d] - fma((double)i, G.fv.h[d], G.fv.lo[d]));
-        }
-#pragma unroll
-        for (int c = 3; c < NV; ++c) y[c] = T(0.);
-        if (DEV) {
-            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(G.basis + 6 * (size_t)pos);
-            const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
-            y[3 % NV] = (T)b0.x; y[4 % NV] = (T)b0.y; y[5 % NV] = (T)b1.x;
-            y[6 % NV] = (T)b1.y; y[7 % NV] = (T)b2.x; y[8 % NV] = (T)b2.y;
-        }
+        for (int c = 3; c < NV; ++c) y[c] = (T)bs[(c - 3) % 6];
         load_cell(A);
         if (SPH && DEV) {     // orthonormal pair -> coordinate deviations (eq. 8 inverted)
             T rcos, r;
@@ -259,6 +241,37 @@ struct LineState3 {
             y[3 % NV] *= m0; y[4 % NV] *= m1; y[6 % NV] *= m0; y[7 % NV] *= m1;
         }
         return true;
+    }
+
+    // Frame (cell index C, offsets y[0..2]) of the absolute point x
+    __device__ __forceinline__ void frame_of(const Args &A, const double x[3])
+    {
+        const TraceArgs &G = A.T0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const double u = (x[d] - G.fv.lo[d]) * G.inv_h[d];
+            int i = (int)floor(u);
+            i = max(0, min(i, A.cmax[d]));
+            C[d] = i;
+            y[d] = (T)(x[d] - fma((double)i, G.fv.h[d], G.fv.lo[d]));
+        }
+    }
+
+    // Starts work item q of the queue
+    __device__ bool init(const Args &A, long long q)
+    {
+        const TraceArgs &G = A.T0;
+        long long pos; int dir;
+        if (G.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= G.n ? 1 : 0; pos = q - (long long)dir * G.n; }
+        const uint32_t si = G.perm[pos];
+        const double x[3] = { G.seeds[3 * (size_t)si], G.seeds[3 * (size_t)si + 1], G.seeds[3 * (size_t)si + 2] };
+        double bs[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
+        if (DEV) {
+            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(G.basis + 6 * (size_t)pos);
+            const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
+            bs[0] = b0.x; bs[1] = b0.y; bs[2] = b1.x; bs[3] = b1.y; bs[4] = b2.x; bs[5] = b2.y;
+        }
+        return start(A, x, bs, (uint32_t)((long long)dir * G.n + pos));
     }
 
     // Writes the per-direction record in fp64: position = origin of the frame cell + offset; `snap` >= 0 puts the
@@ -311,172 +324,196 @@ struct LineState3 {
         return in;
     }
 
-    // One attempt = exactly four field evaluations for every lane, whatever its phase (the state machine of
-    // LineState2::advance, reading A4): phase 0 trial step; phase 1 first landing step of size hp (k1 and the trial end,
-    // as a displacement from y so that it survives a change of frame, go to the stash); phases 2..4 spend the first
-    // evaluation at the previous trial end for one Newton update of hp; phase 4 lands.
-    __device__ bool advance(const Args &A)
+    // Scheduling fence (LineState2::tie): the offsets of the next evaluation are made to depend on `after` through an
+    // integer OR with (bits & tie_zero), tie_zero a kernel argument that is always 0, so that ptxas keeps the independent
+    // work placed after enter_cell() between the table loads of a cell change and their first use.
+    __device__ __forceinline__ static void tie(const Args &A, T d[3], T after)
     {
-#define st (A.stash + ((size_t)blockIdx.x * blockDim.x + threadIdx.x))
-#define TT ((size_t)gridDim.x * blockDim.x)
-        const TraceArgs &G = A.T0;
-        T b[3], k[NV], bn, hs, h = T(0.);
-        T acc[NV], accL, ys[NV];
-        {
-            T p0[3] = { y[0], y[1], y[2] };
-            if (phase >= 2) { p0[0] += st[(S3_DXT + 0) * TT]; p0[1] += st[(S3_DXT + 1) * TT]; p0[2] += st[(S3_DXT + 2) * TT]; }
-            enter_cell(A, p0);
-            stage(p0, y, b, k);
-            bn = to_rates(p0, b, k);
-            if (phase == 0) {
-                if (!(bn >= A.null_eps)) { finish(A, 255, nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL, -1); return true; }
-                if ((long long)nsteps >= G.max_steps || lam >= G.max_length) { finish(A, 255, REC_CAP, -1); return true; }
-                h = A.h_step;
-                if (SPH) {   // physical cell edges (r cos(theta) h_phi, r h_theta, h_r) at the start of the step
-                    T rcos, r;
-                    polar(y, rcos, r);
-                    h = A.step_frac * fmin(rcos * A.hf[0], fmin(r * A.hf[1], A.hf[2]));
-                }
-                if (lam + (double)h > G.max_length) h = (T)(G.max_length - lam);
-                hs = h;
-            } else {
-                T hp = st[S3_HP * TT];
-                if (phase == 1) {
+        if (sizeof(T) == 4) {
+            const int t = __float_as_int((float)after) & (int)A.T0.tie_zero;
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) st[(S3_K1 + c) * TT] = b[c];
+            for (int c = 0; c < 3; ++c) d[c] = (T)__int_as_float(__float_as_int((float)d[c]) | t);
+        } else {
+            const int t = __double2loint((double)after) & (int)A.T0.tie_zero;
 #pragma unroll
-                    for (int c = 3; c < NV; ++c) st[(S3_K1 + c) * TT] = k[c];
-                    st[S3_BN * TT] = bn;
-                } else {
-                    const int af = (int)st[S3_AXIS_FACE * TT];
-                    const int axis = af >> 8, fc = af & 255;
-                    const T hfull = st[S3_HFULL * TT];
-                    const T bd = axis == 0 ? b[0] : (axis == 1 ? b[1] : b[2]);
-                    const T xd = axis == 0 ? p0[0] : (axis == 1 ? p0[1] : p0[2]);
-                    const T gg = back ? -bd : bd, r = xd - face_offset(A, axis, (fc & 1) != 0);
-                    if (gg != T(0.)) {
-                        const T hn = hp - r / gg;
-                        if (hn == hn) hp = fmin(fmax(hn, T(0.)), hfull);
-                    }
-                    st[S3_HP * TT] = hp;
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) b[c] = st[(S3_K1 + c) * TT];
-#pragma unroll
-                    for (int c = 3; c < NV; ++c) k[c] = st[(S3_K1 + c) * TT];
-                    bn = st[S3_BN * TT];
-                }
-                hs = hp;
-            }
+            for (int c = 0; c < 3; ++c) d[c] = (T)__hiloint2double(__double2hiint((double)d[c]), __double2loint((double)d[c]) | t);
         }
+    }
+
+    // Step size of a trial step from the line's point (reading A5; spherical: physical cell edges, reading A19)
+    __device__ __forceinline__ T step_size(const Args &A) const
+    {
+        T h = A.h_step;
+        if (SPH) {
+            T rcos, r;
+            polar(y, rcos, r);
+            h = A.step_frac * fmin(rcos * A.hf[0], fmin(r * A.hf[1], A.hf[2]));
+        }
+        if (lam + (double)h > A.T0.max_length) h = (T)(A.T0.max_length - lam);
+        return h;
+    }
+
+    // One step of size hs from y given k1 = (b, k[3..]) and bn = |b| at y (all three consumed): trial end ys (position
+    // offsets in the frame of the trial end's cell, to which y has been moved as well; deviation components) and the
+    // length accL of the step.  Four evaluations per RK4 step in all; the cached cell on return is that of ys.
+    __device__ __forceinline__ void trial(const Args &A, T hs, T b[3], T *k, T bn, T *ys, T &accL)
+    {
+        const TraceArgs &G = A.T0;
+        T acc[NV];
         const T shs = back ? -hs : hs;
         if (G.method == QSL_EULER) {
 #pragma unroll
             for (int c = 0; c < NV; ++c) ys[c] = fma(shs, c < 3 ? b[c] : k[c], y[c]);
             enter_cell(A, ys);
             accL = hs * bn;
-        } else {
-            const T half = T(0.5) * shs;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
-            enter_cell(A, ys);
-#pragma unroll
-            for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
-            accL = bn;
-            // ---- stage 2
-            stage(ys, ys, b, k);
-            T bnS = T(0.);             // SPH: |b| is taken before the scaling to coordinate rates
-            if (SPH) bnS = to_rates(ys, b, k);
-            {
-                T xn[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
-                enter_cell(A, xn);
-                bn = SPH ? bnS : norm3r_fast<T>(b);
-#pragma unroll
-                for (int c = 0; c < NV; ++c) {
-                    const T kc = c < 3 ? b[c] : k[c];
-                    acc[c] = fma(T(2.), kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(half, kc, y[c]);
-                }
-                accL = fma(T(2.), bn, accL);
-            }
-            // ---- stage 3
-            stage(ys, ys, b, k);
-            if (SPH) bnS = to_rates(ys, b, k);
-            {
-                T xn[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
-                enter_cell(A, xn);
-                bn = SPH ? bnS : norm3r_fast<T>(b);
-#pragma unroll
-                for (int c = 0; c < NV; ++c) {
-                    const T kc = c < 3 ? b[c] : k[c];
-                    acc[c] = fma(T(2.), kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(shs, kc, y[c]);
-                }
-                accL = fma(T(2.), bn, accL);
-            }
-            // ---- stage 4
-            stage(ys, ys, b, k);
-            if (SPH) bnS = to_rates(ys, b, k);
-            {
-                const T fL = hs * (T(1.0) / T(6.0)), f = back ? -fL : fL;
-                T xn[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) xn[c] = fma(f, b[c] + acc[c], y[c]);
-                enter_cell(A, xn);             // the trial end is where the next attempt starts if it is accepted
-                bn = SPH ? bnS : norm3r_fast<T>(b);
-#pragma unroll
-                for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, k[c] + acc[c], y[c]);
-                accL = fL * (bn + accL);
-            }
+            return;
         }
-        // ys = trial end (offsets in the current frame), accL = length of the trial step
-        if (phase == 0) {
+        const T half = T(0.5) * shs;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) ys[c] = fma(half, b[c], y[c]);
+        enter_cell(A, ys);
+#pragma unroll
+        for (int c = 0; c < NV; ++c) { acc[c] = c < 3 ? b[c] : k[c]; if (c >= 3) ys[c] = fma(half, k[c], y[c]); }
+        accL = bn;
+        tie(A, ys, ys[NV - 1]);
+        // ---- stage 2
+        stage(ys, ys, b, k);
+        T bnS = T(0.);             // SPH: |b| is taken before the scaling to coordinate rates
+        if (SPH) bnS = to_rates(ys, b, k);
+        {
+            T xn[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xn[c] = fma(half, b[c], y[c]);
+            enter_cell(A, xn);
+            bn = SPH ? bnS : norm3r_fast<T>(b);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) {
+                const T kc = c < 3 ? b[c] : k[c];
+                acc[c] = fma(T(2.), kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(half, kc, y[c]);
+            }
+            accL = fma(T(2.), bn, accL);
+        }
+        // ---- stage 3
+        stage(ys, ys, b, k);
+        if (SPH) bnS = to_rates(ys, b, k);
+        {
+            T xn[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xn[c] = fma(shs, b[c], y[c]);
+            enter_cell(A, xn);
+            bn = SPH ? bnS : norm3r_fast<T>(b);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) {
+                const T kc = c < 3 ? b[c] : k[c];
+                acc[c] = fma(T(2.), kc, acc[c]); ys[c] = c < 3 ? xn[c] : fma(shs, kc, y[c]);
+            }
+            accL = fma(T(2.), bn, accL);
+            tie(A, ys, accL);
+        }
+        // ---- stage 4
+        stage(ys, ys, b, k);
+        if (SPH) bnS = to_rates(ys, b, k);
+        {
+            const T fL = hs * (T(1.0) / T(6.0)), f = back ? -fL : fL;
+            T xn[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xn[c] = fma(f, b[c] + acc[c], y[c]);
+            enter_cell(A, xn);             // the trial end is where the next attempt starts if it is accepted
+            bn = SPH ? bnS : norm3r_fast<T>(b);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) ys[c] = c < 3 ? xn[c] : fma(f, k[c] + acc[c], y[c]);
+            accL = fL * (bn + accL);
+        }
+    }
+
+    // One attempt of the trace kernel proper (as LineState2::advance): a trial step from y, committed if its end is
+    // inside the closed trace box; a line whose trial step leaves the box is recorded as it stands with REC_LANDING and
+    // landed by landing3_kernel.  Returns true when the line has left this kernel.
+    __device__ __forceinline__ bool advance(const Args &A)
+    {
+        const TraceArgs &G = A.T0;
+        T b[3], k[NV], ys[NV], accL;
+        {
+            T p0[3] = { y[0], y[1], y[2] };
+            enter_cell(A, p0);
+            stage(p0, y, b, k);
+            const T bn = to_rates(p0, b, k);
+            // O4: stall / caps are tested on k1 before the step
+            if (!(bn >= A.null_eps) || (long long)nsteps >= G.max_steps || lam >= G.max_length) {
+                finish(A, 255, !(bn >= A.null_eps) ? (nsteps == 0 ? REC_NULL_AT_SEED : REC_STALL) : REC_CAP, -1);
+                return true;
+            }
+            const T h = step_size(A);
+            trial(A, h, b, k, bn, ys, accL);
             if (inside3(A, ys)) {
 #pragma unroll
                 for (int c = 0; c < NV; ++c) y[c] = ys[c];
                 L += (double)accL; lam += (double)h; ++nsteps;
                 return false;
             }
-            // first face crossed by the chord: smallest fraction, tie -> lowest axis, then low face (reading A4)
-            T phi = INFINITY; int ax = -1, fc = 255; T bd = T(0.);
+        }
+        finish(A, 255, REC_LANDING, -1);
+        return true;
+    }
+
+    // The landing of one line (reading A4; as LineState2::land) from the state the trace kernel recorded: the trial step
+    // again, the chord, then step(hp), Newton, step(hp), Newton, step(hp), Newton, step(hp) -> snap onto the face, with
+    // k1 at y evaluated once.  Returns the number of steps added to the line.
+    __device__ unsigned land(const Args &A)
+    {
+        T b1[3], k1[NV], b[3], k[NV], ys[NV], accL;
+        {
+            T p0[3] = { y[0], y[1], y[2] };
+            enter_cell(A, p0);
+            stage(p0, y, b1, k1);
+        }
+        const T bn1 = to_rates(y, b1, k1);
+        const T h = step_size(A);
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                const bool lo_v = C[d] < A.cl[d] || (C[d] == A.cl[d] && ys[d] < A.off_lo[d]);
-                const bool hi_v = C[d] > A.ch[d] || (C[d] == A.ch[d] && ys[d] > A.off_hi[d]);
-                if (lo_v || hi_v) {
-                    const T fo = face_offset(A, d, !lo_v);
-                    const T f = (fo - y[d]) / (ys[d] - y[d]);
-                    if (f < phi) { phi = f; ax = d; fc = 2 * d + (lo_v ? 0 : 1); bd = fo; }
-                }
+        for (int c = 0; c < NV; ++c) { if (c < 3) b[c] = b1[c]; else k[c] = k1[c]; }
+        trial(A, h, b, k, bn1, ys, accL);
+        // first face crossed by the chord: smallest fraction, tie -> lowest axis, then low face (reading A4)
+        T phi = INFINITY; int ax = -1, fc = 255; T bd = T(0.);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const bool lo_v = C[d] < A.cl[d] || (C[d] == A.cl[d] && ys[d] < A.off_lo[d]);
+            const bool hi_v = C[d] > A.ch[d] || (C[d] == A.ch[d] && ys[d] > A.off_hi[d]);
+            if (lo_v || hi_v) {
+                const T fo = face_offset(A, d, !lo_v);
+                const T f = (fo - y[d]) / (ys[d] - y[d]);
+                if (f < phi) { phi = f; ax = d; fc = 2 * d + (lo_v ? 0 : 1); bd = fo; }
             }
-            if (ax < 0) { finish(A, 255, REC_STALL, -1); return true; }   // non-finite trial point
-            const T yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
-            if (yd == bd) {
-                // the line starts on the face it leaves through: the landing of O4 is one zero-length step
-                ++nsteps;
-                finish(A, fc, 0, ax);
-                return true;
+        }
+        if (ax < 0) { finish(A, 255, REC_STALL, -1); return 0; }   // non-finite trial point
+        const T yd = ax == 0 ? y[0] : (ax == 1 ? y[1] : y[2]);
+        if (yd == bd) {
+            // the line starts on the face it leaves through: the landing of O4 is one zero-length step
+            ++nsteps;
+            finish(A, fc, 0, ax);
+            return 1;
+        }
+        T hp = phi * h;
+        for (int it = 0; it < 4; ++it) {
+#pragma unroll
+            for (int c = 0; c < NV; ++c) { if (c < 3) b[c] = b1[c]; else k[c] = k1[c]; }
+            trial(A, hp, b, k, bn1, ys, accL);
+            if (it == 3) break;
+            // Newton update of hp from the field at the trial end (its cell is the cached one), clamped to [0, h]
+            stage(ys, y, b, k);
+            to_rates(ys, b, k);
+            const T bdn = ax == 0 ? b[0] : (ax == 1 ? b[1] : b[2]);
+            const T xd = ax == 0 ? ys[0] : (ax == 1 ? ys[1] : ys[2]);
+            const T gg = back ? -bdn : bdn, r = xd - face_offset(A, ax, (fc & 1) != 0);
+            if (gg != T(0.)) {
+                const T hn = hp - r / gg;
+                if (hn == hn) hp = fmin(fmax(hn, T(0.)), h);
             }
-            st[S3_HP * TT] = phi * h; st[S3_HFULL * TT] = h;
-            st[S3_AXIS_FACE * TT] = (T)((ax << 8) | fc);
-            phase = 1;
-            return false;
         }
-        if (phase < 4) {
-            st[(S3_DXT + 0) * TT] = ys[0] - y[0]; st[(S3_DXT + 1) * TT] = ys[1] - y[1]; st[(S3_DXT + 2) * TT] = ys[2] - y[2];
-            ++phase;
-            return false;
-        }
-        // phase 4: final landing step
-        const int af = (int)st[S3_AXIS_FACE * TT];
 #pragma unroll
         for (int c = 0; c < NV; ++c) y[c] = ys[c];
-        L += (double)accL; lam += (double)st[S3_HP * TT]; ++nsteps;
-        finish(A, af & 255, 0, af >> 8);
-        return true;
-#undef st
-#undef TT
+        L += (double)accL; lam += (double)hp; ++nsteps;
+        finish(A, fc, 0, ax);
+        return 1;
     }
 };
 
@@ -527,15 +564,20 @@ __global__ void __launch_bounds__(128) seed_basis3_kernel(const TraceArgs A, dou
 #ifndef QSL_T3_MIN_BLOCKS_L64
 #define QSL_T3_MIN_BLOCKS_L64 4
 #endif
-// Persistent grid, work items (one direction of one line) popped from a global counter with a warp-aggregated atomic; a
-// lane whose line ended refills at once (same queue as trace2_kernel).
+// Persistent grid; work items (one direction of one line) are staged per warp in shared memory, up to QSL_T3_CHUNK
+// consecutive items of the Morton order per pop of the global counter, exactly as in trace2_kernel (see there); a lane
+// whose line ended takes the next staged item.
+#ifndef QSL_T3_CHUNK
+#define QSL_T3_CHUNK 8
+#endif
 template <typename T, bool DEV, bool INTERP, bool REFILL, bool SPH = false>
 __global__ void __launch_bounds__(QSL_T3_THREADS, sizeof(T) == 4 ? (DEV ? QSL_T3_MIN_BLOCKS_LQ : QSL_T3_MIN_BLOCKS_L)
                                                                   : (DEV ? QSL_T3_MIN_BLOCKS_LQ64 : QSL_T3_MIN_BLOCKS_L64))
     trace3_kernel(const Trace3Args<T> A)
 {
     LineState3<T, DEV, INTERP, SPH> ls;
-    const long long n_items = 2 * A.T0.n;
+    const TraceArgs &G = A.T0;
+    const long long n_items = 2 * G.n;
     unsigned long long my_steps = 0;
     if (!REFILL) {
         const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -545,29 +587,105 @@ __global__ void __launch_bounds__(QSL_T3_THREADS, sizeof(T) == 4 ? (DEV ? QSL_T3
             my_steps = ls.nsteps;
         }
     } else {
-        const unsigned lane = threadIdx.x & 31u;
-        bool have = false, drained = false;
+        constexpr int NP = DEV ? 9 : 3;
+        __shared__ double pool_v[QSL_T3_THREADS / 32][NP][32];
+        __shared__ uint32_t pool_slot[QSL_T3_THREADS / 32][32];
+        const unsigned lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+        const long long n_warps = (long long)gridDim.x * (QSL_T3_THREADS / 32);
+        int pool_n = 0, pool_head = 0;              // warp-uniform
+        long long left = n_items;                   // work left in the queue when this warp last looked
+        bool have = false, drained = false;         // drained: warp-uniform
         while (true) {
-            if (!have && !drained) {
-                const unsigned m = __activemask();
-                const int leader = __ffs(m) - 1;
-                unsigned long long base = 0;
-                if ((int)lane == leader) base = atomicAdd(A.T0.queue, (unsigned long long)__popc(m));
-                base = __shfl_sync(m, base, leader);
-                const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
-                if (q >= n_items) drained = true;
-                else have = ls.init(A, q);
+            unsigned need = __ballot_sync(0xffffffffu, !have);
+            while (need) {
+                if (pool_n == 0) {
+                    if (drained) break;
+                    long long want = left / (4 * n_warps);
+                    want = max((long long)__popc(need), min(want, (long long)QSL_T3_CHUNK));
+                    unsigned long long base = 0;
+                    if (lane == 0) base = atomicAdd(G.queue, (unsigned long long)want);
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    left = n_items - (long long)base;
+                    const int got = left <= 0 ? 0 : (int)min(left, want);
+                    left -= got;
+                    if (got < (int)want) drained = true;
+                    if ((int)lane < got) {
+                        const long long q = (long long)base + lane;
+                        long long pos; int dir;
+                        if (G.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= G.n ? 1 : 0; pos = q - (long long)dir * G.n; }
+                        const uint32_t si = G.perm[pos];
+                        pool_slot[w][lane] = (uint32_t)((long long)dir * G.n + pos);
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) pool_v[w][c][lane] = G.seeds[3 * (size_t)si + c];
+                        if (DEV) {
+                            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(G.basis + 6 * (size_t)pos);
+                            const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
+                            pool_v[w][3 % NP][lane] = b0.x; pool_v[w][4 % NP][lane] = b0.y; pool_v[w][5 % NP][lane] = b1.x;
+                            pool_v[w][6 % NP][lane] = b1.y; pool_v[w][7 % NP][lane] = b2.x; pool_v[w][8 % NP][lane] = b2.y;
+                        }
+                    }
+                    __syncwarp();
+                    pool_n = got; pool_head = 0;
+                    if (got == 0) break;
+                }
+                const int rank = __popc(need & ((1u << lane) - 1u));
+                if (!have && rank < pool_n) {
+                    const int e = pool_head + rank;
+                    const double x[3] = { pool_v[w][0][e], pool_v[w][1][e], pool_v[w][2][e] };
+                    double bs[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
+                    if (DEV) {
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) bs[c] = pool_v[w][(3 + c) % NP][e];
+                    }
+                    have = ls.start(A, x, bs, pool_slot[w][e]);
+                }
+                const int served = min(pool_n, __popc(need));
+                pool_head += served; pool_n -= served;
+                __syncwarp();
+                need = __ballot_sync(0xffffffffu, !have);
             }
-            if (__all_sync(0xffffffffu, drained && !have)) break;
+            if (!__any_sync(0xffffffffu, have)) break;
             if (have) {
                 if (ls.advance(A)) { my_steps += ls.nsteps; have = false; }
             }
         }
     }
-    if (A.T0.total_steps) {
+    if (G.total_steps) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) my_steps += __shfl_xor_sync(0xffffffffu, my_steps, o);
-        if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(A.T0.total_steps, my_steps);
+        if ((threadIdx.x & 31) == 0 && my_steps) atomicAdd(G.total_steps, my_steps);
+    }
+}
+
+// The landings of all lines of a launch (reading A4): one thread per per-direction record (see landing_kernel).  The
+// frame of the recorded point is found again as for a seed (fp64 cell search, offset rounded to T).
+template <typename T, bool DEV, bool INTERP, bool SPH = false>
+__global__ void __launch_bounds__(128) landing3_kernel(const Trace3Args<T> A)
+{
+    const TraceArgs &G = A.T0;
+    const long long sl = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned added = 0;
+    if (sl < 2 * G.n) {
+        const double2 *__restrict__ r2 = reinterpret_cast<const double2 *>(G.rec + (size_t)sl * REC_DOUBLES);
+        const double2 w5 = r2[5];
+        if ((uint32_t)__double2hiint(w5.x) & REC_LANDING) {
+            LineState3<T, DEV, INTERP, SPH> ls;
+            constexpr int NV = LineState3<T, DEV, INTERP, SPH>::NV;
+            double v[10];
+#pragma unroll
+            for (int c = 0; c < 5; ++c) { const double2 t = r2[c]; v[2 * c] = t.x; v[2 * c + 1] = t.y; }
+            ls.frame_of(A, v);
+#pragma unroll
+            for (int c = 3; c < NV; ++c) ls.y[c] = (T)v[c];
+            ls.L = v[9]; ls.lam = w5.y; ls.nsteps = (uint32_t)__double2loint(w5.x);
+            ls.slot = (uint32_t)sl; ls.back = sl >= G.n; ls.phase = 0;
+            ls.load_cell(A);
+            added = ls.land(A);
+        }
+    }
+    if (G.total_steps) {
+        const unsigned m = __ballot_sync(0xffffffffu, added != 0);
+        if ((threadIdx.x & 31) == 0 && m) atomicAdd(G.total_steps, (unsigned long long)__popc(m));
     }
 }
 

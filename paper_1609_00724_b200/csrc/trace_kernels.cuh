@@ -39,6 +39,9 @@ struct TraceArgs {
 // Per-direction record written once when a line ends: x[3], d1[3], d2[3], L, (nsteps, face|flags) as two uint32, lambda.
 constexpr int REC_DOUBLES = 12;
 constexpr uint32_t REC_STALL = 1u << 8, REC_CAP = 1u << 9, REC_SEED_OUTSIDE = 1u << 10, REC_NULL_AT_SEED = 1u << 11;
+// Record flag of the cell-table and cell-frame kernels: the trial step from the recorded state leaves the trace box, the landing of
+// reading A4 is still to be done (landing_kernel / landing3_kernel clear it).  Bits 8..11 are the status flags above.
+constexpr uint32_t REC_LANDING = 1u << 12;
 
 template <typename S> struct Sample4;
 template <> struct Sample4<float> { using type = float4; };
