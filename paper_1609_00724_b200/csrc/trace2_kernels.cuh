@@ -14,6 +14,11 @@
 
 namespace qsl {
 
+// Build-time switches of the measured variants (QSL_NVCC_EXTRA="-D..."; the defaults are what profiles/r2d measured best):
+//   QSL_T2_HEADTEST  1: in-cell test at the head of an attempt as well (0: the cell of y is the cached one by construction)
+//   QSL_T2_CHUNK     work items a warp stages per pop of the global counter
+//   QSL_T2_TIE       scheduling fence between the work behind enter_cell() and the next polynomial (LineState2::tie)
+//   QSL_T2_DEFER     deviation products behind enter_cell(): 0 never, 1 all stages, 2 stage 1, 3 stages 1 and 3
 #ifndef QSL_T2_HEADTEST
 #define QSL_T2_HEADTEST 0
 #endif
@@ -586,9 +591,6 @@ __global__ void __launch_bounds__(128) seed_basis_kernel(const TraceArgs A, doub
 #ifndef QSL_T2_MIN_BLOCKS_L
 #define QSL_T2_MIN_BLOCKS_L 4
 #endif
-#ifndef QSL_T2_POOL
-#define QSL_T2_POOL 1
-#endif
 // The persistent kernel (REFILL): work items are taken from the global counter by the WARP, up to 32 consecutive items
 // of the Morton order at a time, and their seeds (and orthonormal pairs) are staged in shared memory by all 32 lanes at
 // once; a lane whose line has ended takes the next staged item with a few LDS instead of going through three dependent
@@ -607,7 +609,7 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
             while (!ls.advance(A)) {}
         }
         if (q < n_items) my_steps = ls.nsteps;
-    } else if (QSL_T2_POOL) {
+    } else {
         constexpr int NP = DEV ? 9 : 3;
         __shared__ double pool_v[QSL_T2_THREADS / 32][NP][32];
         __shared__ uint32_t pool_slot[QSL_T2_THREADS / 32][32];
@@ -666,25 +668,6 @@ __global__ void __launch_bounds__(QSL_T2_THREADS, DEV ? QSL_T2_MIN_BLOCKS_LQ : Q
                 need = __ballot_sync(0xffffffffu, !have);
             }
             if (!__any_sync(0xffffffffu, have)) break;
-            if (have) {
-                if (ls.advance(A)) { my_steps += ls.nsteps; have = false; }
-            }
-        }
-    } else {
-        const unsigned lane = threadIdx.x & 31u;
-        bool have = false, drained = false;
-        while (true) {
-            if (!have && !drained) {
-                const unsigned m = __activemask();
-                const int leader = __ffs(m) - 1;
-                unsigned long long base = 0;
-                if ((int)lane == leader) base = atomicAdd(A.queue, (unsigned long long)__popc(m));
-                base = __shfl_sync(m, base, leader);
-                const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
-                if (q >= n_items) drained = true;
-                else have = ls.template init<!QSL_T2_HEADTEST>(A, q);
-            }
-            if (__all_sync(0xffffffffu, drained && !have)) break;
             if (have) {
                 if (ls.advance(A)) { my_steps += ls.nsteps; have = false; }
             }
