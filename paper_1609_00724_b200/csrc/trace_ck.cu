@@ -34,6 +34,12 @@ static int launch_trace_ck_variant(TraceArgs &A, double tol, bool refill, cudaEv
             else trace_ck_kernel<DEV, STRETCHED, INTERP, false, SPH><<<(unsigned)blocks, threads, 0, s>>>(A, tol);
             e = cudaGetLastError();
         }
+        if (e == cudaSuccess) {
+            // the landings (reading A4) of all lines at once; part of the trace time
+            count_launch();
+            landing_ck_kernel<DEV, STRETCHED, INTERP, SPH><<<(unsigned)((n_items + 127) / 128), 128, 0, s>>>(A);
+            e = cudaGetLastError();
+        }
         if (e == cudaSuccess && ev1) e = cudaEventRecord(ev1, s);
         if (e != cudaSuccess) rc = record_cuda(e);
     }

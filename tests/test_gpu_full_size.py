@@ -190,3 +190,28 @@ def test_refined_levels_full_size_sampled(name):
         rep = compare_trace(g, c, cfg["box_lo"], cfg["box_hi"], label="%s level %d of %d children" % (name, level, n))
         assert rep["n"] >= 6000
     fg.destroy()
+
+
+@pytest.mark.parametrize("name,stride", [("cfg2", 97), ("cfg4", 4093)])
+@pytest.mark.parametrize("method", ["euler", "ck45"])
+def test_full_size_sampled_with_the_papers_integrators(name, stride, method):
+    """The paper's own steppers at full size (fixed-step Euler; adaptive Cash-Karp at tolerance 1e-2,
+    readings A5 / A16), L + Q, sampled against the oracle at the north_star gates; for the adaptive stepper the per-line
+    step counts must agree too (the controller takes the oracle's accept / reject / double decisions)."""
+    cfg = qi.make_config(name)
+    m = qsl.QSL_EULER if method == "euler" else qsl.QSL_CK45
+    step_frac = 0.2 if method == "euler" else cfg["step_frac"]       # PAPER.md:143: about five samples per cell
+    fg = gpu_field(cfg["grid"], cfg["B"], cfg["sample_type"], 0)
+    p = qsl.make_trace_params(cfg["box_lo"], cfg["box_hi"], mode=qsl.QSL_TRACE_LQ, method=m, step_frac=step_frac,
+                              max_steps=cfg["max_steps"], null_eps=cfg["null_eps"], tol=1e-2)
+    tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    g = qsl.qsl_trace(fg, torch.from_numpy(cfg["seeds"]).cuda(), p, total_steps=tot)
+    torch.cuda.synchronize()
+    assert int(tot.item()) == int(g["nsteps_f"].to(torch.int64).sum() + g["nsteps_b"].to(torch.int64).sum())
+    idx = _sample(len(cfg["seeds"]), stride, run=1031)
+    fc = cpu_field(cfg["grid"], cfg["B"], cfg["sample_type"], 0)
+    c = oracle.trace(fc, cfg["seeds"][idx], cfg["box_lo"], cfg["box_hi"], mode=oracle.TRACE_LQ, method=m, step_frac=step_frac,
+                     max_steps=cfg["max_steps"], null_eps=cfg["null_eps"], tol=1e-2)
+    rep = compare_trace(_pick(g, idx), c, cfg["box_lo"], cfg["box_hi"], label="%s full %s" % (name, method))
+    assert rep["n"] > 5000 and rep["same_steps"] >= 0.999
+    fg.destroy()
