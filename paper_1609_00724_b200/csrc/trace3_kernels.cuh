@@ -565,8 +565,8 @@ __global__ void __launch_bounds__(128) seed_basis3_kernel(const TraceArgs A, dou
 #define QSL_T3_MIN_BLOCKS_L64 4
 #endif
 // Persistent grid; work items (one direction of one line) are staged per warp in shared memory, up to QSL_T3_CHUNK
-// consecutive items of the Morton order per pop of the global counter, exactly as in trace2_kernel (see there); a lane
-// whose line ended takes the next staged item.
+// consecutive items of the Morton order per pop of the global counter (staged_queue, trace_kernels.cuh); a lane whose
+// line ended takes the next staged item.
 #ifndef QSL_T3_CHUNK
 #define QSL_T3_CHUNK 8
 #endif
@@ -587,68 +587,9 @@ __global__ void __launch_bounds__(QSL_T3_THREADS, sizeof(T) == 4 ? (DEV ? QSL_T3
             my_steps = ls.nsteps;
         }
     } else {
-        constexpr int NP = DEV ? 9 : 3;
-        __shared__ double pool_v[QSL_T3_THREADS / 32][NP][32];
-        __shared__ uint32_t pool_slot[QSL_T3_THREADS / 32][32];
-        const unsigned lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-        const long long n_warps = (long long)gridDim.x * (QSL_T3_THREADS / 32);
-        int pool_n = 0, pool_head = 0;              // warp-uniform
-        long long left = n_items;                   // work left in the queue when this warp last looked
-        bool have = false, drained = false;         // drained: warp-uniform
-        while (true) {
-            unsigned need = __ballot_sync(0xffffffffu, !have);
-            while (need) {
-                if (pool_n == 0) {
-                    if (drained) break;
-                    long long want = left / (4 * n_warps);
-                    want = max((long long)__popc(need), min(want, (long long)QSL_T3_CHUNK));
-                    unsigned long long base = 0;
-                    if (lane == 0) base = atomicAdd(G.queue, (unsigned long long)want);
-                    base = __shfl_sync(0xffffffffu, base, 0);
-                    left = n_items - (long long)base;
-                    const int got = left <= 0 ? 0 : (int)min(left, want);
-                    left -= got;
-                    if (got < (int)want) drained = true;
-                    if ((int)lane < got) {
-                        const long long q = (long long)base + lane;
-                        long long pos; int dir;
-                        if (G.interleave) { pos = q >> 1; dir = (int)(q & 1); } else { dir = q >= G.n ? 1 : 0; pos = q - (long long)dir * G.n; }
-                        const uint32_t si = G.perm[pos];
-                        pool_slot[w][lane] = (uint32_t)((long long)dir * G.n + pos);
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) pool_v[w][c][lane] = G.seeds[3 * (size_t)si + c];
-                        if (DEV) {
-                            const double2 *__restrict__ bp = reinterpret_cast<const double2 *>(G.basis + 6 * (size_t)pos);
-                            const double2 b0 = bp[0], b1 = bp[1], b2 = bp[2];
-                            pool_v[w][3 % NP][lane] = b0.x; pool_v[w][4 % NP][lane] = b0.y; pool_v[w][5 % NP][lane] = b1.x;
-                            pool_v[w][6 % NP][lane] = b1.y; pool_v[w][7 % NP][lane] = b2.x; pool_v[w][8 % NP][lane] = b2.y;
-                        }
-                    }
-                    __syncwarp();
-                    pool_n = got; pool_head = 0;
-                    if (got == 0) break;
-                }
-                const int rank = __popc(need & ((1u << lane) - 1u));
-                if (!have && rank < pool_n) {
-                    const int e = pool_head + rank;
-                    const double x[3] = { pool_v[w][0][e], pool_v[w][1][e], pool_v[w][2][e] };
-                    double bs[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
-                    if (DEV) {
-#pragma unroll
-                        for (int c = 0; c < 6; ++c) bs[c] = pool_v[w][(3 + c) % NP][e];
-                    }
-                    have = ls.start(A, x, bs, pool_slot[w][e]);
-                }
-                const int served = min(pool_n, __popc(need));
-                pool_head += served; pool_n -= served;
-                __syncwarp();
-                need = __ballot_sync(0xffffffffu, !have);
-            }
-            if (!__any_sync(0xffffffffu, have)) break;
-            if (have) {
-                if (ls.advance(A)) { my_steps += ls.nsteps; have = false; }
-            }
-        }
+        staged_queue<DEV, QSL_T3_THREADS, QSL_T3_CHUNK>(
+            G, [&](const double *x, const double *bs, uint32_t sl) { return ls.start(A, x, bs, sl); },
+            [&]() { if (!ls.advance(A)) return false; my_steps += ls.nsteps; return true; });
     }
     if (G.total_steps) {
 #pragma unroll

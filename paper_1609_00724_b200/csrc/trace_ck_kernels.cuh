@@ -170,24 +170,9 @@ __global__ void __launch_bounds__(128, 2) trace_ck_kernel(const TraceArgs A, con
             my_steps = ls.nsteps;
         }
     } else {
-        const unsigned lane = threadIdx.x & 31u;
-        bool have = false, drained = false;
-        while (true) {
-            if (!have && !drained) {
-                const unsigned m = __activemask();
-                const int leader = __ffs(m) - 1;
-                unsigned long long base = 0;
-                if ((int)lane == leader) base = atomicAdd(A.queue, (unsigned long long)__popc(m));
-                base = __shfl_sync(m, base, leader);
-                const long long q = (long long)base + __popc(m & ((1u << lane) - 1u));
-                if (q >= n_items) drained = true;
-                else { ls.j = 0; have = ls.init(A, q); }
-            }
-            if (__all_sync(0xffffffffu, drained && !have)) break;
-            if (have) {
-                if (ls.advance_ck(A, tol)) { my_steps += ls.nsteps; have = false; }
-            }
-        }
+        staged_queue<DEV, 128, QSL_T2_CHUNK>(
+            A, [&](const double *x, const double *bs, uint32_t sl) { ls.j = 0; return ls.start(A, x, bs, sl); },
+            [&]() { if (!ls.advance_ck(A, tol)) return false; my_steps += ls.nsteps; return true; });
     }
     if (A.total_steps) {
 #pragma unroll
