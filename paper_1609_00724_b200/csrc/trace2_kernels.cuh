@@ -367,7 +367,7 @@ struct LineState2 {
         constexpr bool EARLY1 = SPH || !(QSL_T2_DEFER == 1 || QSL_T2_DEFER == 2 || QSL_T2_DEFER == 3);
         constexpr bool EARLY3 = SPH || !(QSL_T2_DEFER == 1 || QSL_T2_DEFER == 3);
         constexpr bool EARLY = SPH || QSL_T2_DEFER != 1;
-        constexpr bool TIE = !SPH && QSL_T2_TIE;
+        constexpr bool TIE = QSL_T2_TIE;
         double b[3], J[NJ], k[NV], d[3], acc[NV], ys[NV], bn;
         const double shs = back ? -hs : hs;
 #pragma unroll
