@@ -523,8 +523,8 @@ def streaming_block(qsl, torch, W):
         cc, cs, cb = qsl.qsl_refine(lat, 0, None, S3.view(-1), tau, capacity=cap)
         m[0] = int(cc.shape[0])
     ms = best(refine)
-    put("refine", ms, 8 * N + 8 * N + 4 * N * 2 + m[0] * (12 + 24) + 8 * N,
-        "flag + scan + emit of 6.7e7 cells, %d children: S read twice, flags write+read, child_base 8 B per cell, 36 B per child (includes the host sync for the count)" % m[0])
+    put("refine", ms, 8 * N * 2 + m[0] * (12 + 24) + 8 * N,
+        "count + scan + fused scan / emit of 6.7e7 cells, %d children: S read twice, child_base 8 B per cell, 36 B per child (includes the host sync for the count)" % m[0])
     # sparse FLEDGE of level 1 on those children
     cc, cs, cb = qsl.qsl_refine(lat, 0, None, S3.view(-1), tau, capacity=cap)
     L1 = torch.rand(cc.shape[0], dtype=torch.float64, device="cuda", generator=gen) + 0.1

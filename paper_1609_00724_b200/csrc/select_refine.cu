@@ -93,51 +93,94 @@ struct RefineArgs {
     long long *child_base;
 };
 
-__global__ void __launch_bounds__(256) refine_flag_kernel(long long n, const double *__restrict__ S, const double *__restrict__ tau,
-                                                          uint32_t *__restrict__ flags)
+// Refinement in three launches without a flag or an offset array: (1) flagged cells per tile of RF_TILE cells, straight
+// from S and tau; (2) exclusive scan of the tile counts (one block); (3) per tile: the flags again, a block-wide
+// exclusive scan, and the children of every flagged cell written at (tile offset + rank) << NDIM - the stable
+// compaction of O7.  Per cell 8 B of S twice and 8 B of child_base, per child 4 NDIM + 24 B.
+constexpr int RF_THREADS = 256;
+constexpr int RF_ITEMS = 8;                          // consecutive cells per thread (the scan order is the cell order)
+constexpr int RF_TILE = RF_THREADS * RF_ITEMS;
+
+__global__ void __launch_bounds__(RF_THREADS) refine_count_kernel(long long n, const double *__restrict__ S,
+                                                                  const double *__restrict__ tau,
+                                                                  unsigned long long *__restrict__ tile_counts)
 {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) flags[i] = S[i] > *tau ? 1u : 0u;                // NaN never flags
+    const double t = *tau;
+    const long long base = (long long)blockIdx.x * RF_TILE;
+    unsigned long long c = 0;
+#pragma unroll
+    for (int k = 0; k < RF_ITEMS; ++k) {
+        const long long i = base + (long long)k * RF_THREADS + threadIdx.x;      // coalesced: the count needs no order
+        if (i < n) c += S[i] > t ? 1u : 0u;                                      // NaN never flags
+    }
+    unsigned long long total;
+    block_exclusive_scan(c, total);
+    if (threadIdx.x == 0) tile_counts[blockIdx.x] = total;
 }
 
 template <int NDIM>
-__global__ void __launch_bounds__(256) refine_emit_kernel(const RefineArgs A, const uint32_t *__restrict__ flags,
-                                                          const unsigned long long *__restrict__ offs)
+__global__ void __launch_bounds__(RF_THREADS) refine_emit_kernel(const RefineArgs A, const unsigned long long *__restrict__ tile_offs)
 {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= A.n) return;
-    if (!flags[i]) { if (A.child_base) A.child_base[i] = -1; return; }
-    const long long first = (long long)offs[i] << NDIM;
-    if (A.child_base) A.child_base[i] = first;
-    uint32_t c[3];
-    if (A.coords) {
+    __shared__ unsigned char s_flag[RF_TILE];
+    __shared__ long long s_first[RF_TILE];          // first child of the cell, or -1
+    const double t = *A.tau;
+    const long long base = (long long)blockIdx.x * RF_TILE;
+    // flags of the tile, loaded with coalesced accesses
 #pragma unroll
-        for (int d = 0; d < NDIM; ++d) c[d] = A.coords[i * NDIM + d];
-    } else {
-        c[0] = (uint32_t)(i % A.n0[0]);
-        c[1] = (uint32_t)((i / A.n0[0]) % A.n0[1]);
-        c[2] = (uint32_t)(i / (A.n0[0] * A.n0[1]));
+    for (int k = 0; k < RF_ITEMS; ++k) {
+        const int e = k * RF_THREADS + threadIdx.x;
+        s_flag[e] = base + e < A.n && A.S[base + e] > t ? 1 : 0;                // NaN never flags
     }
+    __syncthreads();
+    // thread t ranks RF_ITEMS consecutive cells, so that the scan order is the cell order (stable compaction)
+    unsigned long long mine = 0;
+#pragma unroll
+    for (int k = 0; k < RF_ITEMS; ++k) mine += s_flag[threadIdx.x * RF_ITEMS + k];
+    unsigned long long total;
+    unsigned long long rank = block_exclusive_scan(mine, total) + tile_offs[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < RF_ITEMS; ++k) {
+        const int e = threadIdx.x * RF_ITEMS + k;
+        s_first[e] = s_flag[e] ? (long long)(rank++) << NDIM : -1ll;
+    }
+    __syncthreads();
     double inv_den[3];
 #pragma unroll
     for (int d = 0; d < NDIM; ++d) inv_den[d] = (double)(A.n0[d] << (A.level + 1));
+    for (int k = 0; k < RF_ITEMS; ++k) {
+        const int e = k * RF_THREADS + threadIdx.x;
+        const long long i = base + e;
+        if (i >= A.n) break;
+        const long long first = s_first[e];
+        if (A.child_base) A.child_base[i] = first;
+        if (first < 0) continue;
+        uint32_t c[3];
+        if (A.coords) {
 #pragma unroll
-    for (int ch = 0; ch < (1 << NDIM); ++ch) {
-        const long long m = first + ch;
-        if (m >= A.capacity) return;
-        double w[3] = { 0.0, 0.0, 0.0 };
-#pragma unroll
-        for (int d = 0; d < NDIM; ++d) {
-            const uint32_t cc = 2u * c[d] + (uint32_t)((ch >> d) & 1);
-            A.child_coords[m * NDIM + d] = cc;
-            w[d] = __ddiv_rn((double)cc + 0.5, inv_den[d]);      // one IEEE division, as in the definition
+            for (int d = 0; d < NDIM; ++d) c[d] = A.coords[i * NDIM + d];
+        } else {
+            c[0] = (uint32_t)(i % A.n0[0]);
+            c[1] = (uint32_t)((i / A.n0[0]) % A.n0[1]);
+            c[2] = (uint32_t)(i / (A.n0[0] * A.n0[1]));
         }
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            double pos = __fma_rn(w[0], A.e[0][k], A.origin[k]);
-            pos = __fma_rn(w[1], A.e[1][k], pos);
-            if (NDIM == 3) pos = __fma_rn(w[2], A.e[2][k], pos);
-            A.child_seeds[3 * m + k] = pos;
+        for (int ch = 0; ch < (1 << NDIM); ++ch) {
+            const long long m = first + ch;
+            if (m >= A.capacity) break;
+            double w[3] = { 0.0, 0.0, 0.0 };
+#pragma unroll
+            for (int d = 0; d < NDIM; ++d) {
+                const uint32_t cc = 2u * c[d] + (uint32_t)((ch >> d) & 1);
+                A.child_coords[m * NDIM + d] = cc;
+                w[d] = __ddiv_rn((double)cc + 0.5, inv_den[d]);      // one IEEE division, as in the definition
+            }
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                double pos = __fma_rn(w[0], A.e[0][q], A.origin[q]);
+                pos = __fma_rn(w[1], A.e[1][q], pos);
+                if (NDIM == 3) pos = __fma_rn(w[2], A.e[2][q], pos);
+                A.child_seeds[3 * m + q] = pos;
+            }
         }
     }
 }
@@ -196,30 +239,25 @@ extern "C" int qsl_refine(int ndim, int level, long long n, const unsigned int *
     }
     A.capacity = capacity; A.child_coords = child_coords; A.child_seeds = child_seeds; A.child_base = child_base;
 
-    void *flags = nullptr, *offs = nullptr, *tiles = nullptr, *total = nullptr;
-    const long long ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
-    int rc = scratch_alloc(&flags, sizeof(uint32_t) * (size_t)n, s);
-    if (rc == QSL_OK) rc = scratch_alloc(&offs, sizeof(unsigned long long) * (size_t)n, s);
-    if (rc == QSL_OK) rc = scratch_alloc(&tiles, sizeof(unsigned long long) * (size_t)ntiles, s);
+    void *tiles = nullptr, *total = nullptr;
+    const long long ntiles = (n + RF_TILE - 1) / RF_TILE;
+    int rc = scratch_alloc(&tiles, sizeof(unsigned long long) * (size_t)ntiles, s);
     if (rc == QSL_OK) rc = scratch_alloc(&total, sizeof(unsigned long long), s);
     unsigned long long h_total = 0;
     if (rc == QSL_OK) {
-        const unsigned blocks = (unsigned)((n + 255) / 256);
         count_launch();
-        refine_flag_kernel<<<blocks, 256, 0, s>>>(n, S, tau, (uint32_t *)flags);
-        cudaError_t e = exclusive_scan_u32(n, (const uint32_t *)flags, (unsigned long long *)offs, (unsigned long long *)tiles,
-                                           (unsigned long long *)total, s);
-        if (e == cudaSuccess) {
-            count_launch();
-            if (ndim == 2) refine_emit_kernel<2><<<blocks, 256, 0, s>>>(A, (const uint32_t *)flags, (const unsigned long long *)offs);
-            else refine_emit_kernel<3><<<blocks, 256, 0, s>>>(A, (const uint32_t *)flags, (const unsigned long long *)offs);
-            e = cudaGetLastError();
-        }
+        refine_count_kernel<<<(unsigned)ntiles, RF_THREADS, 0, s>>>(n, S, tau, (unsigned long long *)tiles);
+        count_launch();
+        scan_single_block<<<1, 1024, 0, s>>>(ntiles, (unsigned long long *)tiles, (unsigned long long *)total);
+        count_launch();
+        if (ndim == 2) refine_emit_kernel<2><<<(unsigned)ntiles, RF_THREADS, 0, s>>>(A, (const unsigned long long *)tiles);
+        else refine_emit_kernel<3><<<(unsigned)ntiles, RF_THREADS, 0, s>>>(A, (const unsigned long long *)tiles);
+        cudaError_t e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaMemcpyAsync(&h_total, total, sizeof(h_total), cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) rc = record_cuda(e);
     }
-    scratch_free(flags, s); scratch_free(offs, s); scratch_free(tiles, s); scratch_free(total, s);
+    scratch_free(tiles, s); scratch_free(total, s);
     if (rc != QSL_OK) return rc;
     *n_children = (long long)(h_total << ndim);
     if (*n_children > capacity) return QSL_ERANGE;
