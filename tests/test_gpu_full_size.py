@@ -45,6 +45,11 @@ def _properties(cfg, g, total_steps, with_q):
     hi = torch.tensor(cfg["box_hi"], dtype=torch.float64, device="cuda")
     st = g["status"]
     assert int((st & (qsl.QSL_ST_SEED_OUTSIDE | qsl.QSL_ST_NULL_AT_SEED)).count_nonzero()) == 0
+    assert int((st & ~0x7f).count_nonzero()) == 0          # only the documented QSL_ST_* bits (no internal record flag leaks)
+    # every line was landed (or stalled / capped): a face other than 255 goes with a snapped end, face 255 with a status bit
+    for face, bits in ((g["face_f"], qsl.QSL_ST_STALL_F | qsl.QSL_ST_CAP_F), (g["face_b"], qsl.QSL_ST_STALL_B | qsl.QSL_ST_CAP_B)):
+        assert bool((((face == 255) == ((st & bits) != 0))).all())
+        assert bool((face[face != 255] <= 5).all())
     assert total_steps == int(g["nsteps_f"].to(torch.int64).sum() + g["nsteps_b"].to(torch.int64).sum())
     seeds = torch.from_numpy(cfg["seeds"]).cuda()
     for end, face, ns in ((g["end_f"], g["face_f"], g["nsteps_f"]), (g["end_b"], g["face_b"], g["nsteps_b"])):
