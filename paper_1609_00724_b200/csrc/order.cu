@@ -4,7 +4,7 @@
 // result: outputs are scattered back to the caller's order.
 //
 // The sort is a hand-written stable LSD radix sort on 32- or 64-bit keys (8-bit digits): per pass a per-tile digit
-// histogram, one exclusive scan of the (digit-major) count table, and a scatter that sorts a tile of 4096 (64-bit keys: 2048) keys by the
+// histogram, one exclusive scan of the (digit-major) count table, and a scatter that sorts a tile of 2048 keys by the
 // digit in shared memory (warps rank their keys with __match_any_sync) and writes it out run by run.
 #include "qsl_internal.cuh"
 #include "scan.cuh"
@@ -13,7 +13,7 @@ namespace qsl {
 
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-template <typename K> struct SortTile { static constexpr int value = sizeof(K) == 8 ? 2048 : 4096; };   // keys per block per pass (static shared memory <= 48 KB)
+template <typename K> struct SortTile { static constexpr int value = sizeof(K) == 8 ? 2048 : 2048; };   // keys per block per pass (static shared memory <= 48 KB)
 
 __device__ __forceinline__ uint32_t spread3(uint32_t v)   // 10 bits -> every third bit
 {
