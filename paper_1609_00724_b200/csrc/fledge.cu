@@ -184,41 +184,64 @@ struct SparseArgs {
     double *S;
 };
 
-template <int NDIM>
-__device__ __forceinline__ double lookup_L(const SparseArgs &A, long long c0, long long c1, long long c2)
-{
-    const int lev = A.level;
-    long long idx = ((NDIM == 3 ? (c2 >> lev) : 0) * A.n0[1] + (c1 >> lev)) * A.n0[0] + (c0 >> lev);
-    for (int l = 1; l <= lev; ++l) {
-        const long long base = __ldg(A.child_base[l - 1] + idx);
-        if (base < 0) return __ldg(A.L[l - 1] + idx);
-        const int sh = lev - l;
-        int bits = (int)((c0 >> sh) & 1) | ((int)((c1 >> sh) & 1) << 1);
-        if (NDIM == 3) bits |= (int)((c2 >> sh) & 1) << 2;
-        idx = base + bits;
-    }
-    return __ldg(A.L[lev] + idx);
-}
-
+// One thread per cell of `level`.  The 27 (9) neighbours of a cell have at most two distinct ancestors per axis at every
+// coarser level (c - 1 and c + 1 shifted down; c's own ancestor is one of them), so only 2^NDIM walks go down the
+// child_base links to level - 1 instead of 27 (9); the neighbours then read their L through the child_base of their
+// parent's slot, or take the L of the ancestor at which that slot's walk ended (not refined further).
 template <int NDIM>
 __global__ void __launch_bounds__(FL_THREADS) fledge_sparse_kernel(const SparseArgs A)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= A.count) return;
-    const long long dims[3] = { A.n0[0] << A.level, A.n0[1] << A.level, NDIM == 3 ? A.n0[2] << A.level : 1 };
-    const long long c0 = A.coords[i * NDIM], c1 = A.coords[i * NDIM + 1], c2 = NDIM == 3 ? A.coords[i * NDIM + 2] : 0;
+    const int lev = A.level;
+    constexpr int NS = 1 << NDIM;
+    long long nb[3][3];                              // clamped neighbour coordinates per axis
+    long long par[3][2];                             // their two candidate parents (level lev - 1)
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const long long dim = d < NDIM ? A.n0[d] << lev : 1;
+        const long long c = d < NDIM ? (long long)A.coords[i * NDIM + d] : 0;
+#pragma unroll
+        for (int o = 0; o < 3; ++o) nb[d][o] = min(max(c + o - 1, 0ll), dim - 1);
+        par[d][0] = nb[d][0] >> 1; par[d][1] = nb[d][2] >> 1;
+    }
+    long long slot_base[NS];                         // index at level lev of the first child of the slot's cell, or -1
+    double slot_val[NS];                             // L of the ancestor the slot's walk ended at (slot_base < 0)
+#pragma unroll
+    for (int sl = 0; sl < NS; ++sl) {
+        const long long q0 = par[0][sl & 1], q1 = par[1][(sl >> 1) & 1], q2 = NDIM == 3 ? par[2][(sl >> 2) & 1] : 0;
+        const int top = lev - 1;                      // level of (q0, q1, q2)
+        long long idx = ((NDIM == 3 ? (q2 >> top) : 0) * A.n0[1] + (q1 >> top)) * A.n0[0] + (q0 >> top);
+        long long base = 0; double val = 0.0; bool ended = false;
+        for (int l = 1; l <= top; ++l) {
+            base = __ldg(A.child_base[l - 1] + idx);
+            if (base < 0) { val = __ldg(A.L[l - 1] + idx); ended = true; break; }
+            const int sh = top - l;
+            int bits = (int)((q0 >> sh) & 1) | ((int)((q1 >> sh) & 1) << 1);
+            if (NDIM == 3) bits |= (int)((q2 >> sh) & 1) << 2;
+            idx = base + bits;
+        }
+        if (!ended) {
+            base = __ldg(A.child_base[top] + idx);
+            if (base < 0) { val = __ldg(A.L[top] + idx); ended = true; }
+        }
+        slot_base[sl] = ended ? -1 : base;
+        slot_val[sl] = val;
+    }
     double As[3], Bs[3], Cs[3], centre = 0.0;
 #pragma unroll
     for (int o0 = 0; o0 < 3; ++o0) {
-        const long long x = min(max(c0 + o0 - 1, 0ll), dims[0] - 1);
         double a[3][3];
 #pragma unroll
         for (int o2 = 0; o2 < (NDIM == 3 ? 3 : 1); ++o2) {
-            const long long z = NDIM == 3 ? min(max(c2 + o2 - 1, 0ll), dims[2] - 1) : 0;
 #pragma unroll
             for (int o1 = 0; o1 < 3; ++o1) {
-                const long long y = min(max(c1 + o1 - 1, 0ll), dims[1] - 1);
-                a[o2][o1] = lookup_L<NDIM>(A, x, y, z);
+                const long long x = nb[0][o0], y = nb[1][o1], z = NDIM == 3 ? nb[2][o2] : 0;
+                int sl = ((x >> 1) != par[0][0] ? 1 : 0) | ((y >> 1) != par[1][0] ? 2 : 0);
+                int bits = (int)(x & 1) | ((int)(y & 1) << 1);
+                if (NDIM == 3) { sl |= (z >> 1) != par[2][0] ? 4 : 0; bits |= (int)(z & 1) << 2; }
+                const long long base = slot_base[sl];
+                a[o2][o1] = base < 0 ? slot_val[sl] : __ldg(A.L[lev] + base + bits);
             }
         }
         fold_column<NDIM>(a, As[o0], Bs[o0], Cs[o0]);
