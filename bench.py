@@ -48,7 +48,7 @@ FLOPS_PER_STEP = {"LQ": 800, "L": 400}
 # fp32 arithmetic) as a fraction of peak.  Keyed by (workload, arithmetic); absent -> null in the bench line.
 NCU_CAPTURES = {
     ("cfg2", "f64"): {"dram_bytes": 786209280, "pipe_active": 0.620, "source": "profiles/r2d_cfg4_trace_kernel.md (cfg2 capture)"},
-    ("cfg4", "f64"): {"dram_bytes": 46995332000, "pipe_active": 0.643, "source": "profiles/r2d_cfg4_trace_kernel.md"},
+    ("cfg4", "f64"): {"dram_bytes": 47756282000, "pipe_active": 0.649, "source": "profiles/r2f_final_build_cfg4.md"},
     ("cfg5", "f64"): {"dram_bytes": 626591608000, "pipe_active": 0.525,
                       "source": "profiles/r2d_cfg4_trace_kernel.md (cfg5 level 0, the L-only launch)"},
 }
