@@ -732,9 +732,9 @@ def main():
                 continue
             try:
                 Wo = Workload(qsl, torch, name, args)
-                # cfg5 is 30 s per pass: one timed pass after one warm-up at 1/8 scale is not possible on the same field,
-                # so its single pass is cold (memory pools of the previous workloads are warm; reported as warmup 0)
-                To = time_device(Wo, 1 if name == "cfg5" else 3, 0 if name == "cfg5" else 2, flush, barrier)
+                # cfg5 is 24 s per pass: one timed pass after one warm-up pass (a cold pass spends another 0.76 s in
+                # cudaMalloc of the 10 - 60 GB blocks of its levels: 24.36 s cold, 23.60 s warm, profiles/r2f)
+                To = time_device(Wo, 1 if name == "cfg5" else 3, 1 if name == "cfg5" else 2, flush, barrier)
                 per_config[name] = summary(name, To, Wo)
                 if getattr(Wo, "level_sizes", None):
                     per_config[name]["level_sizes"] = Wo.level_sizes

@@ -243,14 +243,7 @@ int qsl_hilbert_convert(const qsl_lattice *lat, int R, int r, long long n, const
 long long qsl_launch_count(void);
 int qsl_profile_enable(int on);
 int qsl_profile_trace_kernel_ms(double ms[2], long long launches[2]);
-/* Roofline denominators measured on this device, each timed with CUDA events (2 warm-up launches, best of `reps`);
- * both synchronise.  fma_per_s (host): fused multiply-adds per second of the plain FP pipe, fp64 != 0 -> DFMA, else
- * FFMA, from 8 independent register-only chains per thread.  samples_per_s (host): divergent pseudo-random gathers per
- * second of one 16-byte (float4) or 32-byte (double4) sample per lane over a zero-filled scratch buffer of
- * footprint_bytes (rounded down to a power of two), i.e. the tracer's load shape with an L1-, L2- or HBM-resident
- * field.  Errors: QSL_EINVAL, QSL_ENOMEM, QSL_ECUDA.                                                                */
-int qsl_peak_fma(int fp64, int reps, double *fma_per_s, void *stream);
-int qsl_peak_gather(int bytes_per_sample, long long footprint_bytes, int reps, double *samples_per_s, void *stream);
+/* (The roofline denominators bench.py measures on the device are not part of this library: include/qsl_peaks.h.) */
 
 #ifdef __cplusplus
 }

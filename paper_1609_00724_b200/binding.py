@@ -14,6 +14,7 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("QSL_LIB_PATH") or os.path.join(_HERE, "libqsl.so")   # override: A/B runs of two builds
+PEAKS_LIB_PATH = os.path.join(_HERE, "libqsl_peaks.so")                         # bench utility (include/qsl_peaks.h)
 
 QSL_F32, QSL_F64 = 0, 1
 QSL_NORMALIZE_FIRST, QSL_INTERP_FIRST = 0, 1
@@ -77,6 +78,20 @@ def lib():
         _lib.qsl_strerror.restype = C.c_char_p
         _lib.qsl_field_bytes.restype = C.c_longlong
     return _lib
+
+
+_peaks = None
+
+
+def peaks_lib():
+    """Loads libqsl_peaks.so: the roofline-denominator micro-kernels of bench.py (include/qsl_peaks.h), not part of libqsl."""
+    global _peaks
+    if _peaks is None:
+        if not os.path.exists(PEAKS_LIB_PATH):
+            from . import build as _build
+            _build.build()
+        _peaks = C.CDLL(PEAKS_LIB_PATH)
+    return _peaks
 
 
 def _check(rc: int, what: str):
@@ -436,17 +451,21 @@ def qsl_profile_trace_kernel_ms():
 
 
 def qsl_peak_fma(fp64: bool, reps: int = 5, stream=None) -> float:
-    """Measured FMA issue rate (FMA/s) of the plain FP pipe: DFMA if fp64 else FFMA."""
+    """Measured FMA issue rate (FMA/s) of the plain FP pipe: DFMA if fp64 else FFMA (libqsl_peaks.so, bench utility)."""
     _require_cuda()
     v = C.c_double(0.0)
-    _check(lib().qsl_peak_fma(C.c_int(1 if fp64 else 0), C.c_int(reps), C.byref(v), _stream_ptr(stream)), "qsl_peak_fma")
+    rc = peaks_lib().qsl_peak_fma(C.c_int(1 if fp64 else 0), C.c_int(reps), C.byref(v), _stream_ptr(stream))
+    if rc != 0:
+        raise QslError("qsl_peak_fma failed (code %d)" % rc)
     return v.value
 
 
 def qsl_peak_gather(bytes_per_sample: int, footprint_bytes: int, reps: int = 5, stream=None) -> float:
-    """Measured rate (samples/s) of divergent 16 B / 32 B gathers over a footprint of the given size."""
+    """Measured rate (samples/s) of divergent 16 B / 32 B gathers over a footprint of the given size (libqsl_peaks.so)."""
     _require_cuda()
     v = C.c_double(0.0)
-    _check(lib().qsl_peak_gather(C.c_int(bytes_per_sample), C.c_longlong(footprint_bytes), C.c_int(reps), C.byref(v),
-                                 _stream_ptr(stream)), "qsl_peak_gather")
+    rc = peaks_lib().qsl_peak_gather(C.c_int(bytes_per_sample), C.c_longlong(footprint_bytes), C.c_int(reps), C.byref(v),
+                                     _stream_ptr(stream))
+    if rc != 0:
+        raise QslError("qsl_peak_gather failed (code %d)" % rc)
     return v.value

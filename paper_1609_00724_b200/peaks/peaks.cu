@@ -3,11 +3,26 @@
 //   qsl_peak_fma     issue rate of the plain FP pipe (DFMA or FFMA), independent chains, no memory traffic
 //   qsl_peak_gather  rate of divergent 16-byte / 32-byte sample gathers (the tracer's load shape) over a footprint
 //                    that is L1-, L2- or HBM-resident
-// Both time themselves with CUDA events (warm-up + best of `reps`) and synchronise; they are bench utilities, not
-// part of the trace path.
-#include "qsl_internal.cuh"
+// Both time themselves with CUDA events (warm-up + best of `reps`) and synchronise.  They are bench utilities, not
+// part of the method: a library of their own (libqsl_peaks.so, include/qsl_peaks.h) that shares nothing with libqsl.
+#include <cuda_runtime.h>
 
-namespace qsl {
+#include "qsl_peaks.h"
+
+namespace qsl_peaks {
+
+static int sm_count()
+{
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1)
+        return 1;
+    return n;
+}
+
+#define PEAK_CUDA(call)                                   \
+    do {                                                  \
+        if ((call) != cudaSuccess) return QSL_PEAKS_ECUDA; \
+    } while (0)
 
 template <typename T>
 __global__ void __launch_bounds__(256) fma_peak_kernel(int iters, T seed, T *out)
@@ -62,8 +77,8 @@ template <typename F>
 static int time_best(int reps, double *best_ms, cudaStream_t s, F launch)
 {
     cudaEvent_t e0, e1;
-    QSL_CUDA(cudaEventCreate(&e0));
-    QSL_CUDA(cudaEventCreate(&e1));
+    PEAK_CUDA(cudaEventCreate(&e0));
+    PEAK_CUDA(cudaEventCreate(&e1));
     double best = 1e300;
     cudaError_t e = cudaSuccess;
     for (int r = 0; r < reps + 2 && e == cudaSuccess; ++r) {       // 2 warm-up launches
@@ -77,44 +92,44 @@ static int time_best(int reps, double *best_ms, cudaStream_t s, F launch)
         if (r >= 2 && ms < best) best = ms;
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
-    if (e != cudaSuccess) return record_cuda(e);
+    if (e != cudaSuccess) return QSL_PEAKS_ECUDA;
     *best_ms = best;
-    return QSL_OK;
+    return 0;
 }
 
-}  // namespace qsl
+}  // namespace qsl_peaks
 
-using namespace qsl;
+using namespace qsl_peaks;
 
 extern "C" int qsl_peak_fma(int fp64, int reps, double *fma_per_s, void *stream)
 {
-    if (!fma_per_s || reps < 1) return QSL_EINVAL;
+    if (!fma_per_s || reps < 1) return QSL_PEAKS_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     void *out = nullptr;
-    int rc = scratch_alloc(&out, 16, s);
-    if (rc != QSL_OK) return rc;
+    if (cudaMalloc(&out, 16) != cudaSuccess) return QSL_PEAKS_ENOMEM;
+    int rc = 0;
     const int iters = fp64 ? 2048 : 4096, threads = 256, blocks = sm_count() * 8;
     double ms = 0.0;
     rc = time_best(reps, &ms, s, [&] {
         if (fp64) fma_peak_kernel<double><<<blocks, threads, 0, s>>>(iters, 1.0, (double *)out);
         else fma_peak_kernel<float><<<blocks, threads, 0, s>>>(iters, 1.0f, (float *)out);
     });
-    scratch_free(out, s);
-    if (rc != QSL_OK) return rc;
+    cudaFree(out);
+    if (rc != 0) return rc;
     *fma_per_s = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
-    return QSL_OK;
+    return 0;
 }
 
 extern "C" int qsl_peak_gather(int bytes_per_sample, long long footprint_bytes, int reps, double *samples_per_s,
                                void *stream)
 {
     if (!samples_per_s || reps < 1 || (bytes_per_sample != 16 && bytes_per_sample != 32) ||
-        footprint_bytes < 4096) return QSL_EINVAL;
+        footprint_bytes < 4096) return QSL_PEAKS_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     void *buf = nullptr, *out = nullptr;
-    int rc = scratch_alloc(&buf, (size_t)footprint_bytes, s);
-    if (rc == QSL_OK) rc = scratch_alloc(&out, 16, s);
-    if (rc != QSL_OK) { scratch_free(buf, s); return rc; }
+    if (cudaMalloc(&buf, (size_t)footprint_bytes) != cudaSuccess) { cudaGetLastError(); return QSL_PEAKS_ENOMEM; }
+    if (cudaMalloc(&out, 16) != cudaSuccess) { cudaGetLastError(); cudaFree(buf); return QSL_PEAKS_ENOMEM; }
+    int rc = 0;
     cudaMemsetAsync(buf, 0, (size_t)footprint_bytes, s);
     unsigned long long n_samples = 1;                               // largest power of two that fits the footprint
     while (n_samples * 2 * (unsigned)bytes_per_sample <= (unsigned long long)footprint_bytes) n_samples *= 2;
@@ -125,8 +140,8 @@ extern "C" int qsl_peak_gather(int bytes_per_sample, long long footprint_bytes, 
         if (bytes_per_sample == 16) gather_peak_kernel<float4><<<blocks, threads, 0, s>>>((const float4 *)buf, mask, iters, (double *)out);
         else gather_peak_kernel<double4><<<blocks, threads, 0, s>>>((const double4 *)buf, mask, iters, (double *)out);
     });
-    scratch_free(buf, s); scratch_free(out, s);
-    if (rc != QSL_OK) return rc;
+    cudaFree(buf); cudaFree(out);
+    if (rc != 0) return rc;
     *samples_per_s = (double)blocks * threads * (double)iters / (ms * 1e-3);
-    return QSL_OK;
+    return 0;
 }

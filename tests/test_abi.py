@@ -10,8 +10,8 @@ import torch
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared_functions():
-    src = open(os.path.join(ROOT, "include", "qsl.h")).read()
+def _declared_functions(header="qsl.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(qsl_[a-z0-9_]+)\s*\(", src)))
 
@@ -26,6 +26,21 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(lib, n), n
     assert qsl.lib().qsl_compiled_arch() == 100
     assert qsl.lib().qsl_strerror(-1).decode() == "invalid argument"
+    # every header under include/ belongs to one of the two libraries
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["qsl.h", "qsl_peaks.h"]
+
+
+def test_peaks_library_is_separate_from_the_product_library():
+    """The roofline-denominator micro-kernels of bench.py live in libqsl_peaks.so (include/qsl_peaks.h): every symbol that
+    header declares is exported there, and libqsl.so exports none of them."""
+    import paper_1609_00724_b200 as qsl
+    names = _declared_functions("qsl_peaks.h")
+    assert names == ["qsl_peak_fma", "qsl_peak_gather"]
+    peaks, prod = ctypes.CDLL(qsl.PEAKS_LIB_PATH), ctypes.CDLL(qsl.LIB_PATH)
+    for n in names:
+        assert hasattr(peaks, n), n
+        assert not hasattr(prod, n), n
+    assert not any("peak" in n for n in _declared_functions())
 
 
 def test_struct_layouts_match_header_sizes():
