@@ -127,6 +127,32 @@ def test_edge_cases_status_caps_empty(kernel):
     compare_trace(g, c, lo, hi, frac=1.0, label="tail")
 
 
+@pytest.mark.parametrize("method", ["rk4", "ck45"])
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_non_finite_seeds_and_seeds_on_faces_edges_corners(kernel, method):
+    """Degenerate seeds: NaN / +-inf coordinates are SEED_OUTSIDE with NaN outputs (no lane may wander off with them), seeds
+    exactly on a face, an edge or a corner of the closed trace box (O2: box_lo <= x <= box_hi) start, leave through the
+    face the oracle names after the same number of steps and give the same L and Q."""
+    cfg = qi.make_config("cfg1", scale=0.25)
+    lo, hi = cfg["box_lo"], cfg["box_hi"]
+    seeds = np.array([[np.nan, 0, 0.5], [0, np.inf, 0.5], [0, 0, -np.inf], [lo[0], lo[1], lo[2]], [hi[0], hi[1], hi[2]],
+                      [lo[0], 0.1, 0.5], [0.2, hi[1], 0.0], [0.0, 0.0, hi[2]], [0.3, -0.2, 0.5], [lo[0], hi[1], 0.25],
+                      [np.nan, np.nan, np.nan], [hi[0], 0.0, lo[2]]])
+    seeds = np.concatenate([seeds, cfg["seeds"][:53]])                    # + ordinary lines around them in the same warps
+    kw = dict(method=qsl.QSL_CK45, tol=1e-4) if method == "ck45" else {}
+    g, c = run_both(cfg["grid"], cfg["B"], "f64", seeds, lo, hi, flags=kernel, **kw)
+    compare_trace(g, c, lo, hi, frac=1.0, label="degenerate seeds")
+    assert np.array_equal(g["status"], c["status"]) and np.array_equal(g["face_f"], c["face_f"])
+    assert np.array_equal(g["face_b"], c["face_b"])
+    bad = np.array([0, 1, 2, 10])
+    assert (c["status"][bad] & 1).all() and (g["status"][bad] & 1).all()       # SEED_OUTSIDE
+    for k in ("L", "q_perp", "q_bnd"):
+        assert np.isnan(g[k][bad]).all(), k
+        assert np.array_equal(np.isnan(g[k]), np.isnan(c[k])), k
+    assert np.isnan(g["end_f"][bad]).all() and np.isnan(g["end_b"][bad]).all()
+    assert (g["nsteps_f"][bad] == 0).all() and (g["nsteps_b"][bad] == 0).all()
+
+
 def test_bad_arguments_are_reported_not_crashed():
     cfg = qi.make_config("cfg1", scale=0.25)
     fg = gpu_field(cfg["grid"], cfg["B"], "f64", 0)
