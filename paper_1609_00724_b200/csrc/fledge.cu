@@ -105,66 +105,137 @@ __global__ void __launch_bounds__(FL_THREADS) fledge_dense_kernel(long long d0, 
     }
 }
 
+// Dense 2-D map, the kernel qsl_fledge_dense launches for ndim = 2.  Same strips of FL_VALID columns and the same
+// arithmetic (and bits) as fledge_dense_kernel<2>; what differs is the shape of the march (profiles/r2g: the kernel above
+// has one load in flight per warp and row, 13.7 of its 19 stall cycles per issue are long_scoreboard): one warp per CTA, so
+// that task index and bounds are provably warp-uniform (no WARPSYNC pair around the shuffles, loop control on the uniform
+// datapath), 32-bit index arithmetic with one moving pointer, and the rows taken FL2_GROUP at a time - their loads are all
+// requested before the first of them is used.
+#ifndef QSL_FL2_ROWS
+#define QSL_FL2_ROWS 64
+#endif
+#ifndef QSL_FL2_GROUP
+#define QSL_FL2_GROUP 8
+#endif
+constexpr int FL2_ROWS = QSL_FL2_ROWS, FL2_GROUP = QSL_FL2_GROUP;
+__global__ void __launch_bounds__(32, 32) fledge_dense2_kernel(int d0, int d1, int rows, const double *__restrict__ L,
+                                                              double *__restrict__ S)
+{
+    constexpr int G = FL2_GROUP;
+    const int lane = threadIdx.x;
+    const int strips = (d0 + FL_VALID - 1) / FL_VALID;
+    const int bands = (d1 + rows - 1) / rows;                            // rows: rows per band, a multiple of G
+    const long long tasks = (long long)strips * bands;
+    for (long long t = blockIdx.x; t < tasks; t += gridDim.x) {
+        const int strip = (int)(t % strips), band = (int)(t / strips);
+        const int col = strip * FL_VALID - 1 + lane;                     // lane 0 / 31 = halo
+        const int cc = min(max(col, 0), d0 - 1);                         // edge replication
+        const int y0 = band * rows, y1 = min(y0 + rows, d1);
+        const bool mine = lane >= 1 && lane <= FL_VALID && col < d0;
+        const double *__restrict__ q = L + (long long)y0 * d0 + cc;      // row y of the lane's column
+        double *__restrict__ so = S + (long long)y0 * d0 + col;
+        double w[G + 2];                                                 // rows y - 1, y, y + 1 .. y + G
+        w[0] = __ldg(y0 > 0 ? q - d0 : q);
+        w[1] = __ldg(q);
+        for (int y = y0; y < y1; y += G) {
+#pragma unroll
+            for (int k = 0; k < G; ++k) {                                // row y + k + 1, clamped to the last row
+                q += y + k + 1 < d1 ? d0 : 0;
+                w[k + 2] = __ldg(q);
+            }
+#pragma unroll
+            for (int k = 0; k < G; ++k) {
+                const double A = (w[k] + w[k + 2]) + 2.0 * w[k + 1], B = w[k + 2] - w[k];
+                double s = combine_lanes<2>(A, B, 0.0);
+                if (!isfinite(w[k + 1])) s = __longlong_as_double(0x7ff8000000000000ll);
+                if (mine && y + k < y1) so[(long long)k * d0] = s;
+            }
+            so += (long long)G * d0;
+            w[0] = w[G]; w[1] = w[G + 1];
+        }
+    }
+}
+
 // Dense 3-D map, each value loaded once (+ halo): a warp owns a strip of FL_VALID columns x a band of FL3_ROWS rows and
 // marches along axis 2 over a chunk of FL3_PLANES planes, holding the raw values of its column for the rows of the band
 // (+ one halo row on either side) of the planes z-1, z, z+1 in registers.  Per plane step: FL3_ROWS + 2 loads per lane
-// for FL3_ROWS outputs instead of 3 per output.  Measured on a 512 x 512 x 256 map: 8 rows (168 registers) 0.48 ms,
-// 4 rows at 5 CTAs / SM 0.46 ms, 2 rows at 8 CTAs / SM (64 registers) 0.40 ms, the row-marching kernel 0.45 ms: the
-// kernel wants resident warps more than it wants fewer loads (the repeated loads hit L2).  The folds are taken in the order of the
-// kernel above (axis 2, then axis 1, then axis 0 across lanes), so both give the same bits.
+// for FL3_ROWS outputs instead of 3 per output.  Measured on a 512 x 512 x 256 map, 128-thread CTAs with 64-bit index
+// arithmetic: 8 rows (168 registers) 0.48 ms, 4 rows at 5 CTAs / SM 0.46 ms, 2 rows at 8 CTAs / SM (64 registers) 0.40 ms,
+// the row-marching kernel 0.45 ms: the kernel wants resident warps more than it wants fewer loads (the repeated loads hit
+// L2).  The form below (2 rows, single-warp CTAs, 32-bit indices, moving pointers, rotating windows): 0.294 ms = 0.56 of
+// the copy rate (profiles/r2g).  The folds are taken in the order of the kernel above (axis 2, then axis 1, then axis 0
+// across lanes), so both give the same bits.
 #ifndef QSL_FL3_ROWS
 #define QSL_FL3_ROWS 2
 #endif
 #ifndef QSL_FL3_MINB
-#define QSL_FL3_MINB 8
+#define QSL_FL3_MINB 32
 #endif
 constexpr int FL3_ROWS = QSL_FL3_ROWS;
 constexpr int FL3_PLANES = 64;
-__global__ void __launch_bounds__(FL_THREADS, QSL_FL3_MINB) fledge_dense3_kernel(long long d0, long long d1, long long d2,
+__global__ void __launch_bounds__(32, QSL_FL3_MINB) fledge_dense3_kernel(int d0, int d1, int d2,
                                                                    const double *__restrict__ L, double *__restrict__ S)
 {
+    // One warp per CTA: the task index then depends on blockIdx alone and the compiler sees that the march is
+    // warp-uniform (task loop and bounds on the uniform datapath, no WARPSYNC / ENDCOLLECTIVE pair around every shuffle).
+    // All per-task index arithmetic in 32 bits (the launcher checks that a plane has fewer than 2^31 values); inside the
+    // march only pointers move, by one plane per step, and the three plane windows rotate by name (three steps per
+    // trip) instead of being copied: the first version spent 55 % of its instructions on 64-bit index arithmetic, the
+    // bounds tests of the rows, register moves and spills (profiles/r2g).
     constexpr int R = FL3_ROWS;
-    const unsigned lane = threadIdx.x & 31u;
-    const long long strips = (d0 + FL_VALID - 1) / FL_VALID;
-    const long long bands = (d1 + R - 1) / R;
-    const long long chunks = (d2 + FL3_PLANES - 1) / FL3_PLANES;
-    const long long tasks = strips * bands * chunks;
-    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long t = (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); t < tasks; t += warps) {
-        const long long strip = t % strips, rest = t / strips;
-        const long long band = rest % bands, chunk = rest / bands;
-        const long long col = strip * FL_VALID - 1 + lane;               // lane 0 / 31 = halo
-        const long long cc = min(max(col, 0ll), d0 - 1);                 // edge replication
-        const long long y0 = band * R, z0 = chunk * FL3_PLANES, z1 = min(z0 + FL3_PLANES, d2);
-        long long row[R + 2];                                            // element offsets of the (clamped) rows
-#pragma unroll
-        for (int r = 0; r < R + 2; ++r) row[r] = min(max(y0 - 1 + r, 0ll), d1 - 1) * d0 + cc;
-        const long long plane = d1 * d0;
+    const int lane = threadIdx.x;
+    const int strips = (d0 + FL_VALID - 1) / FL_VALID;
+    const int bands = (d1 + R - 1) / R;
+    const int chunks = (d2 + FL3_PLANES - 1) / FL3_PLANES;
+    const long long tasks = (long long)strips * bands * chunks;
+    const long long plane = (long long)d1 * d0;
+    for (long long t = blockIdx.x; t < tasks; t += gridDim.x) {
+        const int strip = (int)(t % strips);
+        const int rest = (int)(t / strips);
+        const int band = rest % bands, chunk = rest / bands;
+        const int col = strip * FL_VALID - 1 + lane;                     // lane 0 / 31 = halo
+        const int cc = min(max(col, 0), d0 - 1);                         // edge replication
+        const int y0 = band * R, z0 = chunk * FL3_PLANES, z1 = min(z0 + FL3_PLANES, d2);
+        const double *__restrict__ row[R + 2];                           // the (clamped) rows of the plane loaded last
         double vm[R + 2], vc[R + 2], vp[R + 2];
         {
-            const double *__restrict__ pm = L + max(z0 - 1, 0ll) * plane, *__restrict__ pc = L + z0 * plane;
+            const double *__restrict__ pm = L + (long long)max(z0 - 1, 0) * plane + cc;
+            const long long up = z0 > 0 ? plane : 0;                     // plane z0 - 1 -> plane z0
 #pragma unroll
-            for (int r = 0; r < R + 2; ++r) { vm[r] = __ldg(pm + row[r]); vc[r] = __ldg(pc + row[r]); }
+            for (int r = 0; r < R + 2; ++r) {
+                const double *__restrict__ q = pm + (long long)min(max(y0 - 1 + r, 0), d1 - 1) * d0;
+                vm[r] = __ldg(q); vc[r] = __ldg(q + up);
+                row[r] = q + up;
+            }
         }
-        for (long long z = z0; z < z1; ++z) {
-            const double *__restrict__ pp = L + min(z + 1, d2 - 1) * plane;
+        const bool mine = lane >= 1 && lane <= FL_VALID && col < d0;
+        double *__restrict__ so = S + (long long)z0 * plane + (long long)y0 * d0 + col;
+        // one plane step: a = plane z - 1, b = plane z, c <- plane z + 1
+        auto plane_step = [&](int z, const double *a, const double *b, double *c) {
+            const long long step = z + 1 < d2 ? plane : 0;               // the plane above the last one is the last one
 #pragma unroll
-            for (int r = 0; r < R + 2; ++r) vp[r] = __ldg(pp + row[r]);
+            for (int r = 0; r < R + 2; ++r) { row[r] += step; c[r] = __ldg(row[r]); }
             double P[R + 2], D[R + 2];
 #pragma unroll
-            for (int r = 0; r < R + 2; ++r) { P[r] = (vm[r] + vp[r]) + 2.0 * vc[r]; D[r] = vp[r] - vm[r]; }
+            for (int r = 0; r < R + 2; ++r) { P[r] = (a[r] + c[r]) + 2.0 * b[r]; D[r] = c[r] - a[r]; }
 #pragma unroll
             for (int r = 1; r <= R; ++r) {
-                const long long y = y0 + r - 1;
-                if (y < d1) {                                            // warp-uniform
-                    const double A = (P[r - 1] + P[r + 1]) + 2.0 * P[r], B = P[r + 1] - P[r - 1], C = (D[r - 1] + D[r + 1]) + 2.0 * D[r];
-                    double s = combine_lanes<3>(A, B, C);
-                    if (!isfinite(vc[r])) s = __longlong_as_double(0x7ff8000000000000ll);
-                    if (lane >= 1 && lane <= FL_VALID && col < d0) S[(z * d1 + y) * d0 + col] = s;
-                }
+                const double A = (P[r - 1] + P[r + 1]) + 2.0 * P[r], B = P[r + 1] - P[r - 1], C = (D[r - 1] + D[r + 1]) + 2.0 * D[r];
+                double s = combine_lanes<3>(A, B, C);
+                if (!isfinite(b[r])) s = __longlong_as_double(0x7ff8000000000000ll);
+                if (mine && y0 + r - 1 < d1) so[(long long)(r - 1) * d0] = s;
             }
-#pragma unroll
-            for (int r = 0; r < R + 2; ++r) { vm[r] = vc[r]; vc[r] = vp[r]; }
+            so += plane;
+        };
+        int z = z0;
+        for (; z + 3 <= z1; z += 3) {
+            plane_step(z, vm, vc, vp);
+            plane_step(z + 1, vc, vp, vm);
+            plane_step(z + 2, vp, vm, vc);
+        }
+        if (z < z1) {
+            plane_step(z, vm, vc, vp);
+            if (z + 1 < z1) plane_step(z + 1, vc, vp, vm);
         }
     }
 }
@@ -273,13 +344,20 @@ extern "C" int qsl_fledge_dense(int ndim, const long long dims[3], const double 
     const long long cap = (long long)sm_count() * 32;      // a multiple of the SM count; warps stride over the tasks
     if (blocks > cap) blocks = cap;
     count_launch();
-    if (ndim == 2) fledge_dense_kernel<2><<<(unsigned)blocks, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
-    else if (d2 >= 8) {
+    if (ndim == 2 && d0 < (1ll << 31) - 64 && d1 < (1ll << 31) - 64) {
+        // rows per band: FL2_ROWS on a large map; fewer (a multiple of the group, at least two groups) on a map too small
+        // to give every SM its 32 single-warp CTAs otherwise
+        long long rows = FL2_ROWS;
+        const long long want = (long long)sm_count() * 32;
+        while (rows > 2 * FL2_GROUP && strips * ((d1 + rows - 1) / rows) < want) rows >>= 1;
+        const long long tasks2 = strips * ((d1 + rows - 1) / rows), cap2 = want * 8;
+        fledge_dense2_kernel<<<(unsigned)(tasks2 < cap2 ? tasks2 : cap2), 32, 0, s>>>((int)d0, (int)d1, (int)rows, L, S);
+    } else if (ndim == 2) fledge_dense_kernel<2><<<(unsigned)blocks, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
+    else if (d2 >= 8 && d0 * d1 < (1ll << 31) && d2 < (1ll << 31)) {
         // deep enough along axis 2 for the plane-marching kernel to amortise its two halo planes
         const long long tasks3 = strips * ((d1 + FL3_ROWS - 1) / FL3_ROWS) * ((d2 + FL3_PLANES - 1) / FL3_PLANES);
-        long long blocks3 = (tasks3 + wpb - 1) / wpb;
-        if (blocks3 > cap) blocks3 = cap;
-        fledge_dense3_kernel<<<(unsigned)blocks3, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
+        const long long cap3 = (long long)sm_count() * QSL_FL3_MINB * 8;   // single-warp CTAs, a few waves of them
+        fledge_dense3_kernel<<<(unsigned)(tasks3 < cap3 ? tasks3 : cap3), 32, 0, s>>>((int)d0, (int)d1, (int)d2, L, S);
     } else fledge_dense_kernel<3><<<(unsigned)blocks, FL_THREADS, 0, s>>>(d0, d1, d2, L, S);
     QSL_CUDA(cudaGetLastError());
     return QSL_OK;

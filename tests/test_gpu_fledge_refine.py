@@ -19,7 +19,11 @@ def _cuda(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-@pytest.mark.parametrize("shape", [(13, 17), (1, 9), (8, 1), (64, 95), (6, 7, 9), (5, 4, 1), (2, 2, 2), (33, 31, 70), (1, 1, 1)])
+@pytest.mark.parametrize("shape", [(13, 17), (1, 9), (8, 1), (64, 95), (6, 7, 9), (5, 4, 1), (2, 2, 2), (33, 31, 70), (1, 1, 1),
+                                   # bands / groups / plane chunks of the dense kernels with ragged ends: 2-D rows per band
+                                   # 16 .. 64 in groups of 8, strips of 30 columns; 3-D bands of 2 rows, chunks of 64 planes
+                                   (65, 61), (129, 30), (17, 31), (300, 1), (2, 200), (9, 3, 2), (8, 1, 1), (67, 5, 33),
+                                   (130, 2, 61), (64, 3, 30), (65, 7, 1)])
 def test_fledge_dense_matches_oracle(shape):
     rng = np.random.default_rng(30)
     V = rng.uniform(0.1, 3.0, size=shape)
