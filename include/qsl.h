@@ -28,6 +28,7 @@ extern "C" {
 #define QSL_ENOMEM  (-2)   /* device or host allocation failed                                                    */
 #define QSL_ECUDA   (-3)   /* a CUDA runtime call failed (qsl_last_cuda_error() gives the cudaError_t)             */
 #define QSL_ERANGE  (-4)   /* a size exceeds what the implementation indexes (e.g. > 2^31 - 1 nodes per axis)      */
+#define QSL_ETOOBIG (-5)   /* the input exceeds the fixed scratch of a *_noalloc entry point (use the pooled one)   */
 const char *qsl_strerror(int code);
 int qsl_last_cuda_error(void);
 /* Library version and the SM architecture the kernels were compiled for (e.g. 100 for sm_100a). */
@@ -186,6 +187,24 @@ int qsl_select(long long n, const double *S, double p, double *tau, void *stream
 int qsl_refine(int ndim, int level, long long n, const unsigned int *coords, const double *S, const double *tau,
                const qsl_lattice *lat, long long capacity, unsigned int *child_coords, double *child_seeds,
                long long *child_base, long long *n_children, void *stream);
+
+/* qsl_refine for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc).  Same operation, same kernels and the same bits in child_coords / child_seeds / child_base as
+ * qsl_refine (reading A11), with two differences:
+ *  - it calls no cudaMalloc / cudaMallocAsync / cudaFree and no allocating library routine: the per-tile counts of the
+ *    stream compaction live in a file-scope device array of the library (256 KiB, held by every GPU that loads libqsl
+ *    until the process exits), which limits the call to n <= QSL_REFINE_NOALLOC_MAX_CELLS cells (cfg5's dense level
+ *    0 just fits); a larger n returns QSL_ETOOBIG and launches nothing - use qsl_refine;
+ *  - n_children is a DEVICE pointer (1 long long) written on the stream; the call never synchronises.  If the count
+ *    exceeds `capacity`, nothing beyond capacity was written (no error can be reported: compare on the device or
+ *    after the caller's own synchronisation).
+ * All calls on a device share the scratch array and it keeps the last call's contents; nothing in it needs clearing
+ * (every word a call reads it has written first).  Calls that overlap on the GPU (two streams) race on it: serialise
+ * them.  Errors: QSL_EINVAL, QSL_ERANGE (as qsl_refine), QSL_ETOOBIG, QSL_ECUDA.                                      */
+#define QSL_REFINE_NOALLOC_MAX_CELLS 67108864LL
+int qsl_refine_noalloc(int ndim, int level, long long n, const unsigned int *coords, const double *S, const double *tau,
+                       const qsl_lattice *lat, long long capacity, unsigned int *child_coords, double *child_seeds,
+                       long long *child_base, long long *n_children, void *stream);
 
 /* ---- test hook ------------------------------------------------------------------------------------------------- */
 /* Stable ascending sort of n (key, value) pairs (DEVICE, in place) on the low key_bits (1..32) of the keys: the

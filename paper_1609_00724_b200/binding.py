@@ -315,6 +315,39 @@ def qsl_refine(lattice, level: int, coords, S: torch.Tensor, tau: torch.Tensor, 
     return cc[: m.value], cs[: m.value], cb
 
 
+QSL_REFINE_NOALLOC_MAX_CELLS = 67108864      # include/qsl.h
+
+
+def qsl_refine_noalloc(lattice, level: int, coords, S: torch.Tensor, tau: torch.Tensor, child_coords: torch.Tensor,
+                       child_seeds: torch.Tensor, child_base, n_children: torch.Tensor, *, stream=None) -> None:
+    """qsl_refine without any allocation and without a host synchronisation (include/qsl.h: qsl_refine_noalloc): the
+    caller passes every buffer - child_coords CUDA int32 (capacity, ndim), child_seeds CUDA float64 (capacity, 3),
+    child_base CUDA int64 (n,) or None, n_children CUDA int64 (1,), written on the stream.  n is limited to
+    QSL_REFINE_NOALLOC_MAX_CELLS (QslError beyond it); calls that overlap on the GPU race on the library's fixed scratch."""
+    _require_cuda()
+    lat = make_lattice(lattice)
+    ndim = int(lattice.ndim)
+    n = int(S.numel())
+    cap = int(child_coords.shape[0]) if child_coords is not None else 0
+    ok = (child_coords is None or (child_coords.is_cuda and child_coords.dtype == torch.int32 and child_coords.is_contiguous()
+                                   and child_coords.numel() == cap * ndim))
+    ok = ok and (child_seeds is None or (child_seeds.is_cuda and child_seeds.dtype == torch.float64
+                                         and child_seeds.is_contiguous() and child_seeds.numel() == cap * 3))
+    ok = ok and (child_base is None or (child_base.is_cuda and child_base.dtype == torch.int64 and child_base.numel() == n))
+    ok = ok and n_children.is_cuda and n_children.dtype == torch.int64 and n_children.numel() == 1
+    if not ok:
+        raise QslError("qsl_refine_noalloc: outputs must be contiguous CUDA tensors of the documented types and sizes")
+    cptr = None
+    if coords is not None:
+        if coords.dtype != torch.int32 or not coords.is_cuda or coords.numel() != n * ndim:
+            raise QslError("coords must be CUDA int32 of n*ndim values")
+        cptr = C.c_void_p(coords.data_ptr())
+    _check(lib().qsl_refine_noalloc(C.c_int(ndim), C.c_int(level), C.c_longlong(n), cptr, _dev_f64(S.reshape(-1), "S"),
+                                    _dev_f64(tau, "tau"), C.byref(lat), C.c_longlong(cap), _p(child_coords), _p(child_seeds),
+                                    _p(child_base), C.c_void_p(n_children.data_ptr()), _stream_ptr(stream)),
+           "qsl_refine_noalloc")
+
+
 # ---- the paper's Hilbert-curve refinement (PAPER.md:194-206; include/qsl.h) --------------------------------------------
 def _p(t):
     return C.c_void_p(t.data_ptr()) if t is not None and t.numel() else None

@@ -180,6 +180,7 @@ const char *qsl_strerror(int code)
         case QSL_ENOMEM: return "out of memory";
         case QSL_ECUDA: return "CUDA runtime error (see qsl_last_cuda_error)";
         case QSL_ERANGE: return "size out of range";
+        case QSL_ETOOBIG: return "input larger than the fixed scratch of this no-allocation entry point";
         default: return "unknown error";
     }
 }

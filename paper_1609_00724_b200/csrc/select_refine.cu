@@ -263,3 +263,89 @@ extern "C" int qsl_refine(int ndim, int level, long long n, const unsigned int *
     if (*n_children > capacity) return QSL_ERANGE;
     return QSL_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// qsl_refine for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+// the per-tile counts of the compaction live in a file-scope device array instead of the stream-ordered pool, and the
+// child count stays on the device (no host synchronisation).  Same kernels, same arithmetic, same outputs as qsl_refine.
+//
+// The array is part of the library image: every GPU that loads libqsl holds its 256 KiB (+ 256 B) until the process
+// exits.  All calls on a device share it and it keeps the last call's contents; nothing in it has to start at zero
+// (refine_count_kernel writes every tile count of the call, scan_single_block the total, before either is read).  Two
+// calls that overlap on the GPU (different streams) race on it: serialise them.
+namespace qsl {
+
+constexpr long long RF_NOALLOC_MAX_TILES = QSL_REFINE_NOALLOC_MAX_CELLS / RF_TILE;
+static_assert(QSL_REFINE_NOALLOC_MAX_CELLS % RF_TILE == 0, "the limit is a whole number of tiles");
+// [0, MAX_TILES): tile counts, then their exclusive scan; [MAX_TILES]: the number of flagged cells
+static __device__ __align__(256) unsigned long long g_refine_noalloc_scratch[RF_NOALLOC_MAX_TILES + 32];
+
+__global__ void refine_noalloc_total_kernel(const unsigned long long *__restrict__ flagged, int ndim,
+                                            long long *__restrict__ n_children)
+{
+    *n_children = (long long)(*flagged << ndim);
+}
+
+// Device address of the array on the current device.  In host code the array's name is a host-side stand-in, not a
+// device address: the address comes from cudaGetSymbolAddress, asked once per device with that device current.
+static int refine_noalloc_scratch(unsigned long long **out)
+{
+    static unsigned long long *cache[64];
+    int dev = 0;
+    QSL_CUDA(cudaGetDevice(&dev));
+    unsigned long long *ptr = dev >= 0 && dev < 64 ? cache[dev] : nullptr;
+    if (!ptr) {
+        QSL_CUDA(cudaGetSymbolAddress((void **)&ptr, g_refine_noalloc_scratch));
+        if (!ptr) return QSL_ECUDA;
+        if (dev >= 0 && dev < 64) cache[dev] = ptr;
+    }
+    *out = ptr;
+    return QSL_OK;
+}
+
+}  // namespace qsl
+
+extern "C" int qsl_refine_noalloc(int ndim, int level, long long n, const unsigned int *coords, const double *S,
+                                  const double *tau, const qsl_lattice *lat, long long capacity, unsigned int *child_coords,
+                                  double *child_seeds, long long *child_base, long long *n_children, void *stream)
+{
+    if ((ndim != 2 && ndim != 3) || level < 0 || level > 14 || n < 0 || !lat || !tau || !n_children || capacity < 0) return QSL_EINVAL;
+    if (n > 0 && (!S || (capacity > 0 && (!child_coords || !child_seeds)))) return QSL_EINVAL;
+    if (lat->ndim != ndim) return QSL_EINVAL;
+    if (!coords) {
+        const long long dense = lat->n[0] * lat->n[1] * (ndim == 3 ? lat->n[2] : 1);
+        if (level != 0 || n != dense) return QSL_EINVAL;
+    }
+    for (int d = 0; d < ndim; ++d)
+        if (lat->n[d] < 1 || (lat->n[d] << (level + 1)) > 0xffffffffll) return QSL_ERANGE;
+    if (n > QSL_REFINE_NOALLOC_MAX_CELLS) return QSL_ETOOBIG;       // the fixed scratch array holds no more tile counts
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n == 0) {
+        QSL_CUDA(cudaMemsetAsync(n_children, 0, sizeof(long long), s));
+        return QSL_OK;
+    }
+    unsigned long long *tiles = nullptr;
+    int rc = refine_noalloc_scratch(&tiles);
+    if (rc != QSL_OK) return rc;
+    unsigned long long *total = tiles + RF_NOALLOC_MAX_TILES;
+    RefineArgs A;
+    A.ndim = ndim; A.level = level; A.n = n; A.coords = coords; A.S = S; A.tau = tau;
+    for (int d = 0; d < 3; ++d) {
+        A.n0[d] = d < ndim ? lat->n[d] : 1;
+        A.origin[d] = lat->origin[d];
+        A.e[0][d] = lat->e0[d]; A.e[1][d] = lat->e1[d]; A.e[2][d] = lat->e2[d];
+    }
+    A.capacity = capacity; A.child_coords = child_coords; A.child_seeds = child_seeds; A.child_base = child_base;
+    const long long ntiles = (n + RF_TILE - 1) / RF_TILE;
+    count_launch();
+    refine_count_kernel<<<(unsigned)ntiles, RF_THREADS, 0, s>>>(n, S, tau, tiles);
+    count_launch();
+    scan_single_block<<<1, 1024, 0, s>>>(ntiles, tiles, total);
+    count_launch();
+    if (ndim == 2) refine_emit_kernel<2><<<(unsigned)ntiles, RF_THREADS, 0, s>>>(A, tiles);
+    else refine_emit_kernel<3><<<(unsigned)ntiles, RF_THREADS, 0, s>>>(A, tiles);
+    count_launch();
+    refine_noalloc_total_kernel<<<1, 1, 0, s>>>(total, ndim, n_children);
+    QSL_CUDA(cudaGetLastError());
+    return QSL_OK;
+}
