@@ -118,11 +118,17 @@ __global__ void __launch_bounds__(RF_THREADS) refine_count_kernel(long long n, c
     if (threadIdx.x == 0) tile_counts[blockIdx.x] = total;
 }
 
+// The children of a tile form one contiguous run of the output (tile offset << NDIM onwards), so the block writes them
+// cooperatively - one thread per coordinate word, then one thread per child for its position - instead of every flagged
+// cell's thread writing its own 2^NDIM children (36 B each) at a stride: neighbouring threads store to neighbouring
+// addresses.  The arithmetic per child (one IEEE division per axis, the fma chain) is unchanged.
 template <int NDIM>
 __global__ void __launch_bounds__(RF_THREADS) refine_emit_kernel(const RefineArgs A, const unsigned long long *__restrict__ tile_offs)
 {
     __shared__ unsigned char s_flag[RF_TILE];
-    __shared__ long long s_first[RF_TILE];          // first child of the cell, or -1
+    __shared__ unsigned short s_rank[RF_TILE];      // rank of a flagged cell among the flagged cells of the tile
+    __shared__ unsigned short s_cell[RF_TILE];      // the r-th flagged cell of the tile
+    __shared__ uint32_t s_c[RF_TILE][NDIM];         // and its lattice coordinates
     const double t = *A.tau;
     const long long base = (long long)blockIdx.x * RF_TILE;
     // flags of the tile, loaded with coalesced accesses
@@ -137,50 +143,60 @@ __global__ void __launch_bounds__(RF_THREADS) refine_emit_kernel(const RefineArg
 #pragma unroll
     for (int k = 0; k < RF_ITEMS; ++k) mine += s_flag[threadIdx.x * RF_ITEMS + k];
     unsigned long long total;
-    unsigned long long rank = block_exclusive_scan(mine, total) + tile_offs[blockIdx.x];
+    unsigned rank = (unsigned)block_exclusive_scan(mine, total);
+    const long long first0 = (long long)tile_offs[blockIdx.x] << NDIM;          // first child of the tile
 #pragma unroll
     for (int k = 0; k < RF_ITEMS; ++k) {
         const int e = threadIdx.x * RF_ITEMS + k;
-        s_first[e] = s_flag[e] ? (long long)(rank++) << NDIM : -1ll;
+        if (s_flag[e]) { s_rank[e] = (unsigned short)rank; s_cell[rank] = (unsigned short)e; ++rank; }
     }
     __syncthreads();
+    const int flagged = (int)total;
+    if (A.child_base) {
+        for (int e = threadIdx.x; e < RF_TILE && base + e < A.n; e += RF_THREADS)
+            A.child_base[base + e] = s_flag[e] ? first0 + ((long long)s_rank[e] << NDIM) : -1ll;
+    }
+    // coordinates of the flagged cells
+    for (int r = threadIdx.x; r < flagged; r += RF_THREADS) {
+        const long long i = base + s_cell[r];
+        if (A.coords) {
+#pragma unroll
+            for (int d = 0; d < NDIM; ++d) s_c[r][d] = A.coords[i * NDIM + d];
+        } else {
+            s_c[r][0] = (uint32_t)(i % A.n0[0]);
+            s_c[r][1] = (uint32_t)((i / A.n0[0]) % A.n0[1]);
+            if (NDIM == 3) s_c[r][NDIM - 1] = (uint32_t)(i / (A.n0[0] * A.n0[1]));
+        }
+    }
+    __syncthreads();
+    // children that fit the caller's buffers (the host reports QSL_ERANGE if some did not)
+    long long room = A.capacity - first0;
+    if (room <= 0) return;
+    const int children = (int)min((long long)flagged << NDIM, room);
+    // child coordinates: one thread per 32-bit word of the run
+    for (int w = threadIdx.x; w < children * NDIM; w += RF_THREADS) {
+        const int j = w / NDIM, d = w - j * NDIM;
+        A.child_coords[first0 * NDIM + w] = 2u * s_c[j >> NDIM][d] + (uint32_t)(((j & ((1 << NDIM) - 1)) >> d) & 1);
+    }
     double inv_den[3];
 #pragma unroll
     for (int d = 0; d < NDIM; ++d) inv_den[d] = (double)(A.n0[d] << (A.level + 1));
-    for (int k = 0; k < RF_ITEMS; ++k) {
-        const int e = k * RF_THREADS + threadIdx.x;
-        const long long i = base + e;
-        if (i >= A.n) break;
-        const long long first = s_first[e];
-        if (A.child_base) A.child_base[i] = first;
-        if (first < 0) continue;
-        uint32_t c[3];
-        if (A.coords) {
+    // child positions: one thread per child
+    for (int j = threadIdx.x; j < children; j += RF_THREADS) {
+        const int r = j >> NDIM, ch = j & ((1 << NDIM) - 1);
+        double w[3] = { 0.0, 0.0, 0.0 };
 #pragma unroll
-            for (int d = 0; d < NDIM; ++d) c[d] = A.coords[i * NDIM + d];
-        } else {
-            c[0] = (uint32_t)(i % A.n0[0]);
-            c[1] = (uint32_t)((i / A.n0[0]) % A.n0[1]);
-            c[2] = (uint32_t)(i / (A.n0[0] * A.n0[1]));
+        for (int d = 0; d < NDIM; ++d) {
+            const uint32_t cc = 2u * s_c[r][d] + (uint32_t)((ch >> d) & 1);
+            w[d] = __ddiv_rn((double)cc + 0.5, inv_den[d]);      // one IEEE division, as in the definition
         }
+        double *__restrict__ o = A.child_seeds + 3 * (first0 + j);
 #pragma unroll
-        for (int ch = 0; ch < (1 << NDIM); ++ch) {
-            const long long m = first + ch;
-            if (m >= A.capacity) break;
-            double w[3] = { 0.0, 0.0, 0.0 };
-#pragma unroll
-            for (int d = 0; d < NDIM; ++d) {
-                const uint32_t cc = 2u * c[d] + (uint32_t)((ch >> d) & 1);
-                A.child_coords[m * NDIM + d] = cc;
-                w[d] = __ddiv_rn((double)cc + 0.5, inv_den[d]);      // one IEEE division, as in the definition
-            }
-#pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                double pos = __fma_rn(w[0], A.e[0][q], A.origin[q]);
-                pos = __fma_rn(w[1], A.e[1][q], pos);
-                if (NDIM == 3) pos = __fma_rn(w[2], A.e[2][q], pos);
-                A.child_seeds[3 * m + q] = pos;
-            }
+        for (int q = 0; q < 3; ++q) {
+            double pos = __fma_rn(w[0], A.e[0][q], A.origin[q]);
+            pos = __fma_rn(w[1], A.e[1][q], pos);
+            if (NDIM == 3) pos = __fma_rn(w[2], A.e[2][q], pos);
+            o[q] = pos;
         }
     }
 }
