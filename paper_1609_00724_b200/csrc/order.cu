@@ -5,7 +5,7 @@
 //
 // The sort is a hand-written stable LSD radix sort on 32- or 64-bit keys (8-bit digits): per pass a per-tile digit
 // histogram, one exclusive scan of the (digit-major) count table, and a scatter that sorts a tile of 2048 keys by the
-// digit in shared memory (warps rank their keys with __match_any_sync) and writes it out run by run.
+// digit in shared memory (warps rank their keys with warp votes) and writes it out run by run.
 #include "qsl_internal.cuh"
 #include "scan.cuh"
 
@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(long long n, co
 
 // Scatter of one pass.  A block owns a tile of SORT_TILE consecutive keys (warp w the w-th eighth of it, 32 keys per
 // round, so that index order = (warp, round, lane) order and the ranking below is stable):
-//   1. every warp ranks its keys among the keys of the same digit it has seen so far (__match_any_sync per round + a
+//   1. every warp ranks its keys among the keys of the same digit it has seen so far (warp votes per round + a
 //      running per-warp digit counter in shared memory);
 //   2. thread d adds up the eight warp counters of digit d (-> the warps' bases inside the digit) and a block-wide
 //      exclusive scan of the digit totals gives the place of digit d inside the tile;
@@ -90,8 +90,27 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(long long n, co
 //      tile), so neighbouring threads store to neighbouring addresses within a digit's run (16 keys on average for
 //      uniformly distributed digits, whole rows for the nearly sorted keys of a seed lattice) instead of 32 unrelated
 //      sectors per store instruction.
+// The live lanes of the warp that hold the same 8-bit digit as this lane: nine warp votes and their masks on the integer
+// pipe.  __match_any_sync gives the same set in one instruction, but MATCH runs on the address-divergence unit, which
+// takes one step per distinct value of the warp: with it the scatter kernel sat at 82 % of that unit's issue rate
+// (profiles/r2h), 565 us per pass of 6.7e7 random keys.
+__device__ __forceinline__ unsigned same_digit_lanes(uint32_t digit, bool live)
+{
+    unsigned peers = __ballot_sync(0xffffffffu, live);
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const bool bit = (digit >> b) & 1u;
+        const unsigned v = __ballot_sync(0xffffffffu, bit);
+        peers &= bit ? v : ~v;
+    }
+    return peers;
+}
+
+#ifndef QSL_SORT_MINB
+#define QSL_SORT_MINB 1
+#endif
 template <typename K>
-__global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(long long n, const K *__restrict__ keys,
+__global__ void __launch_bounds__(SORT_THREADS, QSL_SORT_MINB) sort_scatter_kernel(long long n, const K *__restrict__ keys,
                                                                     const uint32_t *__restrict__ vals, int shift, long long n_tiles,
                                                                     const unsigned long long *__restrict__ offsets,
                                                                     K *__restrict__ keys_out, uint32_t *__restrict__ vals_out)
@@ -117,8 +136,8 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(long long n,
         const bool live = i < n;
         k[r] = live ? keys[i] : (K)0;
         v[r] = live ? vals[i] : 0u;
-        const uint32_t digit = live ? ((uint32_t)(k[r] >> shift) & 255u) : 256u + lane;   // dead lanes match nobody
-        const unsigned peers = __match_any_sync(0xffffffffu, digit);
+        const uint32_t digit = live ? ((uint32_t)(k[r] >> shift) & 255u) : 0u;
+        const unsigned peers = same_digit_lanes(digit, live);                             // dead lanes match nobody
         const unsigned rank = __popc(peers & ((1u << lane) - 1u));
         uint32_t before = 0;
         if (live) before = cnt[w][digit];
