@@ -117,3 +117,26 @@ def test_refine_noalloc_rejects_more_cells_than_its_scratch_holds():
     wc, ws, _ = qsl.qsl_refine(lat, 0, None, S, tau)
     torch.cuda.synchronize()
     assert int(m.item()) == 16 and torch.equal(cc, wc) and torch.equal(cs.view(torch.int64), ws.view(torch.int64))
+
+
+@pytest.mark.parametrize("ndim,dims,cap", [(2, (300, 211), 1003), (3, (40, 33, 21), 4097), (2, (300, 211), 0), (3, (40, 33, 21), 5)])
+def test_refine_noalloc_writes_nothing_beyond_capacity(ndim, dims, cap):
+    """Buffers smaller than the child count (qsl.h: "nothing beyond capacity was written"): the first `cap` children are
+    those of the full result - also when the cut falls inside a cell's group of children and inside a tile - the rows
+    behind them stay untouched, child_base and the count are complete."""
+    lat, S, tau = _case(ndim, dims, 11)
+    wc, ws, wb = qsl.qsl_refine(lat, 0, None, S, tau)
+    total = int(wc.shape[0])
+    assert total > cap
+    big_c = torch.full((cap + 64, ndim), -7, dtype=torch.int32, device="cuda")
+    big_s = torch.full((cap + 64, 3), float("nan"), dtype=torch.float64, device="cuda")
+    cb = torch.full((int(S.numel()),), -99, dtype=torch.int64, device="cuda")
+    m = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+    qsl.qsl_refine_noalloc(lat, 0, None, S, tau, big_c[:cap], big_s[:cap], cb, m)
+    torch.cuda.synchronize()
+    assert int(m.item()) == total and torch.equal(cb, wb)
+    assert torch.equal(big_c[:cap], wc[:cap]) and torch.equal(big_s[:cap].view(torch.int64), ws[:cap].view(torch.int64))
+    assert bool((big_c[cap:] == -7).all()) and bool(torch.isnan(big_s[cap:]).all())
+    # the pooled entry point reports the overflow
+    with pytest.raises(qsl.QslError):
+        qsl.qsl_refine(lat, 0, None, S, tau, capacity=cap)
