@@ -53,7 +53,8 @@ NCU_CAPTURES = {
                       "source": "profiles/r2d_cfg4_trace_kernel.md (cfg5 level 0, the L-only launch)"},
 }
 DEFAULT_WORKLOAD = "cfg4"
-SELECT_PASSES = 8          # radix passes of qsl_select (select_refine.cu), for the streaming byte count
+SELECT_PASSES = 3          # passes of qsl_select that read the whole map (select_refine.cu: passes 0 - 2; passes 3 - 7 read the
+                           # candidates kept by pass 2, a few per cent of the map), for the streaming byte count
 SORT_PASSES = 4            # radix passes of the 30-bit seed sort (order.cu)
 
 
@@ -514,7 +515,8 @@ def streaming_block(qsl, torch, W):
     tau = torch.empty(1, dtype=torch.float64, device="cuda")
     passes = SELECT_PASSES
     put("select", best(lambda: qsl.qsl_select(S3.view(-1), 0.95, out=tau)), 8 * N * passes,
-        "order statistic of 6.7e7 values: %d radix passes x 8 B per value" % passes)
+        "order statistic of 6.7e7 values: 8 radix passes of 8 bits, %d of them over the whole map x 8 B per value (the other 5 "
+        "read the candidates pass 2 kept; their data-dependent traffic is not counted)" % passes)
     lat = qi.Lattice(3, (512, 512, 256), (0.0, 0.0, 0.0), (1.0, 0, 0), (0, 1.0, 0), (0, 0, 0.5))
     cap = (N - int(math.ceil(0.95 * N)) + 8) << 3
     m = [0]

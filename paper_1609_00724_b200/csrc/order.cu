@@ -106,8 +106,10 @@ __device__ __forceinline__ unsigned same_digit_lanes(uint32_t digit, bool live)
     return peers;
 }
 
+// 5 CTAs of 256 threads per SM: 48 registers, no spill (un-capped ptxas takes 82 and the sort is 25 % slower; 6 / 8 CTAs
+// spill: profiles/r2g)
 #ifndef QSL_SORT_MINB
-#define QSL_SORT_MINB 1
+#define QSL_SORT_MINB 5
 #endif
 template <typename K>
 __global__ void __launch_bounds__(SORT_THREADS, QSL_SORT_MINB) sort_scatter_kernel(long long n, const K *__restrict__ keys,

@@ -17,6 +17,9 @@ struct SelectState {
     unsigned long long prefix;      // high digits of the answer found so far
     unsigned long long rank;        // 0-based rank still to be located inside the current bucket
     unsigned long long n_finite;
+    unsigned long long n_cand16;    // values that share the answer's top 16 bits (known after pass 1)
+    unsigned int overflow;          // pass 2: some block found more candidates than its segment holds
+    unsigned int pad;
     unsigned int hist[256];
 };
 
@@ -31,23 +34,81 @@ __device__ __forceinline__ double key_to_double(unsigned long long k)
     return __longlong_as_double((long long)b);
 }
 
+// One pass of the radix select: histogram of digit `pass` over the values that share the digits found so far.
+// Passes 0 and 1 read S.  Pass 2 reads S once more and, if no more than `cap` / 2 values share the answer's top 16 bits
+// (sign, exponent, 4 bits of mantissa), also keeps the ordered keys of those values: block b appends the ones it meets to
+// its own segment cand[b seg .. (b + 1) seg) (slots from a counter in shared memory, the count to blk_cnt[b]; no global
+// atomics), and passes 3 - 7 - same grid - read their block's segment instead of S.  For a FLEDGE map the candidates are
+// a few per cent of the values: three reads of S instead of eight.  With more candidates than that (a near-constant
+// map), or if a block's segment overflows, every pass reads S, as before.
 __global__ void __launch_bounds__(256) select_hist_kernel(long long n, const double *__restrict__ S, int pass,
-                                                          SelectState *__restrict__ st)
+                                                          SelectState *__restrict__ st, unsigned long long *__restrict__ cand,
+                                                          unsigned int *__restrict__ blk_cnt, unsigned long long cap)
 {
     __shared__ unsigned int h[256];
+    __shared__ unsigned int s_n;
     h[threadIdx.x] = 0;
+    if (threadIdx.x == 0) s_n = 0;
     __syncthreads();
     const int shift = 56 - 8 * pass;
     const unsigned long long prefix = st->prefix;
+    const bool use_cand = cand != nullptr && 2 * st->n_cand16 <= cap && !st->overflow;   // the same in every thread of the grid
+    const unsigned long long seg = cap / gridDim.x;
+    unsigned long long *__restrict__ mine = cand + (size_t)blockIdx.x * seg;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const double v = S[i];
-        if (!isfinite(v)) continue;
-        const unsigned long long k = ordered_key(v);
-        if (pass == 0 || (k >> (shift + 8)) == (prefix >> (shift + 8))) atomicAdd(&h[(k >> shift) & 255u], 1u);
+    const unsigned lane = threadIdx.x & 31u;
+    if (pass >= 3 && use_cand) {
+        const unsigned m = blk_cnt[blockIdx.x];
+        for (unsigned i = threadIdx.x; i < m; i += blockDim.x) {
+            const unsigned long long k = mine[i];
+            if ((k >> (shift + 8)) == (prefix >> (shift + 8))) atomicAdd(&h[(k >> shift) & 255u], 1u);
+        }
+    } else if (!(pass == 2 && use_cand)) {
+        // plain pass over S (the compiler unrolls it: several loads in flight per thread)
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+            const double v = S[i];
+            if (!isfinite(v)) continue;
+            const unsigned long long k = ordered_key(v);
+            if (pass == 0 || (k >> (shift + 8)) == (prefix >> (shift + 8))) atomicAdd(&h[(k >> shift) & 255u], 1u);
+        }
+    } else {
+        // pass 2 with compaction
+        // warp-uniform loop bounds (every lane of a warp takes part in the vote of the compaction); four loads in
+        // flight per thread (the vote keeps the compiler from unrolling the loop itself)
+        constexpr int U = 4;
+        const double qnan = __longlong_as_double(0x7ff8000000000000ll);
+        for (long long b = (long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); b < n; b += U * stride) {
+            double v[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) { const long long i = b + u * stride + lane; v[u] = i < n ? S[i] : qnan; }
+            unsigned long long k[U]; unsigned m[U]; unsigned tot = 0;
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                k[u] = ordered_key(v[u]);
+                const bool match = isfinite(v[u]) && (k[u] >> (shift + 8)) == (prefix >> (shift + 8));
+                if (match) atomicAdd(&h[(k[u] >> shift) & 255u], 1u);
+                m[u] = __ballot_sync(0xffffffffu, match);
+                tot += __popc(m[u]);
+            }
+            if (tot) {                                   // one slot request per warp and trip
+                unsigned slot = 0;
+                if (lane == 0) slot = atomicAdd(&s_n, tot);
+                slot = __shfl_sync(0xffffffffu, slot, 0);
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const unsigned at = slot + __popc(m[u] & ((1u << lane) - 1u));
+                    if (((m[u] >> lane) & 1u) && at < seg) mine[at] = k[u];
+                    slot += __popc(m[u]);
+                }
+            }
+        }
     }
     __syncthreads();
     if (h[threadIdx.x]) atomicAdd(&st->hist[threadIdx.x], h[threadIdx.x]);
+    if (pass == 2 && use_cand && threadIdx.x == 0) {
+        blk_cnt[blockIdx.x] = s_n;
+        if (s_n > seg) atomicExch(&st->overflow, 1u);
+    }
 }
 
 __global__ void __launch_bounds__(256) select_pick_kernel(int pass, double p, SelectState *__restrict__ st, double *__restrict__ tau)
@@ -70,6 +131,7 @@ __global__ void __launch_bounds__(256) select_pick_kernel(int pass, double p, Se
         const int shift = 56 - 8 * pass;
         st->prefix |= (unsigned long long)threadIdx.x << shift;
         st->rank = rank - before;
+        if (pass == 1) st->n_cand16 = mine;
     }
     st->hist[threadIdx.x] = 0;
     __syncthreads();
@@ -209,22 +271,31 @@ extern "C" int qsl_select(long long n, const double *S, double p, double *tau, v
 {
     if (n < 0 || (n > 0 && !S) || !tau || !(p >= 0.0 && p <= 1.0)) return QSL_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
-    void *stp = nullptr;
+    void *stp = nullptr, *cand = nullptr;
     int rc = scratch_alloc(&stp, sizeof(SelectState), s);
     if (rc != QSL_OK) return rc;
+    long long blocks = (n + 255) / 256;
+    const long long cap_blocks = (long long)sm_count() * 8;
+    if (blocks > cap_blocks) blocks = cap_blocks;
+    if (blocks < 1) blocks = 1;
+    // candidate buffer of pass 2: room for a quarter of the values in one segment per block (+ the blocks' counts); a map
+    // with more candidates than half of that keeps reading S
+    const unsigned long long cap = n >= 65536 ? (unsigned long long)(n / 4) : 0ull;
+    if (cap) {
+        rc = scratch_alloc(&cand, sizeof(unsigned long long) * (size_t)cap + sizeof(unsigned int) * (size_t)blocks, s);
+        if (rc != QSL_OK) { scratch_free(stp, s); return rc; }
+    }
+    unsigned int *blk_cnt = cand ? (unsigned int *)((unsigned long long *)cand + cap) : nullptr;
     SelectState *st = (SelectState *)stp;
     cudaError_t e = cudaMemsetAsync(st, 0, sizeof(SelectState), s);
-    long long blocks = (n + 255) / 256;
-    const long long cap = (long long)sm_count() * 8;
-    if (blocks > cap) blocks = cap;
-    if (blocks < 1) blocks = 1;
     for (int pass = 0; pass < 8 && e == cudaSuccess; ++pass) {
         count_launch();
-        select_hist_kernel<<<(unsigned)blocks, 256, 0, s>>>(n, S, pass, st);
+        select_hist_kernel<<<(unsigned)blocks, 256, 0, s>>>(n, S, pass, st, (unsigned long long *)cand, blk_cnt, cap);
         count_launch();
         select_pick_kernel<<<1, 256, 0, s>>>(pass, p, st, tau);
         e = cudaGetLastError();
     }
+    scratch_free(cand, s);
     scratch_free(stp, s);
     if (e != cudaSuccess) return record_cuda(e);
     return QSL_OK;

@@ -67,6 +67,42 @@ def test_select_negative_values_and_all_nan():
     assert math.isnan(float(qsl.qsl_select(_cuda(np.full(10, np.nan)), 0.95).item()))
 
 
+@pytest.mark.parametrize("kind", ["fledge_like", "constant", "two_values", "one_block", "negative", "tiny_bucket"])
+def test_select_candidate_compaction_paths(kind):
+    """qsl_select on maps large enough for the candidate compaction of pass 2 (n >= 65536), chosen so that every branch
+    runs: candidates kept (fledge_like, tiny_bucket, negative), too many candidates -> every pass reads S (constant,
+    two_values), candidates of the answer's bucket all in the elements of ONE block of the grid-stride loop -> its
+    segment overflows -> fallback (one_block).  Exact against the sorted definition (nearest rank)."""
+    rng = np.random.default_rng(35)
+    n = (1 << 22) + 777
+    if kind == "fledge_like":
+        S = np.abs(rng.normal(10.0, 3.0, size=n)); S[rng.random(n) < 0.01] = np.nan
+        ps = (0.95, 0.5, 0.001)
+    elif kind == "constant":
+        S = np.full(n, 3.25); ps = (0.95, 0.0, 1.0)
+    elif kind == "two_values":
+        S = np.where(rng.random(n) < 0.5, 1.5, 1.5 + 2.0 ** -40); ps = (0.95, 0.25, 0.5)
+    elif kind == "negative":
+        S = -np.abs(rng.normal(10.0, 3.0, size=n)); S[::5] = rng.normal(size=len(S[::5])); ps = (0.95, 0.05, 0.5)
+    elif kind == "tiny_bucket":
+        S = rng.uniform(100.0, 200.0, size=n); S[:40] = 1.0 + np.arange(40) * 2.0 ** -45; ps = (5e-6, 9.5e-6, 0.95)
+    else:
+        # the smallest values (one 16-bit bucket: [1, 1.0625)) sit only where block 0 of the grid-stride loop reads
+        blocks = torch.cuda.get_device_properties(0).multi_processor_count * 8
+        stride = blocks * 256
+        S = rng.uniform(100.0, 200.0, size=n)
+        idx = np.arange(n)
+        own = (idx % stride) < 256
+        S[own] = 1.0 + rng.random(int(own.sum())) * 0.0624
+        assert own.sum() > (n // 4) // blocks                      # more than one segment holds
+        ps = (0.5 * own.sum() / n, 0.95, 1e-7)
+    d = _cuda(S)
+    for p in ps:
+        tau = float(qsl.qsl_select(d, p).item())
+        ref = oracle.select(S, p)
+        assert (math.isnan(tau) and math.isnan(ref)) or tau == ref, (kind, p, tau, ref)
+
+
 @pytest.mark.parametrize("ndim", [2, 3])
 def test_refine_bit_exact_two_levels(ndim):
     rng = np.random.default_rng(34)
