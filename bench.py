@@ -85,21 +85,24 @@ class ClockSampler:
         except Exception:
             self.nv = None
 
-    def _loop(self):
+    def _sample(self):
         nv = self.nv
+        try:
+            with self.enqueue_lock:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+            for bit, name in {**self.BAD, **self.NOTE}.items():
+                if r & bit:
+                    self.reasons.add(name)
+        except Exception:
+            pass
+
+    def _loop(self):
         while not self._stop.is_set():
-            try:
-                with self.enqueue_lock:
-                    self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
-                    try:
-                        r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
-                    except Exception:
-                        r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                for bit, name in {**self.BAD, **self.NOTE}.items():
-                    if r & bit:
-                        self.reasons.add(name)
-            except Exception:
-                pass
+            self._sample()
             self._stop.wait(0.1)
 
     def __enter__(self):
@@ -112,11 +115,19 @@ class ClockSampler:
         self._stop.set()
         if self._t is not None:
             self._t.join(timeout=2)
+            # a timed region shorter than the sampling period (cfg1: 2 ms) can end before the first sample: take one now,
+            # right behind the last timed kernel (`at_end` in the summary says so)
+            self.at_end = not self.samples
+            if self.at_end:
+                self._sample()
 
     def summary(self):
         s = sorted(self.samples)
-        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(s)}
+        out = {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+               "samples": len(s)}
+        if getattr(self, "at_end", False):
+            out["at_end"] = True
+        return out
 
 
 # ---------------------------------------------------------------------------------------------------------------------
