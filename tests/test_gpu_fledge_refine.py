@@ -47,6 +47,38 @@ def test_fledge_dense_full_size_sampled():
         assert np.abs(S - ref).max() <= 1e-12
 
 
+@pytest.mark.parametrize("shape", [(16384, 16384), (512, 1024, 1024)])
+def test_fledge_dense_more_tasks_than_the_grid_sampled(shape):
+    """Maps with more strips x bands (x chunks) than the dense kernels launch CTAs (a few waves of single-warp CTAs per SM),
+    so that their task loops stride: sub-blocks (corners, edges, interior, across band / chunk borders) against the
+    oracle run on the sub-block with one halo cell (the Sobel stencil reaches no further; at the map's edge the
+    sub-block's own edge replication is the map's)."""
+    g = torch.Generator(device="cuda"); g.manual_seed(36)
+    L = torch.rand(shape, dtype=torch.float64, device="cuda", generator=g) * 3.0 + 0.1
+    nd = len(shape)
+    L.view(-1)[12345] = float("nan")
+    S = qsl.qsl_fledge_dense(L, nd)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(37)
+    ext = 40 if nd == 2 else 12
+    starts = [tuple(0 for _ in shape), tuple(n - ext for n in shape)]
+    starts += [tuple(int(rng.integers(0, n - ext)) for n in shape) for _ in range(6)]
+    starts += [tuple(min(max(v, 0), n - ext) for v, n in zip((60, 25) if nd == 2 else (58, 1, 25), shape))]   # band / chunk borders
+    if nd == 2:
+        starts.append((max(12345 // shape[1] - 3, 0), max(12345 % shape[1] - 3, 0)))                        # around the NaN
+    for st in starts:
+        lo = [max(a - 1, 0) for a in st]
+        hi = [min(a + ext + 1, n) for a, n in zip(st, shape)]
+        sl = tuple(slice(a, b) for a, b in zip(lo, hi))
+        ref = oracle.fledge_dense(L[sl].cpu().numpy(), nd)
+        inner = tuple(slice(a - l, a - l + ext) for a, l in zip(st, lo))
+        got = S[tuple(slice(a, a + ext) for a in st)].cpu().numpy()
+        want = ref[inner]
+        assert np.array_equal(np.isnan(got), np.isnan(want)), st
+        ok = ~np.isnan(want)
+        assert np.abs(got[ok] - want[ok]).max() <= 1e-12, st
+
+
 @pytest.mark.parametrize("n", [1, 2, 19, 255, 256, 257, 4097, 1 << 20])
 def test_select_exact(n):
     rng = np.random.default_rng(32)
