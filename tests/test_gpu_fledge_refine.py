@@ -185,6 +185,25 @@ def test_radix_sort_pairs_stable(n, bits):
     assert np.array_equal(v.cpu().numpy().view(np.uint32), vals[order])
 
 
+@pytest.mark.parametrize("kind", ["all_equal", "sorted", "reversed", "three_values", "runs_of_40", "one_odd_lane"])
+def test_radix_sort_pairs_structured_keys(kind):
+    """Keys as a seed lattice produces them - long runs of one digit, whole warps with the same digit, a single lane that
+    differs - through the warp-vote ranking of the scatter kernel; stable, bit-exact against numpy."""
+    n = 70001
+    i = np.arange(n, dtype=np.uint32)
+    keys = {"all_equal": np.full(n, 0x2a5a5a5a, dtype=np.uint32), "sorted": i * 3, "reversed": (n - i) * 5,
+            "three_values": np.array([7, 0x10007, 0x3fffffff], dtype=np.uint32)[i % 3], "runs_of_40": (i // 40) * 0x01010101 % (1 << 30),
+            "one_odd_lane": np.where(i % 32 == 17, 0x12345, 0x12344).astype(np.uint32)}[kind].astype(np.uint32)
+    vals = np.arange(n, dtype=np.uint32)
+    k = _cuda(keys.view(np.int32)); v = _cuda(vals.view(np.int32))
+    rc = qsl.lib().qsl_debug_sort_pairs(C.c_void_p(k.data_ptr()), C.c_void_p(v.data_ptr()), C.c_longlong(n), C.c_int(30),
+                                        C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    assert rc == 0
+    order = np.argsort(keys, kind="stable")
+    assert np.array_equal(k.cpu().numpy().view(np.uint32), keys[order])
+    assert np.array_equal(v.cpu().numpy().view(np.uint32), vals[order])
+
+
 @pytest.mark.parametrize("name,scale", [("cfg3", 1 / 16), ("cfg5", 1 / 16)])
 def test_level_loop_stagewise_against_oracle(name, scale):
     """a9: every stage of the level loop fed with the ORACLE's products of the previous stage."""
