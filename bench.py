@@ -559,6 +559,25 @@ def streaming_block(qsl, torch, W):
     t_copy = best(lambda: (k2.copy_(keys), v2.copy_(vals)))
     put("radix_sort_pairs", best(sort) - t_copy, n * 8 * 2 * SORT_PASSES + n * 4 * SORT_PASSES,
         "6.7e7 (key, index) pairs, 30-bit keys: %d passes x (histogram read 4 B + scatter read 8 B + write 8 B)" % SORT_PASSES)
+    # the same sort on the keys the path really sees: Morton codes of a 512 x 512 x 256 seed lattice in index order (27 bits)
+    def spread3(v):
+        v = v & 0x3ff
+        v = (v | (v << 16)) & 0x030000ff
+        v = (v | (v << 8)) & 0x0300f00f
+        v = (v | (v << 4)) & 0x030c30c3
+        return (v | (v << 2)) & 0x09249249
+    idx = torch.arange(n, dtype=torch.int64, device="cuda")
+    keys.copy_((spread3(idx % 512) | (spread3((idx // 512) % 512) << 1) | (spread3(idx // (512 * 512)) << 2)).to(torch.int32))
+    del idx
+
+    def sort_lattice():
+        k2.copy_(keys); v2.copy_(vals)
+        rc = qsl.lib().qsl_debug_sort_pairs(C.c_void_p(k2.data_ptr()), C.c_void_p(v2.data_ptr()), C.c_longlong(n), C.c_int(27),
+                                            C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        assert rc == 0
+    put("radix_sort_pairs_lattice_keys", best(sort_lattice) - t_copy, n * 8 * 2 * SORT_PASSES + n * 4 * SORT_PASSES,
+        "the same sort on the Morton keys of a 512 x 512 x 256 seed lattice in index order (what qsl_trace sorts): long runs "
+        "per digit, %d passes" % SORT_PASSES)
     del keys, vals, k2, v2
     # field pack + per-cell table: the whole qsl_field_create call of this run's workload (allocation included), warm
     g = W.cfg["grid"]
