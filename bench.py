@@ -542,7 +542,8 @@ def streaming_block(qsl, torch, W):
     cc, cs, cb = qsl.qsl_refine(lat, 0, None, S3.view(-1), tau, capacity=cap)
     L1 = torch.rand(cc.shape[0], dtype=torch.float64, device="cuda", generator=gen) + 0.1
     put("fledge_sparse_3d", best(lambda: qsl.qsl_fledge_sparse(lat, 1, L3.view(-1), [None, cc], [None, L1], [cb])),
-        int(cc.shape[0]) * (12 + 8 + 8), "level-1 cells: 12 B coords + 8 B L in, 8 B out per cell (27 ancestor look-ups from L2)")
+        int(cc.shape[0]) * (12 + 8 + 8), "level-1 cells: 12 B coords + 8 B L in, 8 B out per cell; 8 ancestor walks + 27 look-ups per cell: bound by the L1 "
+        "wavefront rate of these gathers (83 % of it by ncu, profiles/r2g), not by HBM")
     del L3, S3, L2, L1, cc, cs, cb
     # seed ordering: Morton keys + radix sort of (key, index) pairs, as qsl_trace does it; measured through the test hook
     n = 1 << 26
